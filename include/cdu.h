@@ -1,0 +1,140 @@
+/* cdu.h - C ABI of the conic deep-unfolding hot path (batched, unrolled COSMO ADMM, forward + backward)
+ *
+ * Problem statement (Eq. 1):   min 1/2 x'Px + q'x   s.t.  Ax + s = b,  s in K,
+ * K a Cartesian product of zero / nonnegative / second-order / PSD cones.
+ *
+ * One iteration (Eq. 3a-3e L60-72 in the indirect form Eq. 4; sign convention "y in K*",
+ * DESIGN.md reading A1, so that r_p = Ax+s-b and r_d = Px+q+A'y as printed in Eq. 12):
+ *     xi = sigma x - q + A'(rho (b - s) - y)
+ *     xt = M^-1 xi,  M = P + sigma I + rho A'A      (matrix-free Jacobi-preconditioned CG, L80, L294)
+ *     st = b - A xt
+ *     x+ = alpha xt + (1-alpha) x ;  w = alpha st + (1-alpha) s - y/rho
+ *     s+ = Pi_K(w)                                   (PSD blocks: eigendecomposition, clamp, rebuild, Eq. 7)
+ *     y+ = rho (s+ - w)
+ * Backward: BPTT over the stored iterates; adjoint CG on the same M and grad_rho = (A lam) o (A xt)
+ * (Eq. 5-6); Dalecki-Krein VJP for the PSD projection (Eq. 9-10).
+ *
+ * Conventions
+ *   - svec: upper triangle, column by column, off-diagonals scaled by sqrt(2).
+ *   - SOC_d = {(t,u): ||u||_2 <= t}, t first.
+ *   - All floating-point arrays crossing this ABI have the handle's dtype (float for CDU_F32, double for
+ *     CDU_F64). Internally the iterate and all reductions are fp64; CG, eig and DK run in the handle's dtype.
+ *   - No function throws or aborts; every error is a return code, cdu_last_error() gives the text.
+ *   - Thread safety: one handle may be used from one host thread at a time.
+ */
+#ifndef CDU_H_
+#define CDU_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cdu_handle_s* cdu_handle; /* opaque; owns device copies of the problem, scratch and the checkpoint store */
+
+typedef enum { CDU_OK = 0, CDU_EINVAL = 1, CDU_ENOMEM = 2, CDU_ECUDA = 3, CDU_ESTATE = 4, CDU_ENUMERIC = 5 } cdu_status;
+typedef enum { CDU_F32 = 0, CDU_F64 = 1 } cdu_dtype;
+typedef enum { CDU_ZERO = 0, CDU_NONNEG = 1, CDU_SOC = 2, CDU_PSD = 3 } cdu_cone_kind;
+typedef enum { CDU_RHO_PER_ITER = 0,    /* rho[K], alpha[K] shared by the batch; g_rho[K], g_alpha[K], g_sigma[1] are batch sums */
+               CDU_RHO_PER_PROBLEM = 1  /* rho[K][B], alpha[K][B]; g_rho[K][B], g_alpha[K][B], g_sigma[B] */
+} cdu_rho_mode;
+typedef enum { CDU_CKPT_FULL = 0, /* store z^k plus x-tilde, s-tilde and (U, lambda) of every PSD block            */
+               CDU_CKPT_LEAN = 1  /* store z^k only ((n+2m) doubles per iteration); backward re-solves and re-factors */
+} cdu_ckpt_mode;
+
+/* dim = number of rows for ZERO / NONNEG / SOC (SOC: t first); for PSD the matrix order p, rows = p(p+1)/2 */
+typedef struct { int32_t kind; int32_t dim; } cdu_cone;
+
+/* A batch of `batch` independent instances, block-diagonal batched CSR (the paper's "super-batch", L306).
+ * All arrays below are HOST memory and are copied by cdu_create; the caller may free them on return. */
+typedef struct {
+  int32_t batch;
+  int32_t dtype;            /* cdu_dtype of A_val, P_val, q, b and of every array passed to forward/backward */
+  const int64_t* var_off;   /* [batch+1] offsets of x:  n_b = var_off[b+1]-var_off[b]                       */
+  const int64_t* row_off;   /* [batch+1] offsets of the constraint rows: m_b                                */
+  const int64_t* A_rowptr;  /* [sum m_b + 1] global nnz offsets                                              */
+  const int32_t* A_colidx;  /* [nnz A] column index LOCAL to the problem, 0..n_b-1, sorted within a row      */
+  const void*    A_val;     /* [nnz A]                                                                       */
+  const int64_t* P_rowptr;  /* [sum n_b + 1]; P in FULL symmetric storage (both triangles); may hold 0 nnz   */
+  const int32_t* P_colidx;
+  const void*    P_val;
+  const void*    q;         /* [sum n_b] */
+  const void*    b;         /* [sum m_b] */
+  const int64_t* cone_off;  /* [batch+1] into cones[]; the cones of a problem tile its rows in order         */
+  const cdu_cone* cones;
+} cdu_problem;
+
+typedef struct {
+  double  cg_tol;           /* stop when ||xi - M xt||_2 <= cg_tol ||xi||_2; <= 0: 1e-10 (F64) / 1e-6 (F32)     */
+  int32_t cg_max_iter;      /* <= 0: 2 n + 50                                                                   */
+  int32_t K_max;            /* capacity of the checkpoint store (largest K a forward call may use)              */
+  int32_t ckpt_mode;        /* cdu_ckpt_mode                                                                    */
+  int32_t cg_refine;        /* extra passes of fp64-residual iterative refinement around the CG solve;
+                               < 0: default (1 for F32, 0 for F64)                                              */
+  double  cg_refine_tol;    /* each refinement pass reduces the true residual by this factor; <= 0: 1e-4        */
+  int32_t psd_small_max;    /* PSD blocks of order <= this run in the shared-memory Jacobi kernel, larger ones in
+                               the global-memory path; <= 0: default (128 for F32, 88 for F64)                  */
+  int32_t use_tensor_cores; /* large-block rebuild / DK products: 1 = tcgen05 3xTF32 GEMM, 0 = fp32 FMA GEMM;
+                               < 0: default                                                                     */
+} cdu_options;
+
+/* Copies and re-packs the batch onto the current CUDA device (transposed copy of A, diag(P), column square
+ * sums for the Jacobi preconditioner, cone tables) and allocates scratch and the checkpoint store.
+ * `opts` may be NULL (defaults, K_max = 0 is invalid). Returns CDU_EINVAL on malformed input (cones not tiling
+ * the rows, indices out of range, non-symmetric pattern is NOT checked), CDU_ENOMEM / CDU_ECUDA otherwise. */
+cdu_status cdu_create(const cdu_problem* prob, const cdu_options* opts, void* cuda_stream, cdu_handle* out);
+
+/* K unrolled iterations from (x0, s0, y0) (NULL = zeros). rho, alpha: hyper-parameters, layout per rho_mode.
+ * xK, sK, yK (each may be NULL) receive z^K. If io_on_host == 0 all pointers are DEVICE pointers, borrowed for the
+ * stream-ordered work, and the call returns without synchronising. If io_on_host != 0 they are HOST pointers
+ * (pinned memory recommended); the library stages them through its own device buffers and returns after the
+ * results have landed (stream synchronised).
+ * Errors: CDU_EINVAL (K < 1, K > K_max, sigma <= 0, NULL rho/alpha; host-side rho <= 0 or alpha outside (0,2)). */
+cdu_status cdu_forward(cdu_handle h, int32_t K, const void* rho, int32_t rho_mode, double sigma, const void* alpha,
+                       const void* x0, const void* s0, const void* y0,
+                       void* xK, void* sK, void* yK, int32_t io_on_host, void* cuda_stream);
+
+/* Reverse sweep of the last cdu_forward on this handle (CDU_ESTATE if there was none); may be called repeatedly
+ * with different cotangents. g_xK, g_sK, g_yK: dL/d(x_K, s_K, y_K) (NULL = zeros). Outputs (each may be NULL):
+ * g_rho, g_alpha (layout of the forward's rho_mode), g_sigma ([1] or [B]), g_x0, g_s0, g_y0. */
+cdu_status cdu_backward(cdu_handle h, const void* g_xK, const void* g_sK, const void* g_yK,
+                        void* g_rho, void* g_sigma, void* g_alpha, void* g_x0, void* g_s0, void* g_y0,
+                        int32_t io_on_host, void* cuda_stream);
+
+typedef struct {
+  int64_t cg_iters_fwd;      /* CG iterations summed over problems and iterations, last forward            */
+  int64_t cg_iters_bwd;      /* same for the adjoint solves (and LEAN re-solves) of the last backward       */
+  int32_t cg_iters_max;      /* largest single-solve count                                                  */
+  int32_t eig_sweeps_max;    /* largest Jacobi sweep count of a PSD block                                   */
+  int32_t n_flagged;         /* problems with a flag set (CG cap hit, non-positive curvature, sweep cap, NaN) */
+  int32_t flags_or;          /* OR of all per-problem flag words: 1 CG cap, 2 pAp<=0, 4 eig sweep cap, 8 non-finite */
+  int64_t device_bytes;      /* bytes of device memory owned by the handle                                  */
+  int64_t ckpt_bytes;        /* of which checkpoint store                                                   */
+  int64_t launches;          /* kernel launches issued by the handle since creation                         */
+} cdu_stats;
+
+/* Synchronises the stream of the last call and reads back the per-problem counters. */
+cdu_status cdu_get_stats(cdu_handle h, cdu_stats* out);
+
+/* Copies iterate z^k (0 <= k <= K of the last forward) into caller buffers (device or host per io_on_host). */
+cdu_status cdu_get_iterate(cdu_handle h, int32_t k, void* x, void* s, void* y, int32_t io_on_host, void* cuda_stream);
+
+const char* cdu_last_error(cdu_handle h); /* valid until the next call on h; h may be NULL (create errors) */
+cdu_status  cdu_destroy(cdu_handle h);
+const char* cdu_version(void);
+
+/* ---- stand-alone operator entry points (unit tests, micro-benchmarks, ncu isolation) ------------------------
+ * Batched PSD projection S -> Pi(S) = U max(L,0) U' (Eq. 7) and its Dalecki-Krein VJP (Eq. 9-10) on `count`
+ * dense symmetric p x p matrices (row-major, device pointers, dtype as given). `path`: 0 auto, 1 shared-memory
+ * Jacobi, 2 global-memory path. U (row-major, eigenvectors in columns) and lam may be NULL for the projection;
+ * the VJP reads them. */
+cdu_status cdu_psd_project(int32_t dtype, int32_t count, int32_t p, const void* S, void* PiS, void* U, void* lam,
+                           int32_t path, int32_t use_tensor_cores, void* cuda_stream);
+cdu_status cdu_psd_vjp(int32_t dtype, int32_t count, int32_t p, const void* U, const void* lam, const void* Gbar,
+                       void* Sbar, int32_t path, int32_t use_tensor_cores, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CDU_H_ */

@@ -1,0 +1,261 @@
+"""paper_2606_13825_b200 - thin Python binding of the cdu C ABI (include/cdu.h).
+
+Argument marshalling only: every step of the hot path (CSR SpMV / PCG, relaxation, cone projections incl.
+the PSD eigendecomposition, checkpointing, adjoint CG, Dalecki-Krein VJP) runs in the CUDA kernels of
+`csrc/` behind `libcdu.so`. PyTorch is used for device memory and streams only. There is no CPU fallback:
+if the library is missing or no CUDA device is present, the calls raise.
+
+Names follow the C ABI: `cdu_create`, `cdu_forward`, `cdu_backward`, `cdu_get_stats`, `cdu_destroy`,
+`cdu_psd_project`, `cdu_psd_vjp`.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libcdu.so")
+
+CDU_OK, CDU_EINVAL, CDU_ENOMEM, CDU_ECUDA, CDU_ESTATE, CDU_ENUMERIC = range(6)
+CDU_F32, CDU_F64 = 0, 1
+CDU_ZERO, CDU_NONNEG, CDU_SOC, CDU_PSD = 0, 1, 2, 3
+CDU_RHO_PER_ITER, CDU_RHO_PER_PROBLEM = 0, 1
+CDU_CKPT_FULL, CDU_CKPT_LEAN = 0, 1
+_STATUS = {0: "CDU_OK", 1: "CDU_EINVAL", 2: "CDU_ENOMEM", 3: "CDU_ECUDA", 4: "CDU_ESTATE", 5: "CDU_ENUMERIC"}
+
+EXPORTED_SYMBOLS = ("cdu_create", "cdu_forward", "cdu_backward", "cdu_get_stats", "cdu_get_iterate", "cdu_last_error",
+                    "cdu_destroy", "cdu_version", "cdu_psd_project", "cdu_psd_vjp")
+
+
+class CduError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"{_STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+class _Cone(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("dim", C.c_int32)]
+
+
+class _Problem(C.Structure):
+    _fields_ = [("batch", C.c_int32), ("dtype", C.c_int32),
+                ("var_off", C.c_void_p), ("row_off", C.c_void_p),
+                ("A_rowptr", C.c_void_p), ("A_colidx", C.c_void_p), ("A_val", C.c_void_p),
+                ("P_rowptr", C.c_void_p), ("P_colidx", C.c_void_p), ("P_val", C.c_void_p),
+                ("q", C.c_void_p), ("b", C.c_void_p), ("cone_off", C.c_void_p), ("cones", C.c_void_p)]
+
+
+class _Options(C.Structure):
+    _fields_ = [("cg_tol", C.c_double), ("cg_max_iter", C.c_int32), ("K_max", C.c_int32), ("ckpt_mode", C.c_int32),
+                ("cg_refine", C.c_int32), ("cg_refine_tol", C.c_double), ("psd_small_max", C.c_int32),
+                ("use_tensor_cores", C.c_int32)]
+
+
+class _Stats(C.Structure):
+    _fields_ = [("cg_iters_fwd", C.c_int64), ("cg_iters_bwd", C.c_int64), ("cg_iters_max", C.c_int32),
+                ("eig_sweeps_max", C.c_int32), ("n_flagged", C.c_int32), ("flags_or", C.c_int32),
+                ("device_bytes", C.c_int64), ("ckpt_bytes", C.c_int64), ("launches", C.c_int64)]
+
+
+_lib = None
+
+
+def load_library(path: Optional[str] = None) -> C.CDLL:
+    """dlopen libcdu.so (no compute happens here; works without a GPU)."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    p = path or LIB_PATH
+    if not os.path.exists(p):
+        raise CduError(CDU_ECUDA, f"{p} not found - run `python -m paper_2606_13825_b200.build` (there is no CPU fallback)")
+    lib = C.CDLL(p)
+    vp, i32, f64 = C.c_void_p, C.c_int32, C.c_double
+    lib.cdu_create.restype = i32
+    lib.cdu_create.argtypes = [C.POINTER(_Problem), C.POINTER(_Options), vp, C.POINTER(vp)]
+    lib.cdu_forward.restype = i32
+    lib.cdu_forward.argtypes = [vp, i32, vp, i32, f64, vp, vp, vp, vp, vp, vp, vp, i32, vp]
+    lib.cdu_backward.restype = i32
+    lib.cdu_backward.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i32, vp]
+    lib.cdu_get_stats.restype = i32
+    lib.cdu_get_stats.argtypes = [vp, C.POINTER(_Stats)]
+    lib.cdu_get_iterate.restype = i32
+    lib.cdu_get_iterate.argtypes = [vp, i32, vp, vp, vp, i32, vp]
+    lib.cdu_last_error.restype = C.c_char_p
+    lib.cdu_last_error.argtypes = [vp]
+    lib.cdu_destroy.restype = i32
+    lib.cdu_destroy.argtypes = [vp]
+    lib.cdu_version.restype = C.c_char_p
+    lib.cdu_version.argtypes = []
+    lib.cdu_psd_project.restype = i32
+    lib.cdu_psd_project.argtypes = [i32, i32, i32, vp, vp, vp, vp, i32, i32, vp]
+    lib.cdu_psd_vjp.restype = i32
+    lib.cdu_psd_vjp.argtypes = [i32, i32, i32, vp, vp, vp, vp, i32, i32, vp]
+    if path is None:
+        _lib = lib
+    return lib
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _ptr(t) -> Optional[int]:
+    """Address of a torch tensor (device or pinned host) or numpy array; None passes NULL."""
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        assert t.flags["C_CONTIGUOUS"]
+        return t.ctypes.data
+    assert t.is_contiguous()
+    return t.data_ptr()
+
+
+def _stream() -> int:
+    return _torch().cuda.current_stream().cuda_stream
+
+
+class Handle:
+    """Owns a `cdu_handle`. `packed` is the dict of `workloads.pack_batch` (host numpy arrays)."""
+
+    def __init__(self, packed: dict, K_max: int, ckpt_mode: int = CDU_CKPT_FULL, cg_tol: float = 0.0,
+                 cg_max_iter: int = 0, cg_refine: int = -1, cg_refine_tol: float = 0.0, psd_small_max: int = 0,
+                 use_tensor_cores: int = -1):
+        torch = _torch()
+        if not torch.cuda.is_available():
+            raise CduError(CDU_ECUDA, "no CUDA device (there is no CPU fallback)")
+        self.lib = load_library()
+        self.dtype = packed["dtype"]
+        self.np_dtype = np.float32 if self.dtype == "f32" else np.float64
+        self.torch_dtype = torch.float32 if self.dtype == "f32" else torch.float64
+        self.B = int(packed["batch"])
+        self.N = int(packed["var_off"][-1])
+        self.M = int(packed["row_off"][-1])
+        keep = {k: np.ascontiguousarray(packed[k]) for k in
+                ("var_off", "row_off", "A_rowptr", "A_colidx", "A_val", "P_rowptr", "P_colidx", "P_val", "q", "b",
+                 "cone_off", "cones")}
+        assert keep["A_val"].dtype == self.np_dtype and keep["q"].dtype == self.np_dtype
+        assert keep["var_off"].dtype == np.int64 and keep["A_colidx"].dtype == np.int32 and keep["cones"].dtype == np.int32
+        pr = _Problem(batch=self.B, dtype=CDU_F32 if self.dtype == "f32" else CDU_F64,
+                      **{k: v.ctypes.data for k, v in keep.items()})
+        op = _Options(cg_tol=cg_tol, cg_max_iter=cg_max_iter, K_max=K_max, ckpt_mode=ckpt_mode, cg_refine=cg_refine,
+                      cg_refine_tol=cg_refine_tol, psd_small_max=psd_small_max, use_tensor_cores=use_tensor_cores)
+        h = C.c_void_p()
+        st = self.lib.cdu_create(C.byref(pr), C.byref(op), _stream(), C.byref(h))
+        if st != CDU_OK:
+            raise CduError(st, self.lib.cdu_last_error(None).decode())
+        self.h = h
+        self.K_max = K_max
+        self.K = 0
+        self.rho_mode = CDU_RHO_PER_ITER
+
+    def _check(self, st: int):
+        if st != CDU_OK:
+            raise CduError(st, self.lib.cdu_last_error(self.h).decode())
+
+    def forward(self, K, rho, alpha, sigma, x0=None, s0=None, y0=None, rho_mode=CDU_RHO_PER_ITER, out=None, host=False):
+        """cdu_forward. Device mode: torch CUDA tensors in, returns (xK, sK, yK) CUDA tensors.
+        Host mode: pinned torch CPU tensors / numpy arrays in and out (copies are inside the call)."""
+        torch = _torch()
+        if out is None:
+            if host:
+                out = tuple(torch.empty(n, dtype=self.torch_dtype).pin_memory() for n in (self.N, self.M, self.M))
+            else:
+                out = tuple(torch.empty(n, dtype=self.torch_dtype, device="cuda") for n in (self.N, self.M, self.M))
+        self._check(self.lib.cdu_forward(self.h, K, _ptr(rho), rho_mode, float(sigma), _ptr(alpha), _ptr(x0), _ptr(s0),
+                                         _ptr(y0), _ptr(out[0]), _ptr(out[1]), _ptr(out[2]), 1 if host else 0, _stream()))
+        self.K, self.rho_mode = K, rho_mode
+        return out
+
+    def backward(self, g_xK=None, g_sK=None, g_yK=None, out=None, host=False):
+        """cdu_backward -> dict(g_rho, g_alpha, g_sigma, g_x0, g_s0, g_y0)."""
+        torch = _torch()
+        cnt = self.K * (self.B if self.rho_mode == CDU_RHO_PER_PROBLEM else 1)
+        scnt = self.B if self.rho_mode == CDU_RHO_PER_PROBLEM else 1
+        if out is None:
+            sizes = dict(g_rho=cnt, g_alpha=cnt, g_sigma=scnt, g_x0=self.N, g_s0=self.M, g_y0=self.M)
+            if host:
+                out = {k: torch.empty(n, dtype=self.torch_dtype).pin_memory() for k, n in sizes.items()}
+            else:
+                out = {k: torch.empty(n, dtype=self.torch_dtype, device="cuda") for k, n in sizes.items()}
+        self._check(self.lib.cdu_backward(self.h, _ptr(g_xK), _ptr(g_sK), _ptr(g_yK), _ptr(out.get("g_rho")),
+                                          _ptr(out.get("g_sigma")), _ptr(out.get("g_alpha")), _ptr(out.get("g_x0")),
+                                          _ptr(out.get("g_s0")), _ptr(out.get("g_y0")), 1 if host else 0, _stream()))
+        return out
+
+    def iterate(self, k: int):
+        torch = _torch()
+        out = tuple(torch.empty(n, dtype=self.torch_dtype, device="cuda") for n in (self.N, self.M, self.M))
+        self._check(self.lib.cdu_get_iterate(self.h, k, _ptr(out[0]), _ptr(out[1]), _ptr(out[2]), 0, _stream()))
+        return out
+
+    def stats(self) -> dict:
+        s = _Stats()
+        self._check(self.lib.cdu_get_stats(self.h, C.byref(s)))
+        return {k: getattr(s, k) for k, _ in _Stats._fields_}
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.cdu_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+# ---- function-style aliases with the ABI's names ---------------------------------------------------------
+def cdu_create(packed: dict, K_max: int, **options) -> Handle:
+    return Handle(packed, K_max, **options)
+
+
+def cdu_forward(h: Handle, K, rho, alpha, sigma, x0=None, s0=None, y0=None, **kw):
+    return h.forward(K, rho, alpha, sigma, x0, s0, y0, **kw)
+
+
+def cdu_backward(h: Handle, g_xK=None, g_sK=None, g_yK=None, **kw):
+    return h.backward(g_xK, g_sK, g_yK, **kw)
+
+
+def cdu_get_stats(h: Handle) -> dict:
+    return h.stats()
+
+
+def cdu_destroy(h: Handle) -> None:
+    h.close()
+
+
+def cdu_psd_project(S, path: int = 0, use_tensor_cores: int = 0, want_eig: bool = True):
+    """Batched Pi(S) for a CUDA tensor S [count, p, p]; returns (PiS, U, lam)."""
+    torch = _torch()
+    lib = load_library()
+    assert S.is_cuda and S.dim() == 3 and S.shape[1] == S.shape[2]
+    S = S.contiguous()
+    cnt, p = S.shape[0], S.shape[1]
+    dt = CDU_F32 if S.dtype == torch.float32 else CDU_F64
+    out = torch.empty_like(S)
+    U = torch.empty_like(S) if want_eig else None
+    lam = torch.empty(cnt, p, dtype=S.dtype, device=S.device) if want_eig else None
+    st = lib.cdu_psd_project(dt, cnt, p, _ptr(S), _ptr(out), _ptr(U), _ptr(lam), path, use_tensor_cores, _stream())
+    if st != CDU_OK:
+        raise CduError(st, lib.cdu_last_error(None).decode())
+    return out, U, lam
+
+
+def cdu_psd_vjp(U, lam, Gbar, path: int = 0, use_tensor_cores: int = 0):
+    """Batched Dalecki-Krein VJP; U [count,p,p] (eigenvectors in columns), lam [count,p], Gbar [count,p,p]."""
+    torch = _torch()
+    lib = load_library()
+    U, lam, Gbar = U.contiguous(), lam.contiguous(), Gbar.contiguous()
+    cnt, p = U.shape[0], U.shape[1]
+    dt = CDU_F32 if U.dtype == torch.float32 else CDU_F64
+    out = torch.empty_like(Gbar)
+    st = lib.cdu_psd_vjp(dt, cnt, p, _ptr(U), _ptr(lam), _ptr(Gbar), _ptr(out), path, use_tensor_cores, _stream())
+    if st != CDU_OK:
+        raise CduError(st, lib.cdu_last_error(None).decode())
+    return out

@@ -1,0 +1,785 @@
+// cdu_api.cu - host driver behind include/cdu.h: handle, re-packing, the K-loop, the checkpoint store, BPTT.
+// Everything on the hot path runs in the kernels of lin.cuh / psd_small.cuh / psd_large.cuh / gemm_tc.cuh;
+// this file only validates, allocates and launches. No CPU fallback exists: without a CUDA device every entry
+// point that computes returns CDU_ECUDA.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "cdu.h"
+#include "lin.cuh"
+#include "psd_large.cuh"
+#include "psd_small.cuh"
+#include "gemm_tc.cuh"
+
+using namespace cdu;
+
+static thread_local std::string g_create_err;
+
+struct cdu_handle_s {
+  std::string err;
+  virtual ~cdu_handle_s() {}
+  virtual cdu_status forward(int K, const void* rho, int mode, double sigma, const void* alpha, const void* x0,
+                             const void* s0, const void* y0, void* xK, void* sK, void* yK, int host, cudaStream_t st) = 0;
+  virtual cdu_status backward(const void* gx, const void* gs, const void* gy, void* g_rho, void* g_sigma, void* g_alpha,
+                              void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st) = 0;
+  virtual cdu_status stats(cdu_stats* out) = 0;
+  virtual cdu_status iterate(int k, void* x, void* s, void* y, int host, cudaStream_t st) = 0;
+};
+
+namespace {
+
+struct DevPool {  // owns device allocations
+  std::vector<void*> ptrs;
+  size_t bytes = 0;
+  cudaError_t last = cudaSuccess;
+  template <class U> U* alloc(size_t n) {
+    if (n == 0) n = 1;
+    void* p = nullptr;
+    last = cudaMalloc(&p, n * sizeof(U));
+    if (last != cudaSuccess) return nullptr;
+    ptrs.push_back(p);
+    bytes += n * sizeof(U);
+    return reinterpret_cast<U*>(p);
+  }
+  template <class U> U* upload(const std::vector<U>& h, cudaStream_t st) {
+    U* d = alloc<U>(h.size());
+    if (d && !h.empty()) last = cudaMemcpyAsync(d, h.data(), h.size() * sizeof(U), cudaMemcpyHostToDevice, st);
+    return d;
+  }
+  template <class U> U* zeros(size_t n, cudaStream_t st) {
+    U* d = alloc<U>(n);
+    if (d) last = cudaMemsetAsync(d, 0, std::max<size_t>(n, 1) * sizeof(U), st);
+    return d;
+  }
+  void release() {
+    for (void* p : ptrs) cudaFree(p);
+    ptrs.clear();
+    bytes = 0;
+  }
+  ~DevPool() { release(); }
+};
+
+inline int pow2_group(double avg) {
+  int g = 1;
+  while (g < 32 && g < avg * 0.5) g <<= 1;
+  return g;
+}
+
+#define CU_OK(call)                                                                       \
+  do {                                                                                    \
+    cudaError_t e_ = (call);                                                              \
+    if (e_ != cudaSuccess) {                                                              \
+      err = std::string(#call) + ": " + cudaGetErrorString(e_);                           \
+      return CDU_ECUDA;                                                                   \
+    }                                                                                     \
+  } while (0)
+
+// ---------------------------------------------------------------------------------------------------------
+// PSD engine: shared by the handle and the stand-alone operator entry points
+// ---------------------------------------------------------------------------------------------------------
+template <typename T>
+struct PsdEngine {
+  std::string err;
+  PsdTab tab{};
+  int nblk = 0, n_small = 0, n_large = 0, pmax_small = 0, pmax_large = 0;
+  int* d_small_list = nullptr;
+  LargeTab lt{};
+  T *G = nullptr, *Vt = nullptr, *Tm = nullptr, *T2 = nullptr, *mu = nullptr, *lamL = nullptr;
+  float* tc_split = nullptr;   // hi/lo operand staging of the tcgen05 path
+  int* rotflags = nullptr;
+  int* sweeps_max = nullptr;
+  int small_threads = 256;
+  int use_tc = 0;
+  long long launches = 0;
+  std::vector<int> h_large_p;
+  size_t sum_p2 = 0, sum_p = 0;
+
+  cdu_status build(DevPool& pool, const std::vector<int>& prob, const std::vector<int>& row0, const std::vector<int>& p,
+                   int small_max, int want_tc, cudaStream_t st) {
+    nblk = (int)p.size();
+    std::vector<long long> uoff(nblk);
+    std::vector<int> loff(nblk), small_list, gblk, voff, lp;
+    std::vector<long long> moff;
+    long long mo = 0;
+    int vo = 0;
+    for (int i = 0; i < nblk; ++i) {
+      uoff[i] = (long long)sum_p2; loff[i] = (int)sum_p;
+      sum_p2 += (size_t)p[i] * p[i]; sum_p += p[i];
+      if (p[i] <= small_max) { small_list.push_back(i); pmax_small = std::max(pmax_small, p[i]); }
+      else { gblk.push_back(i); moff.push_back(mo); voff.push_back(vo); lp.push_back(p[i]); mo += (long long)p[i] * p[i]; vo += p[i]; pmax_large = std::max(pmax_large, p[i]); }
+    }
+    n_small = (int)small_list.size(); n_large = (int)gblk.size();
+    h_large_p = lp;
+    tab.nblk = nblk;
+    tab.prob = pool.upload(prob, st); tab.row0 = pool.upload(row0, st); tab.p = pool.upload(p, st);
+    tab.uoff = pool.upload(uoff, st); tab.loff = pool.upload(loff, st);
+    d_small_list = pool.upload(small_list, st);
+    sweeps_max = pool.zeros<int>(1, st);
+    small_threads = pmax_small <= 64 ? 256 : 512;
+    if (n_large) {
+      lt.nblk = n_large; lt.pmax = pmax_large;
+      lt.gblk = pool.upload(gblk, st); lt.moff = pool.upload(moff, st); lt.voff = pool.upload(voff, st); lt.pvec = pool.upload(lp, st);
+      G = pool.alloc<T>(mo); Vt = pool.alloc<T>(mo); Tm = pool.alloc<T>(mo); T2 = pool.alloc<T>(mo);
+      mu = pool.alloc<T>(n_large); lamL = pool.alloc<T>(vo);
+      rotflags = pool.zeros<int>((size_t)n_large * HESTENES_MAXSW, st);
+      use_tc = (want_tc != 0) && std::is_same<T, float>::value && gemm_tc_supported(pmax_large) ;
+      for (int q : lp) if (!gemm_tc_supported(q)) use_tc = 0;
+      if (use_tc) tc_split = pool.alloc<float>((size_t)mo * 4);
+      if (!G || !Vt || !Tm || !T2 || !mu || !lamL || !rotflags) { err = "cudaMalloc (PSD large scratch)"; return CDU_ENOMEM; }
+    }
+    if (pool.last != cudaSuccess) { err = std::string("PSD tables: ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
+    if (n_small) {
+      const size_t sf = psd_small_smem_fwd(pmax_small, sizeof(T)), sb = psd_small_smem_bwd(pmax_small, sizeof(T));
+      if (sb > 227 * 1024) { err = "psd_small_max too large for shared memory"; return CDU_EINVAL; }
+      CU_OK(cudaFuncSetAttribute(k_psd_fwd_small<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sf));
+      CU_OK(cudaFuncSetAttribute(k_psd_bwd_small<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb));
+    }
+    return CDU_OK;
+  }
+
+  cdu_status gemm(const T* A, int ta, const T* Bm, int tb, T* C, const T* kscale, int relu, cudaStream_t st) {
+    if (use_tc) {
+      cdu_status s = gemm_tc_batched(n_large, h_large_p.data(), lt.pvec, lt.moff, lt.voff, (const float*)A, ta,
+                                     (const float*)Bm, tb, (float*)C, (const float*)kscale, relu, tc_split, st, &launches, err);
+      return s;
+    }
+    const int tiles = (pmax_large + 63) / 64;
+    k_gemm_fma<T><<<dim3(tiles, tiles, n_large), 256, 0, st>>>(n_large, lt.pvec, lt.moff, lt.voff, A, ta, Bm, tb, C, kscale, relu);
+    ++launches;
+    CU_OK(cudaGetLastError());
+    return CDU_OK;
+  }
+
+  cdu_status eig_large(cudaStream_t st) {   // G (shifted) , Vt = I  ->  Vt, lamL
+    CU_OK(cudaMemsetAsync(rotflags, 0, (size_t)n_large * HESTENES_MAXSW * sizeof(int), st));
+    const int C = 8;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(n_large * C); cfg.blockDim = dim3(512); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    const double tol = std::is_same<T, float>::value ? 3e-7 : 1e-15;
+    const int maxsw = HESTENES_MAXSW - 1;
+    int nl = n_large;
+    const int* pv = lt.pvec; const long long* mo = lt.moff; const int* vo = lt.voff;
+    T *g = G, *v = Vt, *l = lamL; const T* m = mu; int* rf = rotflags; int* sw = sweeps_max;
+    cudaError_t e;
+    if (pmax_large <= 128) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 4>, nl, pv, mo, vo, g, v, m, l, rf, sw, maxsw, tol);
+    else if (pmax_large <= 256) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 8>, nl, pv, mo, vo, g, v, m, l, rf, sw, maxsw, tol);
+    else if (pmax_large <= 512) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 16>, nl, pv, mo, vo, g, v, m, l, rf, sw, maxsw, tol);
+    else if (pmax_large <= 1024) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 32>, nl, pv, mo, vo, g, v, m, l, rf, sw, maxsw, tol);
+    else { err = "PSD block order > 1024 not supported"; return CDU_EINVAL; }
+    ++launches;
+    CU_OK(e);
+    return CDU_OK;
+  }
+
+  cdu_status forward(const Hyper<T>& H, int k, const PsdFwdArgs& A, cudaStream_t st) {
+    if (n_small) {
+      k_psd_fwd_small<T><<<n_small, small_threads, psd_small_smem_fwd(pmax_small, sizeof(T)), st>>>(tab, H, k, A, d_small_list);
+      ++launches;
+      CU_OK(cudaGetLastError());
+    }
+    if (n_large) {
+      k_large_smat<T><<<n_large, 1024, 0, st>>>(tab, lt, A.W, nullptr, H, k, 0, 1, G, Vt, mu);
+      ++launches;
+      CU_OK(cudaGetLastError());
+      cdu_status s = eig_large(st);
+      if (s != CDU_OK) return s;
+      s = gemm(Vt, 1, Vt, 0, Tm, lamL, 1, st);          // Tm = Vt' diag(lam+) Vt
+      if (s != CDU_OK) return s;
+      k_large_finish_fwd<T><<<dim3(64, n_large), 256, 0, st>>>(tab, lt, H, k, Tm, Vt, lamL, A);
+      ++launches;
+      CU_OK(cudaGetLastError());
+    }
+    return CDU_OK;
+  }
+
+  cdu_status backward(const Hyper<T>& H, int k, const PsdBwdArgs& A, cudaStream_t st) {
+    if (n_small) {
+      k_psd_bwd_small<T><<<n_small, small_threads, psd_small_smem_bwd(pmax_small, sizeof(T)), st>>>(tab, H, k, A, d_small_list);
+      ++launches;
+      CU_OK(cudaGetLastError());
+    }
+    if (n_large) {
+      if (A.recompute) {
+        k_large_smat<T><<<n_large, 1024, 0, st>>>(tab, lt, A.W, nullptr, H, k, 0, 1, G, Vt, mu);
+        ++launches;
+        CU_OK(cudaGetLastError());
+        cdu_status s = eig_large(st);
+        if (s != CDU_OK) return s;
+      } else {
+        k_large_fetch<T><<<dim3(64, n_large), 256, 0, st>>>(tab, lt, (const T*)A.Ustore, (const T*)A.Lstore, Vt, lamL);
+        ++launches;
+        CU_OK(cudaGetLastError());
+      }
+      k_large_smat<T><<<n_large, 1024, 0, st>>>(tab, lt, A.Gs, A.Gy, H, k, 1, 0, G, nullptr, nullptr);   // G = smat(g_s + rho g_y)
+      ++launches;
+      CU_OK(cudaGetLastError());
+      cdu_status s;
+      if ((s = gemm(Vt, 0, G, 0, Tm, nullptr, 0, st)) != CDU_OK) return s;     // Tm = Vt G
+      if ((s = gemm(Tm, 0, Vt, 1, G, nullptr, 0, st)) != CDU_OK) return s;     // C  = Tm Vt'
+      k_large_hadamard<T><<<dim3(64, n_large), 256, 0, st>>>(n_large, lt.pvec, lt.moff, lt.voff, G, lamL);
+      ++launches;
+      CU_OK(cudaGetLastError());
+      if ((s = gemm(Vt, 1, G, 0, Tm, nullptr, 0, st)) != CDU_OK) return s;     // Tm = Vt' C
+      if ((s = gemm(Tm, 0, Vt, 0, G, nullptr, 0, st)) != CDU_OK) return s;     // out = Tm Vt
+      k_large_finish_bwd<T><<<n_large, 1024, 0, st>>>(tab, lt, H, k, G, A);
+      ++launches;
+      CU_OK(cudaGetLastError());
+    }
+    return CDU_OK;
+  }
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// handle
+// ---------------------------------------------------------------------------------------------------------
+template <typename T>
+struct HandleT : cdu_handle_s {
+  DevPool pool;
+  BatchDev<T> D{};
+  PsdEngine<T> psd;
+  int B = 0, K_max = 0, ckpt_mode = 0, lin_threads = 256;
+  long long N = 0, Mtot = 0;
+  size_t zstride = 0;
+  double* Z = nullptr;       // [(K_max+1)][N + 2 Mtot]
+  double* XT = nullptr;      // FULL: [K_max][N], LEAN: [N]
+  double* ST = nullptr;      // FULL: [K_max][Mtot], LEAN: [Mtot]
+  T* Ustore = nullptr;       // FULL: [K_max][sum p^2], LEAN: one slot
+  T* Lstore = nullptr;
+  double* GZ[2] = {nullptr, nullptr};
+  double *g_rho_pb = nullptr, *g_alpha_pb = nullptr, *g_sigma_pb = nullptr, *part_pre = nullptr;
+  T *d_rho = nullptr, *d_alpha = nullptr;
+  T* stage = nullptr;        // host-I/O staging, N + 2 Mtot (+ gradient outputs)
+  T* stage_g = nullptr;      // 2 K_max B + B
+  int *cg_f = nullptr, *cg_b = nullptr, *cg_max = nullptr, *flags = nullptr;
+  int K_last = 0, mode_last = 0;
+  double sigma_last = 0;
+  size_t ckpt_bytes = 0;
+  long long launches = 0;
+  cudaStream_t last_stream = nullptr;
+  bool has_psd = false;
+
+  double* z_at(int k) { return Z + (size_t)k * zstride; }
+
+  cdu_status init(const cdu_problem* pr, const cdu_options* op, cudaStream_t st);
+  Hyper<T> hyper() const {
+    Hyper<T> H;
+    H.rho = d_rho; H.alpha = d_alpha; H.sigma = sigma_last;
+    H.kstride = mode_last == CDU_RHO_PER_ITER ? 1 : B; H.pstride = mode_last == CDU_RHO_PER_ITER ? 0 : 1;
+    return H;
+  }
+  cdu_status forward(int K, const void* rho, int mode, double sigma, const void* alpha, const void* x0, const void* s0,
+                     const void* y0, void* xK, void* sK, void* yK, int host, cudaStream_t st) override;
+  cdu_status backward(const void* gx, const void* gs, const void* gy, void* g_rho, void* g_sigma, void* g_alpha,
+                      void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st) override;
+  cdu_status stats(cdu_stats* out) override;
+  cdu_status iterate(int k, void* x, void* s, void* y, int host, cudaStream_t st) override;
+  cdu_status export_state(const double* z, void* x, void* s, void* y, int host, cudaStream_t st);
+  cdu_status import_state(double* z, const void* x, const void* s, const void* y, int host, cudaStream_t st);
+};
+
+template <typename T>
+cdu_status HandleT<T>::init(const cdu_problem* pr, const cdu_options* op, cudaStream_t st) {
+  B = pr->batch;
+  if (B < 1 || !pr->var_off || !pr->row_off || !pr->A_rowptr || !pr->P_rowptr || !pr->cone_off || !pr->cones || !pr->q || !pr->b) {
+    err = "cdu_create: NULL array or batch < 1"; return CDU_EINVAL;
+  }
+  if (pr->var_off[0] != 0 || pr->row_off[0] != 0 || pr->cone_off[0] != 0) { err = "cdu_create: offsets must start at 0"; return CDU_EINVAL; }
+  for (int b = 0; b < B; ++b)
+    if (pr->var_off[b + 1] <= pr->var_off[b] || pr->row_off[b + 1] < pr->row_off[b] || pr->cone_off[b + 1] < pr->cone_off[b]) {
+      err = "cdu_create: offsets must be increasing (n_b >= 1)"; return CDU_EINVAL;
+    }
+  N = pr->var_off[B]; Mtot = pr->row_off[B];
+  const long long nnzA = pr->A_rowptr[Mtot], nnzP = pr->P_rowptr[N];
+  if (N >= (1LL << 31) || Mtot >= (1LL << 31) || nnzA >= (1LL << 31) || nnzP >= (1LL << 31) || nnzA < 0 || nnzP < 0) {
+    err = "cdu_create: sizes exceed int32 range"; return CDU_EINVAL;
+  }
+  if ((nnzA && (!pr->A_colidx || !pr->A_val)) || (nnzP && (!pr->P_colidx || !pr->P_val))) { err = "cdu_create: NULL CSR arrays"; return CDU_EINVAL; }
+  cdu_options o{};
+  if (op) o = *op;
+  else { o.cg_refine = -1; o.use_tensor_cores = -1; }
+  if (o.K_max < 1) { err = "cdu_create: options.K_max must be >= 1"; return CDU_EINVAL; }
+  const bool f32 = std::is_same<T, float>::value;
+  K_max = o.K_max; ckpt_mode = o.ckpt_mode == CDU_CKPT_LEAN ? CDU_CKPT_LEAN : CDU_CKPT_FULL;
+  const int small_max = o.psd_small_max > 0 ? o.psd_small_max : (f32 ? 128 : 88);
+
+  // ---- cones ------------------------------------------------------------------------------------------
+  std::vector<uint8_t> rowkind((size_t)Mtot);
+  std::vector<int> soc_off(B + 1, 0), soc_start, soc_dim, psdblk_off(B + 1, 0), psd_prob, psd_row0, psd_p;
+  int nmax = 0, mmax = 0;
+  for (int b = 0; b < B; ++b) {
+    const long long r0 = pr->row_off[b], m = pr->row_off[b + 1] - r0;
+    nmax = std::max<long long>(nmax, pr->var_off[b + 1] - pr->var_off[b]); mmax = std::max<long long>(mmax, m);
+    long long r = 0;
+    for (long long c = pr->cone_off[b]; c < pr->cone_off[b + 1]; ++c) {
+      const int kind = pr->cones[c].kind, dim = pr->cones[c].dim;
+      if (dim < 1 || kind < 0 || kind > 3) { err = "cdu_create: bad cone"; return CDU_EINVAL; }
+      const long long rows = kind == CDU_PSD ? (long long)dim * (dim + 1) / 2 : dim;
+      if (r + rows > m) { err = "cdu_create: cones exceed the rows of a problem"; return CDU_EINVAL; }
+      if (kind == CDU_SOC) { soc_start.push_back((int)r); soc_dim.push_back(dim); }
+      if (kind == CDU_PSD) { psd_prob.push_back(b); psd_row0.push_back((int)(r0 + r)); psd_p.push_back(dim); }
+      std::fill(rowkind.begin() + r0 + r, rowkind.begin() + r0 + r + rows, (uint8_t)kind);
+      r += rows;
+    }
+    if (r != m) { err = "cdu_create: cones do not tile the rows of a problem"; return CDU_EINVAL; }
+    soc_off[b + 1] = (int)soc_start.size(); psdblk_off[b + 1] = (int)psd_p.size();
+  }
+  has_psd = !psd_p.empty();
+
+  // ---- CSR re-packing: int32 rowptr, transposed copy, diag(P), column square sums ----------------------------
+  const T* Av = reinterpret_cast<const T*>(pr->A_val);
+  const T* Pv = reinterpret_cast<const T*>(pr->P_val);
+  std::vector<int> A_rp((size_t)Mtot + 1), P_rp((size_t)N + 1), AT_rp((size_t)N + 1, 0), AT_ci((size_t)nnzA);
+  std::vector<T> AT_v((size_t)nnzA), diagP((size_t)N, (T)0), colsq((size_t)N, (T)0);
+  for (long long i = 0; i <= Mtot; ++i) A_rp[i] = (int)pr->A_rowptr[i];
+  for (long long i = 0; i <= N; ++i) P_rp[i] = (int)pr->P_rowptr[i];
+  for (long long i = 0; i < Mtot; ++i) if (A_rp[i + 1] < A_rp[i]) { err = "cdu_create: A_rowptr not monotone"; return CDU_EINVAL; }
+  for (long long i = 0; i < N; ++i) if (P_rp[i + 1] < P_rp[i]) { err = "cdu_create: P_rowptr not monotone"; return CDU_EINVAL; }
+  {
+    std::vector<double> csq((size_t)N, 0.0);
+    for (int b = 0; b < B; ++b) {
+      const long long v0 = pr->var_off[b], n = pr->var_off[b + 1] - v0, r0 = pr->row_off[b], r1 = pr->row_off[b + 1];
+      for (long long e = A_rp[r0]; e < A_rp[r1]; ++e) {
+        const int c = pr->A_colidx[e];
+        if (c < 0 || c >= n) { err = "cdu_create: A column index out of range"; return CDU_EINVAL; }
+        ++AT_rp[v0 + c + 1];
+      }
+    }
+    for (long long i = 0; i < N; ++i) AT_rp[i + 1] += AT_rp[i];
+    std::vector<int> fill(AT_rp.begin(), AT_rp.end() - 1);
+    for (int b = 0; b < B; ++b) {
+      const long long v0 = pr->var_off[b], r0 = pr->row_off[b], r1 = pr->row_off[b + 1];
+      for (long long r = r0; r < r1; ++r)
+        for (long long e = A_rp[r]; e < A_rp[r + 1]; ++e) {
+          const long long col = v0 + pr->A_colidx[e];
+          const int dst = fill[col]++;
+          AT_ci[dst] = (int)(r - r0);
+          AT_v[dst] = Av[e];
+          csq[col] += (double)Av[e] * (double)Av[e];
+        }
+      const long long n = pr->var_off[b + 1] - v0;
+      for (long long i = 0; i < n; ++i)
+        for (long long e = P_rp[v0 + i]; e < P_rp[v0 + i + 1]; ++e) {
+          const int c = pr->P_colidx[e];
+          if (c < 0 || c >= n) { err = "cdu_create: P column index out of range"; return CDU_EINVAL; }
+          if (c == i) diagP[v0 + i] += Pv[e];
+        }
+    }
+    for (long long i = 0; i < N; ++i) colsq[i] = (T)csq[i];
+  }
+  std::vector<int> var_off32(B + 1), row_off32(B + 1);
+  for (int b = 0; b <= B; ++b) { var_off32[b] = (int)pr->var_off[b]; row_off32[b] = (int)pr->row_off[b]; }
+
+  // ---- upload -------------------------------------------------------------------------------------------
+  D.B = B; D.N = N; D.Mtot = Mtot;
+  D.var_off = pool.upload(var_off32, st); D.row_off = pool.upload(row_off32, st);
+  D.A_rp = pool.upload(A_rp, st); D.P_rp = pool.upload(P_rp, st); D.AT_rp = pool.upload(AT_rp, st);
+  {
+    int* ci = pool.alloc<int>(nnzA); T* v = pool.alloc<T>(nnzA);
+    int* pci = pool.alloc<int>(nnzP); T* pv = pool.alloc<T>(nnzP);
+    T* q = pool.alloc<T>(N); T* bb = pool.alloc<T>(Mtot);
+    if (!ci || !v || !pci || !pv || !q || !bb) { err = "cudaMalloc (problem data)"; return CDU_ENOMEM; }
+    if (nnzA) { CU_OK(cudaMemcpyAsync(ci, pr->A_colidx, nnzA * sizeof(int), cudaMemcpyHostToDevice, st)); CU_OK(cudaMemcpyAsync(v, Av, nnzA * sizeof(T), cudaMemcpyHostToDevice, st)); }
+    if (nnzP) { CU_OK(cudaMemcpyAsync(pci, pr->P_colidx, nnzP * sizeof(int), cudaMemcpyHostToDevice, st)); CU_OK(cudaMemcpyAsync(pv, Pv, nnzP * sizeof(T), cudaMemcpyHostToDevice, st)); }
+    CU_OK(cudaMemcpyAsync(q, pr->q, N * sizeof(T), cudaMemcpyHostToDevice, st));
+    if (Mtot) CU_OK(cudaMemcpyAsync(bb, pr->b, Mtot * sizeof(T), cudaMemcpyHostToDevice, st));
+    D.A_ci = ci; D.A_v = v; D.P_ci = pci; D.P_v = pv; D.q = q; D.b = bb;
+  }
+  D.AT_ci = pool.upload(AT_ci, st); D.AT_v = pool.upload(AT_v, st);
+  D.diagP = pool.upload(diagP, st); D.colsq = pool.upload(colsq, st);
+  D.rowkind = pool.upload(rowkind, st);
+  D.soc_off = pool.upload(soc_off, st); D.soc_start = pool.upload(soc_start, st); D.soc_dim = pool.upload(soc_dim, st);
+  D.psdblk_off = pool.upload(psdblk_off, st);
+  D.A_G = pow2_group((double)nnzA / std::max<long long>(Mtot, 1));
+  D.AT_G = pow2_group((double)nnzA / (double)N);
+  D.P_G = pow2_group((double)nnzP / (double)N);
+  // scratch
+  D.xi = pool.alloc<double>(N); D.xt_scr = pool.alloc<double>(N); D.rd = pool.alloc<double>(N); D.lam = pool.alloc<double>(N);
+  D.tm = pool.alloc<double>(Mtot); D.st_scr = pool.alloc<double>(Mtot); D.W = pool.alloc<double>(Mtot); D.GW = pool.alloc<double>(Mtot);
+  D.r = pool.alloc<T>(N); D.p = pool.alloc<T>(N); D.Ap = pool.alloc<T>(N); D.d = pool.alloc<T>(N); D.dinv = pool.alloc<T>(N);
+  D.tA = pool.alloc<T>(Mtot);
+  D.tol = o.cg_tol > 0 ? o.cg_tol : (f32 ? 1e-6 : 1e-10);
+  D.tol_ref = o.cg_refine_tol > 0 ? o.cg_refine_tol : 1e-4;
+  D.refine = o.cg_refine >= 0 ? o.cg_refine : (f32 ? 1 : 0);
+  D.maxit = o.cg_max_iter > 0 ? o.cg_max_iter : 2 * nmax + 50;
+  cg_f = pool.zeros<int>(B, st); cg_b = pool.zeros<int>(B, st); cg_max = pool.zeros<int>(B, st); flags = pool.zeros<int>(B, st);
+  D.cg_iters = cg_f; D.cg_max = cg_max; D.flags = flags;
+  lin_threads = std::max(nmax, mmax) <= 16384 ? 256 : 1024;
+  if (pool.last != cudaSuccess) { err = std::string("cdu_create: ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
+
+  // ---- PSD engine -----------------------------------------------------------------------------------------
+  {
+    cdu_status s = psd.build(pool, psd_prob, psd_row0, psd_p, small_max, o.use_tensor_cores, st);
+    if (s != CDU_OK) { err = psd.err; return s; }
+  }
+  D.psd_part = pool.zeros<double>(2 * (size_t)std::max(psd.nblk, 1), st);
+
+  // ---- checkpoint store -------------------------------------------------------------------------------------
+  const size_t before = pool.bytes;
+  zstride = (size_t)N + 2 * (size_t)Mtot;
+  Z = pool.alloc<double>((size_t)(K_max + 1) * zstride);
+  const size_t slots = ckpt_mode == CDU_CKPT_FULL ? (size_t)K_max : 1;
+  XT = pool.alloc<double>(slots * N); ST = pool.alloc<double>(slots * Mtot);
+  Ustore = pool.alloc<T>(slots * psd.sum_p2); Lstore = pool.alloc<T>(slots * psd.sum_p);
+  if (!Z || !XT || !ST || !Ustore || !Lstore) { err = "cudaMalloc (checkpoint store)"; return CDU_ENOMEM; }
+  ckpt_bytes = pool.bytes - before;
+  GZ[0] = pool.alloc<double>(zstride); GZ[1] = pool.alloc<double>(zstride);
+  g_rho_pb = pool.zeros<double>((size_t)K_max * B, st); g_alpha_pb = pool.zeros<double>((size_t)K_max * B, st);
+  g_sigma_pb = pool.zeros<double>((size_t)K_max * B, st); part_pre = pool.zeros<double>(2 * (size_t)B, st);
+  d_rho = pool.alloc<T>((size_t)K_max * B); d_alpha = pool.alloc<T>((size_t)K_max * B);
+  stage = pool.alloc<T>(zstride); stage_g = pool.alloc<T>(2 * (size_t)K_max * B + B);
+  if (pool.last != cudaSuccess || !GZ[0] || !GZ[1] || !stage || !stage_g) { err = std::string("cdu_create: ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
+  CU_OK(cudaStreamSynchronize(st));   // host vectors above go out of scope
+  return CDU_OK;
+}
+
+template <typename T>
+cdu_status HandleT<T>::import_state(double* z, const void* x, const void* s, const void* y, int host, cudaStream_t st) {
+  const void* src[3] = {x, s, y};
+  const long long len[3] = {N, Mtot, Mtot};
+  double* dst[3] = {z, z + N, z + N + Mtot};
+  T* stg = stage;
+  for (int i = 0; i < 3; ++i) {
+    const T* dsrc = reinterpret_cast<const T*>(src[i]);
+    if (src[i] && host) {
+      CU_OK(cudaMemcpyAsync(stg, src[i], len[i] * sizeof(T), cudaMemcpyHostToDevice, st));
+      dsrc = stg; stg += len[i];
+    }
+    if (len[i] == 0) continue;
+    if (!src[i]) { CU_OK(cudaMemsetAsync(dst[i], 0, len[i] * sizeof(double), st)); }
+    else { k_load_vec<T><<<(int)std::min<long long>((len[i] + 255) / 256, 2048), 256, 0, st>>>(dst[i], dsrc, len[i]); ++launches; CU_OK(cudaGetLastError()); }
+  }
+  return CDU_OK;
+}
+
+template <typename T>
+cdu_status HandleT<T>::export_state(const double* z, void* x, void* s, void* y, int host, cudaStream_t st) {
+  void* dstp[3] = {x, s, y};
+  const long long len[3] = {N, Mtot, Mtot};
+  const double* src[3] = {z, z + N, z + N + Mtot};
+  T* stg = stage;
+  for (int i = 0; i < 3; ++i) {
+    if (!dstp[i] || len[i] == 0) continue;
+    T* ddst = host ? stg : reinterpret_cast<T*>(dstp[i]);
+    k_store_vec<T><<<(int)std::min<long long>((len[i] + 255) / 256, 2048), 256, 0, st>>>(ddst, src[i], len[i]);
+    ++launches;
+    CU_OK(cudaGetLastError());
+    if (host) { CU_OK(cudaMemcpyAsync(dstp[i], stg, len[i] * sizeof(T), cudaMemcpyDeviceToHost, st)); stg += len[i]; }
+  }
+  return CDU_OK;
+}
+
+template <typename T>
+cdu_status HandleT<T>::forward(int K, const void* rho, int mode, double sigma, const void* alpha, const void* x0,
+                               const void* s0, const void* y0, void* xK, void* sK, void* yK, int host, cudaStream_t st) {
+  if (K < 1 || K > K_max) { err = "cdu_forward: K out of [1, K_max]"; return CDU_EINVAL; }
+  if (!rho || !alpha) { err = "cdu_forward: NULL rho/alpha"; return CDU_EINVAL; }
+  if (!(sigma > 0.0)) { err = "cdu_forward: sigma must be > 0"; return CDU_EINVAL; }
+  if (mode != CDU_RHO_PER_ITER && mode != CDU_RHO_PER_PROBLEM) { err = "cdu_forward: bad rho_mode"; return CDU_EINVAL; }
+  const size_t cnt = (size_t)K * (mode == CDU_RHO_PER_ITER ? 1 : B);
+  if (host) {
+    const T* r = reinterpret_cast<const T*>(rho); const T* a = reinterpret_cast<const T*>(alpha);
+    for (size_t i = 0; i < cnt; ++i)
+      if (!(r[i] > (T)0) || !(a[i] > (T)0) || !(a[i] < (T)2)) { err = "cdu_forward: rho must be > 0 and alpha in (0,2)"; return CDU_EINVAL; }
+  }
+  const cudaMemcpyKind kind = host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+  CU_OK(cudaMemcpyAsync(d_rho, rho, cnt * sizeof(T), kind, st));
+  CU_OK(cudaMemcpyAsync(d_alpha, alpha, cnt * sizeof(T), kind, st));
+  K_last = 0; mode_last = mode; sigma_last = sigma; last_stream = st;
+  cdu_status s = import_state(z_at(0), x0, s0, y0, host, st);
+  if (s != CDU_OK) return s;
+  CU_OK(cudaMemsetAsync(cg_f, 0, B * sizeof(int), st));
+  CU_OK(cudaMemsetAsync(cg_max, 0, B * sizeof(int), st));
+  CU_OK(cudaMemsetAsync(flags, 0, B * sizeof(int), st));
+  CU_OK(cudaMemsetAsync(psd.sweeps_max, 0, sizeof(int), st));
+  const Hyper<T> H = hyper();
+  BatchDev<T> Df = D; Df.cg_iters = cg_f;
+  const bool full = ckpt_mode == CDU_CKPT_FULL;
+  for (int k = 0; k < K; ++k) {
+    IterPtrs I;
+    I.Zk = z_at(k); I.Zk1 = z_at(k + 1);
+    I.XT = XT + (full ? (size_t)k * N : 0); I.ST = ST + (full ? (size_t)k * Mtot : 0);
+    k_fwd<T><<<B, lin_threads, 0, st>>>(Df, H, I, k);
+    ++launches;
+    CU_OK(cudaGetLastError());
+    if (has_psd) {
+      PsdFwdArgs A;
+      A.W = D.W; A.S1 = z_at(k + 1) + N; A.Y1 = z_at(k + 1) + N + Mtot;
+      A.Ustore = Ustore + (full ? (size_t)k * psd.sum_p2 : 0); A.Lstore = Lstore + (full ? (size_t)k * psd.sum_p : 0);
+      A.sweeps_max = psd.sweeps_max; A.flags = flags;
+      s = psd.forward(H, k, A, st);
+      if (s != CDU_OK) { err = psd.err; return s; }
+    }
+  }
+  K_last = K;
+  s = export_state(z_at(K), xK, sK, yK, host, st);
+  if (s != CDU_OK) return s;
+  if (host) CU_OK(cudaStreamSynchronize(st));
+  return CDU_OK;
+}
+
+template <typename T>
+cdu_status HandleT<T>::backward(const void* gx, const void* gs, const void* gy, void* g_rho, void* g_sigma, void* g_alpha,
+                                void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st) {
+  if (K_last < 1) { err = "cdu_backward: no forward pass on this handle"; return CDU_ESTATE; }
+  const int K = K_last;
+  last_stream = st;
+  cdu_status s = import_state(GZ[K & 1], gx, gs, gy, host, st);
+  if (s != CDU_OK) return s;
+  CU_OK(cudaMemsetAsync(cg_b, 0, B * sizeof(int), st));
+  const Hyper<T> H = hyper();
+  BatchDev<T> Db = D; Db.cg_iters = cg_b;
+  const bool full = ckpt_mode == CDU_CKPT_FULL;
+  for (int k = K - 1; k >= 0; --k) {
+    BwdPtrs Q;
+    Q.Zk = z_at(k); Q.Zk1 = z_at(k + 1);
+    Q.XT = XT + (full ? (size_t)k * N : 0); Q.ST = ST + (full ? (size_t)k * Mtot : 0);
+    Q.Gin = GZ[(k + 1) & 1]; Q.Gout = GZ[k & 1];
+    Q.g_rho_pb = g_rho_pb; Q.g_alpha_pb = g_alpha_pb; Q.g_sigma_pb = g_sigma_pb; Q.part_pre = part_pre;
+    Q.recompute = full ? 0 : 1;
+    if (!has_psd) {
+      k_bwd<T><<<B, lin_threads, 0, st>>>(Db, H, Q, k, 0);
+      ++launches;
+      CU_OK(cudaGetLastError());
+    } else {
+      k_bwd<T><<<B, lin_threads, 0, st>>>(Db, H, Q, k, 1);
+      ++launches;
+      CU_OK(cudaGetLastError());
+      PsdBwdArgs A;
+      A.W = D.W; A.Yk = z_at(k) + N + Mtot; A.S1 = z_at(k + 1) + N;
+      A.Gs = Q.Gin + N; A.Gy = Q.Gin + N + Mtot; A.GW = D.GW; A.part = D.psd_part;
+      A.Ustore = Ustore + (full ? (size_t)k * psd.sum_p2 : 0); A.Lstore = Lstore + (full ? (size_t)k * psd.sum_p : 0);
+      A.recompute = full ? 0 : 1; A.flags = flags;
+      s = psd.backward(H, k, A, st);
+      if (s != CDU_OK) { err = psd.err; return s; }
+      k_bwd<T><<<B, lin_threads, 0, st>>>(Db, H, Q, k, 2);
+      ++launches;
+      CU_OK(cudaGetLastError());
+    }
+  }
+  const int pp = mode_last == CDU_RHO_PER_PROBLEM;
+  const size_t cnt = (size_t)K * (pp ? B : 1), scnt = pp ? B : 1;
+  T* o_rho = host ? stage_g : reinterpret_cast<T*>(g_rho);
+  T* o_alpha = host ? stage_g + cnt : reinterpret_cast<T*>(g_alpha);
+  T* o_sigma = host ? stage_g + 2 * cnt : reinterpret_cast<T*>(g_sigma);
+  if (host) { if (!g_rho) o_rho = nullptr; if (!g_alpha) o_alpha = nullptr; if (!g_sigma) o_sigma = nullptr; }
+  k_reduce_grads<T><<<1, 256, 0, st>>>(g_rho_pb, g_alpha_pb, g_sigma_pb, K, B, pp, o_rho, o_alpha, o_sigma);
+  ++launches;
+  CU_OK(cudaGetLastError());
+  if (host) {
+    if (g_rho) CU_OK(cudaMemcpyAsync(g_rho, o_rho, cnt * sizeof(T), cudaMemcpyDeviceToHost, st));
+    if (g_alpha) CU_OK(cudaMemcpyAsync(g_alpha, o_alpha, cnt * sizeof(T), cudaMemcpyDeviceToHost, st));
+    if (g_sigma) CU_OK(cudaMemcpyAsync(g_sigma, o_sigma, scnt * sizeof(T), cudaMemcpyDeviceToHost, st));
+  }
+  s = export_state(GZ[0], g_x0, g_s0, g_y0, host, st);
+  if (s != CDU_OK) return s;
+  if (host) CU_OK(cudaStreamSynchronize(st));
+  return CDU_OK;
+}
+
+template <typename T>
+cdu_status HandleT<T>::iterate(int k, void* x, void* s, void* y, int host, cudaStream_t st) {
+  if (k < 0 || k > K_last) { err = "cdu_get_iterate: k out of range"; return CDU_EINVAL; }
+  cdu_status r = export_state(z_at(k), x, s, y, host, st);
+  if (r != CDU_OK) return r;
+  if (host) CU_OK(cudaStreamSynchronize(st));
+  return CDU_OK;
+}
+
+template <typename T>
+cdu_status HandleT<T>::stats(cdu_stats* out) {
+  if (!out) { err = "cdu_get_stats: NULL out"; return CDU_EINVAL; }
+  CU_OK(cudaStreamSynchronize(last_stream));
+  std::vector<int> f(B), bw(B), mx(B), fl(B);
+  int sw = 0;
+  CU_OK(cudaMemcpy(f.data(), cg_f, B * sizeof(int), cudaMemcpyDeviceToHost));
+  CU_OK(cudaMemcpy(bw.data(), cg_b, B * sizeof(int), cudaMemcpyDeviceToHost));
+  CU_OK(cudaMemcpy(mx.data(), cg_max, B * sizeof(int), cudaMemcpyDeviceToHost));
+  CU_OK(cudaMemcpy(fl.data(), flags, B * sizeof(int), cudaMemcpyDeviceToHost));
+  CU_OK(cudaMemcpy(&sw, psd.sweeps_max, sizeof(int), cudaMemcpyDeviceToHost));
+  std::memset(out, 0, sizeof(*out));
+  for (int b = 0; b < B; ++b) {
+    out->cg_iters_fwd += f[b]; out->cg_iters_bwd += bw[b];
+    out->cg_iters_max = std::max(out->cg_iters_max, mx[b]);
+    if (fl[b]) { ++out->n_flagged; out->flags_or |= fl[b]; }
+  }
+  out->eig_sweeps_max = sw;
+  out->device_bytes = (int64_t)pool.bytes; out->ckpt_bytes = (int64_t)ckpt_bytes;
+  out->launches = launches + psd.launches;
+  return CDU_OK;
+}
+
+template <typename T>
+cdu_status create_t(const cdu_problem* pr, const cdu_options* op, cudaStream_t st, cdu_handle* out) {
+  HandleT<T>* h = new (std::nothrow) HandleT<T>();
+  if (!h) { g_create_err = "out of host memory"; return CDU_ENOMEM; }
+  cdu_status s;
+  try { s = h->init(pr, op, st); }
+  catch (const std::bad_alloc&) { h->err = "out of host memory"; s = CDU_ENOMEM; }
+  if (s != CDU_OK) { g_create_err = h->err; delete h; return s; }
+  *out = h;
+  return CDU_OK;
+}
+
+// ---- stand-alone PSD operators ------------------------------------------------------------------------------
+template <typename T>
+__global__ void k_dense_to_svec(int p, const T* S, double* v) {   // one block per matrix
+  const long long off = (long long)blockIdx.x * p * p;
+  const int nsv = p * (p + 1) / 2;
+  for (long long t = threadIdx.x; t < (long long)p * p; t += blockDim.x) {
+    const int r = (int)(t / p), c = (int)(t - (long long)r * p);
+    if (r <= c) {
+      const double x = r == c ? (double)S[off + t] : 0.5 * ((double)S[off + t] + (double)S[off + (long long)c * p + r]) * 1.41421356237309504880;
+      v[(long long)blockIdx.x * nsv + svec_idx(r, c)] = x;
+    }
+  }
+}
+template <typename T>
+__global__ void k_svec_to_dense(int p, const double* v, T* S) {
+  const long long off = (long long)blockIdx.x * p * p;
+  const int nsv = p * (p + 1) / 2;
+  for (long long t = threadIdx.x; t < (long long)p * p; t += blockDim.x) {
+    const int r = (int)(t / p), c = (int)(t - (long long)r * p);
+    const double x = v[(long long)blockIdx.x * nsv + (r <= c ? svec_idx(r, c) : svec_idx(c, r))];
+    S[off + t] = (T)(r == c ? x : x * 0.70710678118654752440);
+  }
+}
+template <typename T>
+__global__ void k_transpose_batched(int p, const T* A, T* Bm) {
+  const long long off = (long long)blockIdx.x * p * p;
+  for (long long t = threadIdx.x; t < (long long)p * p; t += blockDim.x) {
+    const int r = (int)(t / p), c = (int)(t - (long long)r * p);
+    Bm[off + (long long)c * p + r] = A[off + t];
+  }
+}
+
+template <typename T>
+cdu_status psd_op_t(bool vjp, int count, int p, const void* in1, const void* in2, const void* in3, void* out1, void* out2,
+                    void* out3, int path, int use_tc, cudaStream_t st, std::string& err) {
+  // projection: in1 = S           -> out1 = PiS, out2 = U, out3 = lam
+  // vjp       : in1 = U, in2 = lam, in3 = Gbar -> out1 = Sbar
+  if (count < 1 || p < 1 || !in1 || !out1 || (vjp && (!in2 || !in3))) { err = "cdu_psd_*: bad arguments"; return CDU_EINVAL; }
+  DevPool pool;
+  PsdEngine<T> eng;
+  const int nsv = p * (p + 1) / 2;
+  std::vector<int> prob(count), row0(count), pv(count, p);
+  for (int i = 0; i < count; ++i) { prob[i] = i; row0[i] = i * nsv; }
+  const bool f32 = std::is_same<T, float>::value;
+  int small_max = f32 ? 128 : 88;
+  if (path == 1) small_max = 1 << 30; else if (path == 2) small_max = 0;
+  cdu_status s = eng.build(pool, prob, row0, pv, small_max, use_tc, st);
+  if (s != CDU_OK) { err = eng.err; return s; }
+  const size_t tot = (size_t)count * nsv;
+  double* W = pool.zeros<double>(tot, st); double* S1 = pool.zeros<double>(tot, st); double* Y1 = pool.zeros<double>(tot, st);
+  double* GW = pool.zeros<double>(tot, st); double* part = pool.zeros<double>(2 * (size_t)count, st);
+  double* Gs = pool.zeros<double>(tot, st);
+  T* Us = pool.alloc<T>((size_t)count * p * p); T* Ls = pool.alloc<T>((size_t)count * p);
+  int* flags = pool.zeros<int>(count, st);
+  std::vector<T> one(1, (T)1);
+  T* d_one = pool.upload(one, st);
+  if (pool.last != cudaSuccess || !W || !S1 || !Y1 || !GW || !part || !Gs || !Us || !Ls || !flags || !d_one) { err = "cudaMalloc (psd op)"; return CDU_ENOMEM; }
+  Hyper<T> H; H.rho = d_one; H.alpha = d_one; H.kstride = 0; H.pstride = 0; H.sigma = 1.0;
+  const bool large = eng.n_large > 0;
+  if (!vjp) {
+    k_dense_to_svec<T><<<count, 256, 0, st>>>(p, (const T*)in1, W);
+    PsdFwdArgs A; A.W = W; A.S1 = S1; A.Y1 = Y1; A.Ustore = Us; A.Lstore = Ls; A.sweeps_max = eng.sweeps_max; A.flags = flags;
+    s = eng.forward(H, 0, A, st);
+    if (s != CDU_OK) { err = eng.err; return s; }
+    k_svec_to_dense<T><<<count, 256, 0, st>>>(p, S1, (T*)out1);
+    if (out2) {
+      if (large) k_transpose_batched<T><<<count, 256, 0, st>>>(p, Us, (T*)out2);
+      else CU_OK(cudaMemcpyAsync(out2, Us, (size_t)count * p * p * sizeof(T), cudaMemcpyDeviceToDevice, st));
+    }
+    if (out3) CU_OK(cudaMemcpyAsync(out3, Ls, (size_t)count * p * sizeof(T), cudaMemcpyDeviceToDevice, st));
+  } else {
+    if (large) k_transpose_batched<T><<<count, 256, 0, st>>>(p, (const T*)in1, Us);
+    else CU_OK(cudaMemcpyAsync(Us, in1, (size_t)count * p * p * sizeof(T), cudaMemcpyDeviceToDevice, st));
+    CU_OK(cudaMemcpyAsync(Ls, in2, (size_t)count * p * sizeof(T), cudaMemcpyDeviceToDevice, st));
+    k_dense_to_svec<T><<<count, 256, 0, st>>>(p, (const T*)in3, Gs);
+    PsdBwdArgs A; A.W = W; A.Yk = Y1; A.S1 = S1; A.Gs = Gs; A.Gy = W /* zeros */; A.GW = GW; A.part = part;
+    A.Ustore = Us; A.Lstore = Ls; A.recompute = 0; A.flags = flags;
+    s = eng.backward(H, 0, A, st);
+    if (s != CDU_OK) { err = eng.err; return s; }
+    k_svec_to_dense<T><<<count, 256, 0, st>>>(p, GW, (T*)out1);
+  }
+  CU_OK(cudaGetLastError());
+  CU_OK(cudaStreamSynchronize(st));
+  return CDU_OK;
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------------------
+// C ABI
+// ---------------------------------------------------------------------------------------------------------
+extern "C" {
+
+cdu_status cdu_create(const cdu_problem* prob, const cdu_options* opts, void* cuda_stream, cdu_handle* out) {
+  if (!prob || !out) { g_create_err = "cdu_create: NULL argument"; return CDU_EINVAL; }
+  *out = nullptr;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { g_create_err = "cdu_create: no CUDA device (there is no CPU fallback)"; return CDU_ECUDA; }
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  if (prob->dtype == CDU_F32) return create_t<float>(prob, opts, st, out);
+  if (prob->dtype == CDU_F64) return create_t<double>(prob, opts, st, out);
+  g_create_err = "cdu_create: bad dtype";
+  return CDU_EINVAL;
+}
+
+cdu_status cdu_forward(cdu_handle h, int32_t K, const void* rho, int32_t rho_mode, double sigma, const void* alpha,
+                       const void* x0, const void* s0, const void* y0, void* xK, void* sK, void* yK, int32_t io_on_host,
+                       void* cuda_stream) {
+  if (!h) return CDU_EINVAL;
+  return h->forward(K, rho, rho_mode, sigma, alpha, x0, s0, y0, xK, sK, yK, io_on_host, reinterpret_cast<cudaStream_t>(cuda_stream));
+}
+
+cdu_status cdu_backward(cdu_handle h, const void* g_xK, const void* g_sK, const void* g_yK, void* g_rho, void* g_sigma,
+                        void* g_alpha, void* g_x0, void* g_s0, void* g_y0, int32_t io_on_host, void* cuda_stream) {
+  if (!h) return CDU_EINVAL;
+  return h->backward(g_xK, g_sK, g_yK, g_rho, g_sigma, g_alpha, g_x0, g_s0, g_y0, io_on_host, reinterpret_cast<cudaStream_t>(cuda_stream));
+}
+
+cdu_status cdu_get_stats(cdu_handle h, cdu_stats* out) { return h ? h->stats(out) : CDU_EINVAL; }
+
+cdu_status cdu_get_iterate(cdu_handle h, int32_t k, void* x, void* s, void* y, int32_t io_on_host, void* cuda_stream) {
+  if (!h) return CDU_EINVAL;
+  return h->iterate(k, x, s, y, io_on_host, reinterpret_cast<cudaStream_t>(cuda_stream));
+}
+
+const char* cdu_last_error(cdu_handle h) { return h ? h->err.c_str() : g_create_err.c_str(); }
+
+cdu_status cdu_destroy(cdu_handle h) {
+  if (!h) return CDU_EINVAL;
+  cudaDeviceSynchronize();
+  delete h;
+  return CDU_OK;
+}
+
+const char* cdu_version(void) { return "cdu 0.1 (sm_100a)"; }
+
+cdu_status cdu_psd_project(int32_t dtype, int32_t count, int32_t p, const void* S, void* PiS, void* U, void* lam,
+                           int32_t path, int32_t use_tensor_cores, void* cuda_stream) {
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  if (dtype == CDU_F32) return psd_op_t<float>(false, count, p, S, nullptr, nullptr, PiS, U, lam, path, use_tensor_cores, st, g_create_err);
+  if (dtype == CDU_F64) return psd_op_t<double>(false, count, p, S, nullptr, nullptr, PiS, U, lam, path, use_tensor_cores, st, g_create_err);
+  return CDU_EINVAL;
+}
+
+cdu_status cdu_psd_vjp(int32_t dtype, int32_t count, int32_t p, const void* U, const void* lam, const void* Gbar,
+                       void* Sbar, int32_t path, int32_t use_tensor_cores, void* cuda_stream) {
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  if (dtype == CDU_F32) return psd_op_t<float>(true, count, p, U, lam, Gbar, Sbar, nullptr, nullptr, path, use_tensor_cores, st, g_create_err);
+  if (dtype == CDU_F64) return psd_op_t<double>(true, count, p, U, lam, Gbar, Sbar, nullptr, nullptr, path, use_tensor_cores, st, g_create_err);
+  return CDU_EINVAL;
+}
+
+}  // extern "C"

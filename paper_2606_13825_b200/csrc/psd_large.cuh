@@ -1,0 +1,280 @@
+// psd_large.cuh - PSD projection / Dalecki-Krein VJP for blocks too large for one CTA's shared memory.
+//
+// Eigendecomposition: one-sided (Hestenes) Jacobi on the shifted matrix S + mu I >= 0, one thread-block
+// cluster per matrix, one warp per column pair, columns contiguous in memory (coalesced, L2 resident),
+// rounds separated by cluster barriers. On convergence the columns g_i = (S + mu I) v_i are orthogonal, so
+// v_i are eigenvectors and lambda_i = ||g_i|| - mu. Only Pi(S) and the DK products are compared with the
+// oracle, never U (any orthonormal basis inside an eigenvalue cluster is valid).
+// Rebuild U max(L,0) U' (Eq. 7) and the four DK products (Eq. 9) are dense p x p x p GEMMs:
+// fp32/fp64 FMA kernel here, tcgen05 3xTF32 kernel in gemm_tc.cuh.
+// Eigenvectors are stored as ROWS (Vt[i][:] = v_i).
+#pragma once
+#include <cooperative_groups.h>
+#include "common.cuh"
+#include "psd_small.cuh"
+
+namespace cdu {
+namespace cg = cooperative_groups;
+
+struct LargeTab {
+  int nblk;              // number of large blocks
+  const int* gblk;       // index into the global PSD table
+  const long long* moff; // offset of the block's p x p scratch matrices (elements)
+  const int* voff;       // offset of the block's length-p scratch vectors
+  const int* pvec;       // order of each large block
+  int pmax;
+};
+
+// G = smat(v [+ scale v2]) + mu I with mu = ||smat||_F (shift = 1) or mu = 0; optionally Vt = I. One CTA per block.
+template <typename T>
+__global__ void __launch_bounds__(1024) k_large_smat(PsdTab tab, LargeTab lt, const double* v, const double* v2,
+                                                     Hyper<T> H, int k, int use_rho_scale, int shift, T* G, T* Vt, T* mu) {
+  __shared__ double sh[32];
+  const int lb = blockIdx.x, blk = lt.gblk[lb];
+  const int p = tab.p[blk];
+  const long long row0 = tab.row0[blk];
+  const double sc = use_rho_scale ? H.rho_at(k, tab.prob[blk]) : 0.0;
+  T* g = G + lt.moff[lb];
+  const double* a = v + row0;
+  const double* a2 = v2 ? v2 + row0 : nullptr;
+  double acc[1] = {0.0};
+  const int nsv = p * (p + 1) / 2;
+  for (int t = threadIdx.x; t < nsv; t += blockDim.x) {
+    double x = a[t];
+    if (a2) x += sc * a2[t];
+    acc[0] += x * x;       // svec is an isometry: ||smat||_F = ||svec||_2
+  }
+  block_sum<1>(acc, sh);
+  const double m = shift ? sqrt(acc[0]) : 0.0;
+  if (threadIdx.x == 0 && mu) mu[lb] = (T)m;
+  for (long long t = threadIdx.x; t < (long long)p * p; t += blockDim.x) {
+    const int r = (int)(t / p), c = (int)(t - (long long)r * p);
+    const int idx = r <= c ? svec_idx(r, c) : svec_idx(c, r);
+    double x = a[idx];
+    if (a2) x += sc * a2[idx];
+    g[t] = (T)(r == c ? x + m : x * 0.70710678118654752440);
+    if (Vt) Vt[lt.moff[lb] + t] = (r == c) ? (T)1 : (T)0;
+  }
+}
+
+// Dense-input variant for the stand-alone entry points: G = S + mu I, Vt = I.
+template <typename T>
+__global__ void __launch_bounds__(1024) k_large_dense_init(int p, const T* S, T* G, T* Vt, T* mu) {
+  __shared__ double sh[32];
+  const long long off = (long long)blockIdx.x * p * p;
+  double acc[1] = {0.0};
+  for (long long t = threadIdx.x; t < (long long)p * p; t += blockDim.x) { const double x = (double)S[off + t]; acc[0] += x * x; }
+  block_sum<1>(acc, sh);
+  const double m = sqrt(acc[0]);
+  if (threadIdx.x == 0) mu[blockIdx.x] = (T)m;
+  for (long long t = threadIdx.x; t < (long long)p * p; t += blockDim.x) {
+    const int r = (int)(t / p), c = (int)(t - (long long)r * p);
+    G[off + t] = S[off + t] + ((r == c) ? (T)m : (T)0);
+    Vt[off + t] = (r == c) ? (T)1 : (T)0;
+  }
+}
+
+constexpr int HESTENES_MAXSW = 64;
+
+// One cluster per matrix. G, Vt: p x p row-major with column i of the working matrix stored as row i.
+template <typename T, int NE>
+__global__ void __launch_bounds__(512) k_hestenes(int nblk, const int* pvec, const long long* moff, const int* voff, T* G, T* Vt,
+                                                  const T* mu, T* lam, int* rotflags, int* sweeps_out, int max_sweeps,
+                                                  double tol) {
+  cg::cluster_group cluster = cg::this_cluster();
+  const int C = cluster.num_blocks();
+  const int lb = blockIdx.x / C, rank = cluster.block_rank();
+  const int p = pvec[lb], pe = (p + 1) & ~1, h = pe >> 1;
+  T* g = G + moff[lb];
+  T* vt = Vt + moff[lb];
+  const int lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+  const int gw = rank * nw + (threadIdx.x >> 5), wtot = C * nw;
+  int* rf = rotflags + lb * HESTENES_MAXSW;
+  int sweep = 0;
+  for (; sweep < max_sweeps; ++sweep) {
+    for (int r = 0; r < pe - 1; ++r) {
+      for (int q = gw; q < h; q += wtot) {
+        int i, j; rr_pair(r, q, pe, i, j);
+        if (j >= p) continue;
+        T gi[NE], gj[NE];
+        double a = 0.0, b = 0.0, c = 0.0;
+#pragma unroll
+        for (int e = 0; e < NE; ++e) {
+          const int col = lane + 32 * e;
+          gi[e] = col < p ? __ldcg(g + (long long)i * p + col) : (T)0;
+          gj[e] = col < p ? __ldcg(g + (long long)j * p + col) : (T)0;
+          a += (double)gi[e] * (double)gi[e]; b += (double)gj[e] * (double)gj[e]; c += (double)gi[e] * (double)gj[e];
+        }
+        a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
+        if (fabs(c) > tol * sqrt(a * b) && a > 0.0 && b > 0.0) {
+          const double zeta = (b - a) / (2.0 * c);
+          const double t = (zeta >= 0.0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+          const double cd = 1.0 / sqrt(1.0 + t * t);
+          const T cs = (T)cd, sn = (T)(t * cd);
+#pragma unroll
+          for (int e = 0; e < NE; ++e) {
+            const int col = lane + 32 * e;
+            if (col < p) {
+              __stcg(g + (long long)i * p + col, cs * gi[e] - sn * gj[e]);
+              __stcg(g + (long long)j * p + col, sn * gi[e] + cs * gj[e]);
+              const T vi = __ldcg(vt + (long long)i * p + col), vj = __ldcg(vt + (long long)j * p + col);
+              __stcg(vt + (long long)i * p + col, cs * vi - sn * vj);
+              __stcg(vt + (long long)j * p + col, sn * vi + cs * vj);
+            }
+          }
+          if (lane == 0) rf[sweep] = 1;
+        }
+      }
+      cluster.sync();
+    }
+    const int rot = __ldcg(rf + sweep);
+    if (!rot) break;
+  }
+  // eigenvalues
+  for (int i = gw; i < p; i += wtot) {
+    double a = 0.0;
+    for (int col = lane; col < p; col += 32) { const double x = (double)__ldcg(g + (long long)i * p + col); a += x * x; }
+    a = warp_sum(a);
+    if (lane == 0) lam[voff[lb] + i] = (T)(sqrt(a) - (double)mu[lb]);
+  }
+  if (rank == 0 && threadIdx.x == 0) atomicMax(sweeps_out, sweep);
+}
+
+// Batched row-major GEMM C = op(A) op(B) (p x p x p per block), FMA path. 64x64 tile, 16x16 threads, 4x4 each.
+// Optional row scaling of op(A): op(A)(i,k) *= rs[k] (used for U diag(lam+) U').
+template <typename T>
+__global__ void __launch_bounds__(256) k_gemm_fma(int nblk, const int* pvec, const long long* moff, const int* voff, const T* A, int ta,
+                                                  const T* Bm, int tb, T* Cm, const T* kscale, int kscale_relu) {
+  __shared__ T As[16][64 + 1];
+  __shared__ T Bs[16][64 + 1];
+  const int lb = blockIdx.z, p = pvec[lb];
+  const int i0 = blockIdx.y * 64, j0 = blockIdx.x * 64;
+  if (i0 >= p || j0 >= p) return;
+  const T* a = A + moff[lb];
+  const T* b = Bm + moff[lb];
+  T* c = Cm + moff[lb];
+  const T* ks = kscale ? kscale + voff[lb] : nullptr;
+  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+  T acc[4][4] = {};
+  for (int k0 = 0; k0 < p; k0 += 16) {
+    for (int t = threadIdx.x; t < 16 * 64; t += 256) {
+      int kk, ii;
+      if (ta) { kk = t / 64; ii = t % 64; } else { ii = t / 16; kk = t % 16; }   // coalesce along the contiguous axis
+      const int gi = i0 + ii, gk = k0 + kk;
+      T v = (T)0;
+      if (gi < p && gk < p) {
+        v = ta ? a[(long long)gk * p + gi] : a[(long long)gi * p + gk];
+        if (ks) { T s = ks[gk]; if (kscale_relu && !(s > (T)0)) s = (T)0; v *= s; }
+      }
+      As[kk][ii] = v;
+    }
+    for (int t = threadIdx.x; t < 16 * 64; t += 256) {
+      int kk, jj;
+      if (tb) { jj = t / 16; kk = t % 16; } else { kk = t / 64; jj = t % 64; }
+      const int gj = j0 + jj, gk = k0 + kk;
+      T v = (T)0;
+      if (gj < p && gk < p) v = tb ? b[(long long)gj * p + gk] : b[(long long)gk * p + gj];
+      Bs[kk][jj] = v;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int kk = 0; kk < 16; ++kk) {
+      T x[4], y[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { x[u] = As[kk][ty * 4 + u]; y[u] = Bs[kk][tx * 4 + u]; }
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+#pragma unroll
+        for (int w = 0; w < 4; ++w) acc[u][w] += x[u] * y[w];
+    }
+    __syncthreads();
+  }
+#pragma unroll
+  for (int u = 0; u < 4; ++u)
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+      const int gi = i0 + ty * 4 + u, gj = j0 + tx * 4 + w;
+      if (gi < p && gj < p) c[(long long)gi * p + gj] = acc[u][w];
+    }
+}
+
+template <typename T>
+__global__ void k_large_hadamard(int nblk, const int* pvec, const long long* moff, const int* voff, T* Cm, const T* lam) {
+  const int lb = blockIdx.y, p = pvec[lb];
+  T* c = Cm + moff[lb];
+  const T* l = lam + voff[lb];
+  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < (long long)p * p; t += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(t / p), j = (int)(t - (long long)i * p);
+    c[t] *= gamma_relu<T>(l[i], l[j]);
+  }
+}
+
+// s+ = svec(Tm), y+ = rho (s+ - w); also copies Vt, lam into the checkpoint store.
+template <typename T>
+__global__ void __launch_bounds__(1024) k_large_finish_fwd(PsdTab tab, LargeTab lt, Hyper<T> H, int k, const T* Tm,
+                                                           const T* Vt, const T* lam, PsdFwdArgs A) {
+  const int lb = blockIdx.y, blk = lt.gblk[lb];
+  const int p = tab.p[blk];
+  const long long row0 = tab.row0[blk];
+  const double rho = H.rho_at(k, tab.prob[blk]);
+  const T* tm = Tm + lt.moff[lb];
+  const double* w = A.W + row0;
+  double *s1 = A.S1 + row0, *y1 = A.Y1 + row0;
+  T* U = reinterpret_cast<T*>(A.Ustore) + tab.uoff[blk];
+  T* L = reinterpret_cast<T*>(A.Lstore) + tab.loff[blk];
+  const long long stride = (long long)gridDim.x * blockDim.x, t0 = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  for (long long t = t0; t < (long long)p * p; t += stride) {
+    const int r = (int)(t / p), c = (int)(t - (long long)r * p);
+    if (U != Vt + lt.moff[lb]) U[t] = Vt[lt.moff[lb] + t];
+    if (r <= c) {
+      const double o = (r == c) ? (double)tm[t] : 0.5 * ((double)tm[t] + (double)tm[(long long)c * p + r]) * 1.41421356237309504880;
+      const int idx = svec_idx(r, c);
+      s1[idx] = o;
+      y1[idx] = rho * (o - w[idx]);
+    }
+  }
+  for (long long t = t0; t < p; t += stride) L[t] = lam[lt.voff[lb] + t];
+}
+
+// FULL-checkpoint backward: bring (Vt, lam) of step k from the store into the large-path scratch layout.
+template <typename T>
+__global__ void k_large_fetch(PsdTab tab, LargeTab lt, const T* Ustore, const T* Lstore, T* Vt, T* lam) {
+  const int lb = blockIdx.y, blk = lt.gblk[lb];
+  const int p = tab.p[blk];
+  const T* U = Ustore + tab.uoff[blk];
+  const T* L = Lstore + tab.loff[blk];
+  const long long stride = (long long)gridDim.x * blockDim.x, t0 = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  for (long long t = t0; t < (long long)p * p; t += stride) Vt[lt.moff[lb] + t] = U[t];
+  for (long long t = t0; t < p; t += stride) lam[lt.voff[lb] + t] = L[t];
+}
+
+// g_w = -rho g_y + svec(Out); partial dots for g_rho.
+template <typename T>
+__global__ void __launch_bounds__(1024) k_large_finish_bwd(PsdTab tab, LargeTab lt, Hyper<T> H, int k, const T* Out,
+                                                           PsdBwdArgs A) {
+  __shared__ double sh[64];
+  const int lb = blockIdx.x, blk = lt.gblk[lb];
+  const int p = tab.p[blk];
+  const long long row0 = tab.row0[blk];
+  const double rho = H.rho_at(k, tab.prob[blk]);
+  const T* o = Out + lt.moff[lb];
+  const double *w = A.W + row0, *yk = A.Yk + row0, *s1 = A.S1 + row0, *gy = A.Gy + row0;
+  double* gw = A.GW + row0;
+  double acc[2] = {0.0, 0.0};
+  for (long long t = threadIdx.x; t < (long long)p * p; t += blockDim.x) {
+    const int r = (int)(t / p), c = (int)(t - (long long)r * p);
+    if (r <= c) {
+      const double ov = (r == c) ? (double)o[t] : 0.5 * ((double)o[t] + (double)o[(long long)c * p + r]) * 1.41421356237309504880;
+      const int idx = svec_idx(r, c);
+      const double gyv = gy[idx];
+      const double g = -rho * gyv + ov;
+      gw[idx] = g;
+      acc[0] += gyv * (s1[idx] - w[idx]);
+      acc[1] += g * yk[idx];
+    }
+  }
+  block_sum<2>(acc, sh);
+  if (threadIdx.x == 0) { A.part[2 * blk] = acc[0]; A.part[2 * blk + 1] = acc[1]; }
+}
+
+}  // namespace cdu

@@ -1,0 +1,144 @@
+"""Shared helpers of the GPU parity tests: run a Workload through the C ABI and through the oracle and
+compare norm-wise (reading A10). The oracle is imported here (tests only)."""
+from __future__ import annotations
+
+import numpy as np
+
+import workloads as W
+from oracle import cosmo_oracle as O
+
+TOL = {"f64": dict(iter=1e-9, grad=1e-7), "f32": dict(iter=1e-4, grad=1e-3)}   # BASELINE.json north_star
+
+
+def round_to(a, dtype):
+    a = np.asarray(a, np.float64)
+    return a.astype(np.float32).astype(np.float64) if dtype == "f32" else a
+
+
+def nrm_err(a, ref, fallback_scale=None):
+    """||a-ref||_inf / ||ref||_inf; identically-zero references are compared against `fallback_scale`."""
+    a = np.asarray(a, np.float64).ravel(); ref = np.asarray(ref, np.float64).ravel()
+    if ref.size == 0:
+        return 0.0
+    sc = np.max(np.abs(ref))
+    if sc == 0.0:
+        sc = fallback_scale if fallback_scale else 1.0
+    return float(np.max(np.abs(a - ref)) / sc)
+
+
+def oracle_reference(wl, problems=None, x_star=None):
+    """Oracle forward, terminal cotangent of the A13 loss (fp64, from the oracle's z_K, rounded to the GPU dtype
+    so both sides read identical numbers), oracle backward with that cotangent."""
+    idx = list(range(wl.batch)) if problems is None else list(problems)
+    ref = dict(idx=idx, xK=[], sK=[], yK=[], cot=[], g_x0=[], g_s0=[], g_y0=[], g_rho=[], g_alpha=[], g_sigma=[])
+    for b in idx:
+        pr = wl.problems[b]
+        un = O.unroll(pr, wl.K, wl.rho, wl.alpha, wl.sigma, wl.x0[b], wl.s0[b], wl.y0[b])
+        xK, sK, yK = un.xs[-1], un.ss[-1], un.ys[-1]
+        xs = np.zeros(pr.n) if x_star is None else x_star[b]
+        cot = tuple(round_to(c, wl.dtype) for c in O.terminal_loss_grad(pr, xK, sK, yK, xs))
+        g = O.backward(pr, un, *cot)
+        ref["xK"].append(xK); ref["sK"].append(sK); ref["yK"].append(yK); ref["cot"].append(cot)
+        ref["g_x0"].append(g.g_x0); ref["g_s0"].append(g.g_s0); ref["g_y0"].append(g.g_y0)
+        ref["g_rho"].append(g.g_rho_scalar); ref["g_alpha"].append(g.g_alpha); ref["g_sigma"].append(g.g_sigma)
+    return ref
+
+
+def gpu_run(wl, cot_full, ckpt_mode=0, per_problem=False, host=False, **opts):
+    """Forward + backward through the C ABI. cot_full: list over the WHOLE batch of (gx, gs, gy) or None (zeros).
+    Returns numpy results split per problem."""
+    import torch
+    import paper_2606_13825_b200 as cdu
+
+    packed = W.pack_batch(wl.problems, wl.dtype)
+    h = cdu.cdu_create(packed, K_max=wl.K, ckpt_mode=ckpt_mode, **opts)
+    tdt = torch.float32 if wl.dtype == "f32" else torch.float64
+    dev = "cpu" if host else "cuda"
+
+    def T(a):
+        t = torch.as_tensor(np.ascontiguousarray(a), dtype=tdt)
+        return t.pin_memory() if host else t.to(dev)
+
+    B = wl.batch
+    rho, alpha = wl.rho, wl.alpha
+    mode = cdu.CDU_RHO_PER_ITER
+    if per_problem:
+        rho = np.repeat(wl.rho[:, None], B, 1).ravel(); alpha = np.repeat(wl.alpha[:, None], B, 1).ravel()
+        mode = cdu.CDU_RHO_PER_PROBLEM
+    cat = lambda xs: np.concatenate(xs) if len(xs) else np.zeros(0)
+    xK, sK, yK = cdu.cdu_forward(h, wl.K, T(rho), T(alpha), wl.sigma, T(cat(wl.x0)), T(cat(wl.s0)), T(cat(wl.y0)),
+                                 rho_mode=mode, host=host)
+    if cot_full is None:
+        g = cdu.cdu_backward(h, host=host)
+    else:
+        g = cdu.cdu_backward(h, T(cat([c[0] for c in cot_full])), T(cat([c[1] for c in cot_full])),
+                             T(cat([c[2] for c in cot_full])), host=host)
+    if not host:
+        torch.cuda.synchronize()
+    st = cdu.cdu_get_stats(h)
+    vo, ro = packed["var_off"], packed["row_off"]
+    npy = lambda t: t.detach().cpu().numpy().astype(np.float64)
+    split = lambda v, off: [v[off[i]:off[i + 1]] for i in range(B)]
+    res = dict(xK=split(npy(xK), vo), sK=split(npy(sK), ro), yK=split(npy(yK), ro),
+               g_x0=split(npy(g["g_x0"]), vo), g_s0=split(npy(g["g_s0"]), ro), g_y0=split(npy(g["g_y0"]), ro),
+               stats=st)
+    if per_problem:
+        res["g_rho"] = npy(g["g_rho"]).reshape(wl.K, B); res["g_alpha"] = npy(g["g_alpha"]).reshape(wl.K, B)
+        res["g_sigma"] = npy(g["g_sigma"])
+    else:
+        res["g_rho"] = npy(g["g_rho"]); res["g_alpha"] = npy(g["g_alpha"]); res["g_sigma"] = float(npy(g["g_sigma"])[0])
+    cdu.cdu_destroy(h)
+    return res
+
+
+def compare(wl, ref, res, per_problem):
+    """Max norm-wise errors over the compared problems. Returns dict of errors."""
+    e = dict(x=0.0, s=0.0, y=0.0, g_x0=0.0, g_s0=0.0, g_y0=0.0)
+    for j, b in enumerate(ref["idx"]):
+        fb = max(np.max(np.abs(ref["xK"][j]), initial=0.0), np.max(np.abs(ref["yK"][j]), initial=0.0), 1e-300)
+        e["x"] = max(e["x"], nrm_err(res["xK"][b], ref["xK"][j], fb))
+        e["s"] = max(e["s"], nrm_err(res["sK"][b], ref["sK"][j], fb))
+        e["y"] = max(e["y"], nrm_err(res["yK"][b], ref["yK"][j], fb))
+        gfb = max(np.max(np.abs(ref[k][j]), initial=0.0) for k in ("g_x0", "g_s0", "g_y0")) or 1.0
+        for k in ("g_x0", "g_s0", "g_y0"):
+            e[k] = max(e[k], nrm_err(res[k][b], ref[k][j], gfb))
+    if per_problem:
+        e["g_rho"] = max(nrm_err(res["g_rho"][:, b], ref["g_rho"][j]) for j, b in enumerate(ref["idx"]))
+        e["g_alpha"] = max(nrm_err(res["g_alpha"][:, b], ref["g_alpha"][j]) for j, b in enumerate(ref["idx"]))
+        e["g_sigma"] = max(nrm_err([res["g_sigma"][b]], [ref["g_sigma"][j]]) for j, b in enumerate(ref["idx"]))
+    else:
+        assert len(ref["idx"]) == wl.batch
+        e["g_rho"] = nrm_err(res["g_rho"], np.sum(ref["g_rho"], axis=0))
+        e["g_alpha"] = nrm_err(res["g_alpha"], np.sum(ref["g_alpha"], axis=0))
+        e["g_sigma"] = nrm_err([res["g_sigma"]], [np.sum(ref["g_sigma"])])
+    return e
+
+
+def full_cotangent(wl, ref):
+    """Cotangent list for the whole batch: the oracle's for compared problems, zeros elsewhere."""
+    cots = [(np.zeros(pr.n), np.zeros(pr.m), np.zeros(pr.m)) for pr in wl.problems]
+    for j, b in enumerate(ref["idx"]):
+        cots[b] = ref["cot"][j]
+    return cots
+
+
+def check(wl, problems=None, per_problem=None, x_star=None, ckpt_mode=0, host=False, tol_scale=1.0, **opts):
+    """Oracle vs GPU on `problems` (default: all). Returns (errors, stats)."""
+    ref = oracle_reference(wl, problems, x_star)
+    if per_problem is None:
+        per_problem = problems is not None and len(list(problems)) != wl.batch
+    res = gpu_run(wl, full_cotangent(wl, ref), ckpt_mode=ckpt_mode, per_problem=per_problem, host=host, **opts)
+    e = compare(wl, ref, res, per_problem)
+    return e, res["stats"]
+
+
+def assert_within(e, dtype, tol_scale=1.0, skip=()):
+    t = TOL[dtype]
+    bad = {}
+    for k, v in e.items():
+        if k in skip:
+            continue
+        lim = (t["iter"] if k in ("x", "s", "y") else t["grad"]) * tol_scale
+        if not (v <= lim):
+            bad[k] = (v, lim)
+    assert not bad, f"parity failures (value, limit): {bad}; all errors: {e}"
