@@ -112,6 +112,7 @@ typedef struct {
   int64_t device_bytes;      /* bytes of device memory owned by the handle                                  */
   int64_t ckpt_bytes;        /* of which checkpoint store                                                   */
   int64_t launches;          /* kernel launches issued by the handle since creation                         */
+  int64_t eig_sweeps_sum;    /* Jacobi sweeps summed over PSD blocks and iterations of the last forward     */
 } cdu_stats;
 
 /* Synchronises the stream of the last call and reads back the per-problem counters. */
@@ -123,6 +124,15 @@ cdu_status cdu_get_iterate(cdu_handle h, int32_t k, void* x, void* s, void* y, i
 const char* cdu_last_error(cdu_handle h); /* valid until the next call on h; h may be NULL (create errors) */
 cdu_status  cdu_destroy(cdu_handle h);
 const char* cdu_version(void);
+
+/* ---- per-kernel-class timing (CUDA events on the launching stream; used by bench.py's roofline leg) ---------
+ * Classes: 0 linear step forward (xi, PCG, relaxation, zero/nonneg/SOC), 1 PSD forward small (shared-memory
+ * Jacobi + rebuild), 2 large-block eigendecomposition, 3 large-block GEMMs (rebuild / DK), 4 linear step
+ * backward (adjoint PCG, Eq. 6), 5 PSD backward small (DK), 6 large-block glue, 7 other. cdu_get_profile
+ * synchronises on the recorded events, returns summed milliseconds and launch counts since the last call. */
+#define CDU_PROFILE_CLASSES 8
+cdu_status cdu_profile(cdu_handle h, int32_t enable);
+cdu_status cdu_get_profile(cdu_handle h, int32_t nclass, double* ms, int64_t* count);
 
 /* ---- stand-alone operator entry points (unit tests, micro-benchmarks, ncu isolation) ------------------------
  * Batched PSD projection S -> Pi(S) = U max(L,0) U' (Eq. 7) and its Dalecki-Krein VJP (Eq. 9-10) on `count`

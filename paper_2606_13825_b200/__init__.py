@@ -27,7 +27,7 @@ CDU_CKPT_FULL, CDU_CKPT_LEAN = 0, 1
 _STATUS = {0: "CDU_OK", 1: "CDU_EINVAL", 2: "CDU_ENOMEM", 3: "CDU_ECUDA", 4: "CDU_ESTATE", 5: "CDU_ENUMERIC"}
 
 EXPORTED_SYMBOLS = ("cdu_create", "cdu_forward", "cdu_backward", "cdu_get_stats", "cdu_get_iterate", "cdu_last_error",
-                    "cdu_destroy", "cdu_version", "cdu_psd_project", "cdu_psd_vjp")
+                    "cdu_destroy", "cdu_version", "cdu_psd_project", "cdu_psd_vjp", "cdu_profile", "cdu_get_profile")
 
 
 class CduError(RuntimeError):
@@ -57,7 +57,8 @@ class _Options(C.Structure):
 class _Stats(C.Structure):
     _fields_ = [("cg_iters_fwd", C.c_int64), ("cg_iters_bwd", C.c_int64), ("cg_iters_max", C.c_int32),
                 ("eig_sweeps_max", C.c_int32), ("n_flagged", C.c_int32), ("flags_or", C.c_int32),
-                ("device_bytes", C.c_int64), ("ckpt_bytes", C.c_int64), ("launches", C.c_int64)]
+                ("device_bytes", C.c_int64), ("ckpt_bytes", C.c_int64), ("launches", C.c_int64),
+                ("eig_sweeps_sum", C.c_int64)]
 
 
 _lib = None
@@ -89,6 +90,10 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.cdu_destroy.argtypes = [vp]
     lib.cdu_version.restype = C.c_char_p
     lib.cdu_version.argtypes = []
+    lib.cdu_profile.restype = i32
+    lib.cdu_profile.argtypes = [vp, i32]
+    lib.cdu_get_profile.restype = i32
+    lib.cdu_get_profile.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
     lib.cdu_psd_project.restype = i32
     lib.cdu_psd_project.argtypes = [i32, i32, i32, vp, vp, vp, vp, i32, i32, vp]
     lib.cdu_psd_vjp.restype = i32
@@ -196,6 +201,17 @@ class Handle:
         s = _Stats()
         self._check(self.lib.cdu_get_stats(self.h, C.byref(s)))
         return {k: getattr(s, k) for k, _ in _Stats._fields_}
+
+    PROFILE_CLASSES = ("lin_fwd", "psd_fwd_small", "eig_large", "gemm_large", "lin_bwd", "psd_bwd_small", "large_misc", "misc")
+
+    def profile(self, enable: bool):
+        self._check(self.lib.cdu_profile(self.h, 1 if enable else 0))
+
+    def get_profile(self) -> dict:
+        n = len(self.PROFILE_CLASSES)
+        ms = (C.c_double * n)(); cnt = (C.c_int64 * n)()
+        self._check(self.lib.cdu_get_profile(self.h, n, ms, cnt))
+        return {name: dict(ms=ms[i], launches=cnt[i]) for i, name in enumerate(self.PROFILE_CLASSES)}
 
     def close(self):
         if getattr(self, "h", None):

@@ -31,6 +31,8 @@ struct cdu_handle_s {
                               void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st) = 0;
   virtual cdu_status stats(cdu_stats* out) = 0;
   virtual cdu_status iterate(int k, void* x, void* s, void* y, int host, cudaStream_t st) = 0;
+  virtual void profile_enable(int on) = 0;
+  virtual void profile_collect(double* ms, long long* cnt) = 0;
 };
 
 namespace {
@@ -66,6 +68,37 @@ struct DevPool {  // owns device allocations
   ~DevPool() { release(); }
 };
 
+// Optional per-kernel-class timing with CUDA events on the launching stream (bench.py's roofline leg).
+enum ProfClass { PC_LIN_FWD = 0, PC_PSD_FWD_SMALL, PC_EIG_LARGE, PC_GEMM_LARGE, PC_LIN_BWD, PC_PSD_BWD_SMALL, PC_LARGE_MISC, PC_MISC, PC_COUNT };
+struct Prof {
+  bool on = false;
+  std::vector<cudaEvent_t> pool;
+  std::vector<int> cls;
+  size_t used = 0;
+  void begin(int c, cudaStream_t st) {
+    if (!on) return;
+    if (used + 2 > pool.size()) { cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b); pool.push_back(a); pool.push_back(b); }
+    cls.push_back(c);
+    cudaEventRecord(pool[used], st);
+  }
+  void end(cudaStream_t st) {
+    if (!on) return;
+    cudaEventRecord(pool[used + 1], st);
+    used += 2;
+  }
+  void collect(double* ms, long long* cnt) {
+    for (int i = 0; i < PC_COUNT; ++i) { ms[i] = 0; cnt[i] = 0; }
+    for (size_t i = 0; i < cls.size(); ++i) {
+      float t = 0.f;
+      cudaEventSynchronize(pool[2 * i + 1]);
+      cudaEventElapsedTime(&t, pool[2 * i], pool[2 * i + 1]);
+      ms[cls[i]] += t; cnt[cls[i]] += 1;
+    }
+    cls.clear(); used = 0;
+  }
+  ~Prof() { for (auto e : pool) cudaEventDestroy(e); }
+};
+
 inline int pow2_group(double avg) {
   int g = 1;
   while (g < 32 && g < avg * 0.5) g <<= 1;
@@ -95,9 +128,13 @@ struct PsdEngine {
   float* tc_split = nullptr;   // hi/lo operand staging of the tcgen05 path
   int* rotflags = nullptr;
   int* sweeps_max = nullptr;
+  unsigned long long* sweeps_sum = nullptr;
   int small_threads = 256;
   int use_tc = 0;
   long long launches = 0;
+  Prof* prof = nullptr;
+  void pb(int c, cudaStream_t st) { if (prof) prof->begin(c, st); }
+  void pe(cudaStream_t st) { if (prof) prof->end(st); }
   std::vector<int> h_large_p;
   size_t sum_p2 = 0, sum_p = 0;
 
@@ -122,6 +159,7 @@ struct PsdEngine {
     tab.uoff = pool.upload(uoff, st); tab.loff = pool.upload(loff, st);
     d_small_list = pool.upload(small_list, st);
     sweeps_max = pool.zeros<int>(1, st);
+    sweeps_sum = pool.zeros<unsigned long long>(1, st);
     small_threads = pmax_small <= 64 ? 256 : 512;
     if (n_large) {
       lt.nblk = n_large; lt.pmax = pmax_large;
@@ -145,6 +183,12 @@ struct PsdEngine {
   }
 
   cdu_status gemm(const T* A, int ta, const T* Bm, int tb, T* C, const T* kscale, int relu, cudaStream_t st) {
+    pb(PC_GEMM_LARGE, st);
+    cdu_status s = gemm_(A, ta, Bm, tb, C, kscale, relu, st);
+    pe(st);
+    return s;
+  }
+  cdu_status gemm_(const T* A, int ta, const T* Bm, int tb, T* C, const T* kscale, int relu, cudaStream_t st) {
     if (use_tc) {
       cdu_status s = gemm_tc_batched(n_large, h_large_p.data(), lt.pvec, lt.moff, lt.voff, (const float*)A, ta,
                                      (const float*)Bm, tb, (float*)C, (const float*)kscale, relu, tc_split, st, &launches, err);
@@ -169,13 +213,15 @@ struct PsdEngine {
     const int maxsw = HESTENES_MAXSW - 1;
     int nl = n_large;
     const int* pv = lt.pvec; const long long* mo = lt.moff; const int* vo = lt.voff;
-    T *g = G, *v = Vt, *l = lamL; const T* m = mu; int* rf = rotflags; int* sw = sweeps_max;
+    T *g = G, *v = Vt, *l = lamL; const T* m = mu; int* rf = rotflags; int* sw = sweeps_max; unsigned long long* ss = sweeps_sum;
     cudaError_t e;
-    if (pmax_large <= 128) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 4>, nl, pv, mo, vo, g, v, m, l, rf, sw, maxsw, tol);
-    else if (pmax_large <= 256) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 8>, nl, pv, mo, vo, g, v, m, l, rf, sw, maxsw, tol);
-    else if (pmax_large <= 512) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 16>, nl, pv, mo, vo, g, v, m, l, rf, sw, maxsw, tol);
-    else if (pmax_large <= 1024) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 32>, nl, pv, mo, vo, g, v, m, l, rf, sw, maxsw, tol);
+    pb(PC_EIG_LARGE, st);
+    if (pmax_large <= 128) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 4>, nl, pv, mo, vo, g, v, m, l, rf, sw, ss, maxsw, tol);
+    else if (pmax_large <= 256) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 8>, nl, pv, mo, vo, g, v, m, l, rf, sw, ss, maxsw, tol);
+    else if (pmax_large <= 512) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 16>, nl, pv, mo, vo, g, v, m, l, rf, sw, ss, maxsw, tol);
+    else if (pmax_large <= 1024) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 32>, nl, pv, mo, vo, g, v, m, l, rf, sw, ss, maxsw, tol);
     else { err = "PSD block order > 1024 not supported"; return CDU_EINVAL; }
+    pe(st);
     ++launches;
     CU_OK(e);
     return CDU_OK;
@@ -183,19 +229,25 @@ struct PsdEngine {
 
   cdu_status forward(const Hyper<T>& H, int k, const PsdFwdArgs& A, cudaStream_t st) {
     if (n_small) {
+      pb(PC_PSD_FWD_SMALL, st);
       k_psd_fwd_small<T><<<n_small, small_threads, psd_small_smem_fwd(pmax_small, sizeof(T)), st>>>(tab, H, k, A, d_small_list);
+      pe(st);
       ++launches;
       CU_OK(cudaGetLastError());
     }
     if (n_large) {
+      pb(PC_LARGE_MISC, st);
       k_large_smat<T><<<n_large, 1024, 0, st>>>(tab, lt, A.W, nullptr, H, k, 0, 1, G, Vt, mu);
+      pe(st);
       ++launches;
       CU_OK(cudaGetLastError());
       cdu_status s = eig_large(st);
       if (s != CDU_OK) return s;
       s = gemm(Vt, 1, Vt, 0, Tm, lamL, 1, st);          // Tm = Vt' diag(lam+) Vt
       if (s != CDU_OK) return s;
+      pb(PC_LARGE_MISC, st);
       k_large_finish_fwd<T><<<dim3(64, n_large), 256, 0, st>>>(tab, lt, H, k, Tm, Vt, lamL, A);
+      pe(st);
       ++launches;
       CU_OK(cudaGetLastError());
     }
@@ -204,34 +256,46 @@ struct PsdEngine {
 
   cdu_status backward(const Hyper<T>& H, int k, const PsdBwdArgs& A, cudaStream_t st) {
     if (n_small) {
+      pb(PC_PSD_BWD_SMALL, st);
       k_psd_bwd_small<T><<<n_small, small_threads, psd_small_smem_bwd(pmax_small, sizeof(T)), st>>>(tab, H, k, A, d_small_list);
+      pe(st);
       ++launches;
       CU_OK(cudaGetLastError());
     }
     if (n_large) {
       if (A.recompute) {
-        k_large_smat<T><<<n_large, 1024, 0, st>>>(tab, lt, A.W, nullptr, H, k, 0, 1, G, Vt, mu);
+        pb(PC_LARGE_MISC, st);
+      k_large_smat<T><<<n_large, 1024, 0, st>>>(tab, lt, A.W, nullptr, H, k, 0, 1, G, Vt, mu);
+      pe(st);
         ++launches;
         CU_OK(cudaGetLastError());
         cdu_status s = eig_large(st);
         if (s != CDU_OK) return s;
       } else {
-        k_large_fetch<T><<<dim3(64, n_large), 256, 0, st>>>(tab, lt, (const T*)A.Ustore, (const T*)A.Lstore, Vt, lamL);
+        pb(PC_LARGE_MISC, st);
+      k_large_fetch<T><<<dim3(64, n_large), 256, 0, st>>>(tab, lt, (const T*)A.Ustore, (const T*)A.Lstore, Vt, lamL);
+      pe(st);
         ++launches;
         CU_OK(cudaGetLastError());
       }
+      pb(PC_LARGE_MISC, st);
       k_large_smat<T><<<n_large, 1024, 0, st>>>(tab, lt, A.Gs, A.Gy, H, k, 1, 0, G, nullptr, nullptr);   // G = smat(g_s + rho g_y)
+      pe(st);
       ++launches;
       CU_OK(cudaGetLastError());
       cdu_status s;
       if ((s = gemm(Vt, 0, G, 0, Tm, nullptr, 0, st)) != CDU_OK) return s;     // Tm = Vt G
       if ((s = gemm(Tm, 0, Vt, 1, G, nullptr, 0, st)) != CDU_OK) return s;     // C  = Tm Vt'
+      pb(PC_LARGE_MISC, st);
       k_large_hadamard<T><<<dim3(64, n_large), 256, 0, st>>>(n_large, lt.pvec, lt.moff, lt.voff, G, lamL);
+      pe(st);
       ++launches;
       CU_OK(cudaGetLastError());
       if ((s = gemm(Vt, 1, G, 0, Tm, nullptr, 0, st)) != CDU_OK) return s;     // Tm = Vt' C
       if ((s = gemm(Tm, 0, Vt, 0, G, nullptr, 0, st)) != CDU_OK) return s;     // out = Tm Vt
+      pb(PC_LARGE_MISC, st);
       k_large_finish_bwd<T><<<n_large, 1024, 0, st>>>(tab, lt, H, k, G, A);
+      pe(st);
       ++launches;
       CU_OK(cudaGetLastError());
     }
@@ -267,6 +331,7 @@ struct HandleT : cdu_handle_s {
   long long launches = 0;
   cudaStream_t last_stream = nullptr;
   bool has_psd = false;
+  Prof prof;
 
   double* z_at(int k) { return Z + (size_t)k * zstride; }
 
@@ -283,6 +348,8 @@ struct HandleT : cdu_handle_s {
                       void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st) override;
   cdu_status stats(cdu_stats* out) override;
   cdu_status iterate(int k, void* x, void* s, void* y, int host, cudaStream_t st) override;
+  void profile_enable(int on) override { prof.on = on != 0; }
+  void profile_collect(double* ms, long long* cnt) override { prof.collect(ms, cnt); }
   cdu_status export_state(const double* z, void* x, void* s, void* y, int host, cudaStream_t st);
   cdu_status import_state(double* z, const void* x, const void* s, const void* y, int host, cudaStream_t st);
 };
@@ -418,6 +485,7 @@ cdu_status HandleT<T>::init(const cdu_problem* pr, const cdu_options* op, cudaSt
 
   // ---- PSD engine -----------------------------------------------------------------------------------------
   {
+    psd.prof = &prof;
     cdu_status s = psd.build(pool, psd_prob, psd_row0, psd_p, small_max, o.use_tensor_cores, st);
     if (s != CDU_OK) { err = psd.err; return s; }
   }
@@ -501,6 +569,7 @@ cdu_status HandleT<T>::forward(int K, const void* rho, int mode, double sigma, c
   CU_OK(cudaMemsetAsync(cg_max, 0, B * sizeof(int), st));
   CU_OK(cudaMemsetAsync(flags, 0, B * sizeof(int), st));
   CU_OK(cudaMemsetAsync(psd.sweeps_max, 0, sizeof(int), st));
+  CU_OK(cudaMemsetAsync(psd.sweeps_sum, 0, sizeof(unsigned long long), st));
   const Hyper<T> H = hyper();
   BatchDev<T> Df = D; Df.cg_iters = cg_f;
   const bool full = ckpt_mode == CDU_CKPT_FULL;
@@ -508,14 +577,16 @@ cdu_status HandleT<T>::forward(int K, const void* rho, int mode, double sigma, c
     IterPtrs I;
     I.Zk = z_at(k); I.Zk1 = z_at(k + 1);
     I.XT = XT + (full ? (size_t)k * N : 0); I.ST = ST + (full ? (size_t)k * Mtot : 0);
+    prof.begin(PC_LIN_FWD, st);
     k_fwd<T><<<B, lin_threads, 0, st>>>(Df, H, I, k);
+    prof.end(st);
     ++launches;
     CU_OK(cudaGetLastError());
     if (has_psd) {
       PsdFwdArgs A;
       A.W = D.W; A.S1 = z_at(k + 1) + N; A.Y1 = z_at(k + 1) + N + Mtot;
       A.Ustore = Ustore + (full ? (size_t)k * psd.sum_p2 : 0); A.Lstore = Lstore + (full ? (size_t)k * psd.sum_p : 0);
-      A.sweeps_max = psd.sweeps_max; A.flags = flags;
+      A.sweeps_max = psd.sweeps_max; A.flags = flags; A.sweeps_sum = psd.sweeps_sum;
       s = psd.forward(H, k, A, st);
       if (s != CDU_OK) { err = psd.err; return s; }
     }
@@ -547,11 +618,15 @@ cdu_status HandleT<T>::backward(const void* gx, const void* gs, const void* gy, 
     Q.g_rho_pb = g_rho_pb; Q.g_alpha_pb = g_alpha_pb; Q.g_sigma_pb = g_sigma_pb; Q.part_pre = part_pre;
     Q.recompute = full ? 0 : 1;
     if (!has_psd) {
+      prof.begin(PC_LIN_BWD, st);
       k_bwd<T><<<B, lin_threads, 0, st>>>(Db, H, Q, k, 0);
+      prof.end(st);
       ++launches;
       CU_OK(cudaGetLastError());
     } else {
+      prof.begin(PC_LIN_BWD, st);
       k_bwd<T><<<B, lin_threads, 0, st>>>(Db, H, Q, k, 1);
+      prof.end(st);
       ++launches;
       CU_OK(cudaGetLastError());
       PsdBwdArgs A;
@@ -561,7 +636,9 @@ cdu_status HandleT<T>::backward(const void* gx, const void* gs, const void* gy, 
       A.recompute = full ? 0 : 1; A.flags = flags;
       s = psd.backward(H, k, A, st);
       if (s != CDU_OK) { err = psd.err; return s; }
+      prof.begin(PC_LIN_BWD, st);
       k_bwd<T><<<B, lin_threads, 0, st>>>(Db, H, Q, k, 2);
+      prof.end(st);
       ++launches;
       CU_OK(cudaGetLastError());
     }
@@ -606,6 +683,8 @@ cdu_status HandleT<T>::stats(cdu_stats* out) {
   CU_OK(cudaMemcpy(mx.data(), cg_max, B * sizeof(int), cudaMemcpyDeviceToHost));
   CU_OK(cudaMemcpy(fl.data(), flags, B * sizeof(int), cudaMemcpyDeviceToHost));
   CU_OK(cudaMemcpy(&sw, psd.sweeps_max, sizeof(int), cudaMemcpyDeviceToHost));
+  unsigned long long ssum = 0;
+  CU_OK(cudaMemcpy(&ssum, psd.sweeps_sum, sizeof(ssum), cudaMemcpyDeviceToHost));
   std::memset(out, 0, sizeof(*out));
   for (int b = 0; b < B; ++b) {
     out->cg_iters_fwd += f[b]; out->cg_iters_bwd += bw[b];
@@ -613,6 +692,7 @@ cdu_status HandleT<T>::stats(cdu_stats* out) {
     if (fl[b]) { ++out->n_flagged; out->flags_or |= fl[b]; }
   }
   out->eig_sweeps_max = sw;
+  out->eig_sweeps_sum = (int64_t)ssum;
   out->device_bytes = (int64_t)pool.bytes; out->ckpt_bytes = (int64_t)ckpt_bytes;
   out->launches = launches + psd.launches;
   return CDU_OK;
@@ -691,7 +771,7 @@ cdu_status psd_op_t(bool vjp, int count, int p, const void* in1, const void* in2
   const bool large = eng.n_large > 0;
   if (!vjp) {
     k_dense_to_svec<T><<<count, 256, 0, st>>>(p, (const T*)in1, W);
-    PsdFwdArgs A; A.W = W; A.S1 = S1; A.Y1 = Y1; A.Ustore = Us; A.Lstore = Ls; A.sweeps_max = eng.sweeps_max; A.flags = flags;
+    PsdFwdArgs A; A.W = W; A.S1 = S1; A.Y1 = Y1; A.Ustore = Us; A.Lstore = Ls; A.sweeps_max = eng.sweeps_max; A.flags = flags; A.sweeps_sum = eng.sweeps_sum;
     s = eng.forward(H, 0, A, st);
     if (s != CDU_OK) { err = eng.err; return s; }
     k_svec_to_dense<T><<<count, 256, 0, st>>>(p, S1, (T*)out1);
@@ -765,6 +845,20 @@ cdu_status cdu_destroy(cdu_handle h) {
 }
 
 const char* cdu_version(void) { return "cdu 0.1 (sm_100a)"; }
+
+cdu_status cdu_profile(cdu_handle h, int32_t enable) {
+  if (!h) return CDU_EINVAL;
+  h->profile_enable(enable);
+  return CDU_OK;
+}
+
+cdu_status cdu_get_profile(cdu_handle h, int32_t nclass, double* ms, int64_t* count) {
+  if (!h || !ms || !count || nclass < 1) return CDU_EINVAL;
+  double m[PC_COUNT]; long long c[PC_COUNT];
+  h->profile_collect(m, c);
+  for (int i = 0; i < nclass; ++i) { ms[i] = i < PC_COUNT ? m[i] : 0.0; count[i] = i < PC_COUNT ? c[i] : 0; }
+  return CDU_OK;
+}
 
 cdu_status cdu_psd_project(int32_t dtype, int32_t count, int32_t p, const void* S, void* PiS, void* U, void* lam,
                            int32_t path, int32_t use_tensor_cores, void* cuda_stream) {

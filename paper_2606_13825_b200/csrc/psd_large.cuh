@@ -79,8 +79,8 @@ constexpr int HESTENES_MAXSW = 64;
 // One cluster per matrix. G, Vt: p x p row-major with column i of the working matrix stored as row i.
 template <typename T, int NE>
 __global__ void __launch_bounds__(512) k_hestenes(int nblk, const int* pvec, const long long* moff, const int* voff, T* G, T* Vt,
-                                                  const T* mu, T* lam, int* rotflags, int* sweeps_out, int max_sweeps,
-                                                  double tol) {
+                                                  const T* mu, T* lam, int* rotflags, int* sweeps_out, unsigned long long* sweeps_sum,
+                                                  int max_sweeps, double tol) {
   cg::cluster_group cluster = cg::this_cluster();
   const int C = cluster.num_blocks();
   const int lb = blockIdx.x / C, rank = cluster.block_rank();
@@ -110,16 +110,16 @@ __global__ void __launch_bounds__(512) k_hestenes(int nblk, const int* pvec, con
           const double zeta = (b - a) / (2.0 * c);
           const double t = (zeta >= 0.0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
           const double cd = 1.0 / sqrt(1.0 + t * t);
-          const T cs = (T)cd, sn = (T)(t * cd);
+          const T sn = (T)(t * cd), tau = (T)(t * cd / (1.0 + cd));      // Rutishauser form, see psd_small.cuh
 #pragma unroll
           for (int e = 0; e < NE; ++e) {
             const int col = lane + 32 * e;
             if (col < p) {
-              __stcg(g + (long long)i * p + col, cs * gi[e] - sn * gj[e]);
-              __stcg(g + (long long)j * p + col, sn * gi[e] + cs * gj[e]);
+              __stcg(g + (long long)i * p + col, gi[e] - sn * (gj[e] + tau * gi[e]));
+              __stcg(g + (long long)j * p + col, gj[e] + sn * (gi[e] - tau * gj[e]));
               const T vi = __ldcg(vt + (long long)i * p + col), vj = __ldcg(vt + (long long)j * p + col);
-              __stcg(vt + (long long)i * p + col, cs * vi - sn * vj);
-              __stcg(vt + (long long)j * p + col, sn * vi + cs * vj);
+              __stcg(vt + (long long)i * p + col, vi - sn * (vj + tau * vi));
+              __stcg(vt + (long long)j * p + col, vj + sn * (vi - tau * vj));
             }
           }
           if (lane == 0) rf[sweep] = 1;
@@ -137,7 +137,7 @@ __global__ void __launch_bounds__(512) k_hestenes(int nblk, const int* pvec, con
     a = warp_sum(a);
     if (lane == 0) lam[voff[lb] + i] = (T)(sqrt(a) - (double)mu[lb]);
   }
-  if (rank == 0 && threadIdx.x == 0) atomicMax(sweeps_out, sweep);
+  if (rank == 0 && threadIdx.x == 0) { atomicMax(sweeps_out, sweep); if (sweeps_sum) atomicAdd(sweeps_sum, (unsigned long long)sweep); }
 }
 
 // Batched row-major GEMM C = op(A) op(B) (p x p x p per block), FMA path. 64x64 tile, 16x16 threads, 4x4 each.

@@ -69,36 +69,42 @@ __device__ int jacobi_smem(int pe, int ld, T* S, T* V, T* cs, double* shred, int
       for (int q = tid; q < h; q += nt) {
         int i, j; rr_pair(r, q, pe, i, j);
         const T aij = S[i * ld + j];
-        T c = (T)1, s = (T)0;
+        // Rutishauser form: x' = x - s (y + tau x), y' = y + s (x - tau y), tau = s / (1 + c). The deviation from
+        // orthogonality is O((1-c) eps) per rotation instead of O(eps), so V stays orthogonal to a few eps.
+        T sn = (T)0, tau = (T)0, tt = (T)0;
         if (fabs(aij) > skip) {
-          const T tau = (S[j * ld + j] - S[i * ld + i]) / ((T)2 * aij);
-          const T t = (tau >= (T)0 ? (T)1 : (T)-1) / (fabs(tau) + sqrt((T)1 + tau * tau));
-          c = (T)1 / sqrt((T)1 + t * t);
-          s = t * c;
+          const double th = ((double)S[j * ld + j] - (double)S[i * ld + i]) / (2.0 * (double)aij);
+          const double t = (th >= 0.0 ? 1.0 : -1.0) / (fabs(th) + sqrt(1.0 + th * th));
+          const double c = 1.0 / sqrt(1.0 + t * t);
+          sn = (T)(t * c); tau = (T)(t * c / (1.0 + c)); tt = (T)t;
         }
-        cs[2 * q] = c; cs[2 * q + 1] = s;
+        cs[3 * q] = sn; cs[3 * q + 1] = tau; cs[3 * q + 2] = tt;
       }
       __syncthreads();
       for (int t = tid; t < h * h; t += nt) {
         const int q1 = t / h, q2 = t - q1 * h;
         int i1, j1, i2, j2;
         rr_pair(r, q1, pe, i1, j1); rr_pair(r, q2, pe, i2, j2);
-        const T c1 = cs[2 * q1], s1 = cs[2 * q1 + 1], c2 = cs[2 * q2], s2 = cs[2 * q2 + 1];
+        const T s1 = cs[3 * q1], t1 = cs[3 * q1 + 1], s2 = cs[3 * q2], t2 = cs[3 * q2 + 1];
         T a = S[i1 * ld + i2], b = S[i1 * ld + j2], c = S[j1 * ld + i2], d = S[j1 * ld + j2];
-        const T ra = c1 * a - s1 * c, rc = s1 * a + c1 * c;      // rows:  J' S
-        const T rb = c1 * b - s1 * d, rd = s1 * b + c1 * d;
-        a = c2 * ra - s2 * rb; b = s2 * ra + c2 * rb;            // cols:  (.) J
-        c = c2 * rc - s2 * rd; d = s2 * rc + c2 * rd;
-        if (q1 == q2) { b = (T)0; c = (T)0; }
+        if (q1 == q2) {
+          const T g = cs[3 * q1 + 2] * b;                        // t * a_ij
+          a -= g; d += g; b = (T)0; c = (T)0;
+        } else {
+          const T ra = a - s1 * (c + t1 * a), rc = c + s1 * (a - t1 * c);   // rows:  J' S
+          const T rb = b - s1 * (d + t1 * b), rd = d + s1 * (b - t1 * d);
+          a = ra - s2 * (rb + t2 * ra); b = rb + s2 * (ra - t2 * rb);       // cols:  (.) J
+          c = rc - s2 * (rd + t2 * rc); d = rd + s2 * (rc - t2 * rd);
+        }
         S[i1 * ld + i2] = a; S[i1 * ld + j2] = b; S[j1 * ld + i2] = c; S[j1 * ld + j2] = d;
       }
       for (int t = tid; t < pe * h; t += nt) {
         const int row = t / h, q2 = t - row * h;
         int i2, j2; rr_pair(r, q2, pe, i2, j2);
-        const T c2 = cs[2 * q2], s2 = cs[2 * q2 + 1];
+        const T s2 = cs[3 * q2], t2 = cs[3 * q2 + 1];
         const T a = V[row * ld + i2], b = V[row * ld + j2];
-        V[row * ld + i2] = c2 * a - s2 * b;
-        V[row * ld + j2] = s2 * a + c2 * b;
+        V[row * ld + i2] = a - s2 * (b + t2 * a);
+        V[row * ld + j2] = b + s2 * (a - t2 * b);
       }
       __syncthreads();
     }
@@ -151,6 +157,7 @@ struct PsdFwdArgs {
   void* Ustore;      // eigenvector store of this iteration (or scratch)
   void* Lstore;
   int* sweeps_max; int* flags;
+  unsigned long long* sweeps_sum;   // total Jacobi sweeps over blocks (statistics for the ALU roofline)
 };
 
 template <typename T>
@@ -164,7 +171,7 @@ __global__ void __launch_bounds__(512) k_psd_fwd_small(PsdTab tab, Hyper<T> H, i
   T* S = reinterpret_cast<T*>(shred + 32);
   T* V = S + pe * ld;
   T* cs = V + pe * ld;
-  T* lp = cs + pe;
+  T* lp = cs + 2 * pe;
   const double rho = H.rho_at(k, prob);
   const double* w = A.W + row0;
   load_smat<T>(p, pe, ld, S, w, 0.0, nullptr);
@@ -196,6 +203,7 @@ __global__ void __launch_bounds__(512) k_psd_fwd_small(PsdTab tab, Hyper<T> H, i
   }
   if (threadIdx.x == 0) {
     atomicMax(A.sweeps_max, sweeps);
+    if (A.sweeps_sum) atomicAdd(A.sweeps_sum, (unsigned long long)sweeps);
     if (flag) atomicOr(A.flags + prob, flag);
   }
 }
@@ -225,7 +233,7 @@ __global__ void __launch_bounds__(512) k_psd_bwd_small(PsdTab tab, Hyper<T> H, i
   T* G = V + pe * ld;       // S during a recompute, then smat(G), then C
   T* Tm = G + pe * ld;      // V accumulates here during recompute? no: scratch product
   T* cs = Tm + pe * ld;
-  T* lam = cs + pe;
+  T* lam = cs + 2 * pe;
   const double rho = H.rho_at(k, prob);
   const double* w = A.W + row0;
   int flag = 0;
@@ -287,7 +295,7 @@ __global__ void __launch_bounds__(512) k_psd_bwd_small(PsdTab tab, Hyper<T> H, i
   }
 }
 
-static inline size_t psd_small_smem_fwd(int p, size_t sz) { const int pe = (p + 1) & ~1; return 32 * 8 + (2 * (size_t)pe * pe + 2 * pe) * sz; }
-static inline size_t psd_small_smem_bwd(int p, size_t sz) { const int pe = (p + 1) & ~1; return 64 * 8 + (3 * (size_t)pe * pe + 2 * pe) * sz; }
+static inline size_t psd_small_smem_fwd(int p, size_t sz) { const int pe = (p + 1) & ~1; return 32 * 8 + (2 * (size_t)pe * pe + 3 * pe) * sz; }
+static inline size_t psd_small_smem_bwd(int p, size_t sz) { const int pe = (p + 1) & ~1; return 64 * 8 + (3 * (size_t)pe * pe + 3 * pe) * sz; }
 
 }  // namespace cdu

@@ -1,0 +1,187 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the fp64 oracle on the same seeded inputs.
+
+Tolerances are BASELINE.json north_star's: fp64 <= 1e-9 (iterates) / 1e-7 (gradients); fp32 <= 1e-4 / 1e-3,
+norm-wise per vector and per problem (reading A10)."""
+import numpy as np
+import pytest
+
+import workloads as W
+from workloads.generators import ZERO, NONNEG, SOC, PSD, Workload, Problem, _round_problem
+
+import parity_util as PU
+
+pytestmark = pytest.mark.gpu
+
+
+def _mixed_workload(dtype, seed=5, B=3, K=6, cones=((ZERO, 2), (NONNEG, 3), (SOC, 4), (PSD, 3), (SOC, 2), (PSD, 5)), n=9):
+    rng = np.random.default_rng(seed)
+    probs = [_round_problem(W.random_mixed_problem(rng, n=n, cones=cones), dtype) for _ in range(B)]
+    rd = lambda a: PU.round_to(a, dtype)
+    return Workload("mixed", dtype, probs, K, rd(np.exp(rng.uniform(-1, 1, K))), rd(rng.uniform(1, 1.8, K)), 1e-6,
+                    [rd(0.1 * rng.standard_normal(p.n)) for p in probs], [rd(0.1 * rng.standard_normal(p.m)) for p in probs],
+                    [rd(0.1 * rng.standard_normal(p.m)) for p in probs])
+
+
+# ---- cfg1: the fp64 bar, full size, loss of reading A13 -------------------------------------------------
+@pytest.mark.parametrize("ckpt", [0, 1])
+def test_cfg1_fp64_full(ckpt):
+    from oracle import cosmo_oracle as O
+    wl = W.make_config(1)
+    x_star = [O.solve_to_convergence(pr, iters=5000, rho=1.0, alpha=1.6)[0] for pr in wl.problems]
+    e, st = PU.check(wl, x_star=x_star, ckpt_mode=ckpt)
+    PU.assert_within(e, "f64")
+    assert st["flags_or"] == 0 and st["cg_iters_max"] <= 2          # M is diagonal for max-cut
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("ckpt", [0, 1])
+def test_all_cone_types_ragged_batch(dtype, ckpt):
+    wl = _mixed_workload(dtype)
+    wl.problems[1] = _round_problem(W.random_mixed_problem(np.random.default_rng(9), n=6, cones=((PSD, 4), (SOC, 3), (ZERO, 1))), dtype)
+    pr = wl.problems[1]
+    wl.x0[1], wl.s0[1], wl.y0[1] = np.zeros(pr.n), np.zeros(pr.m), np.zeros(pr.m)
+    e, st = PU.check(wl, ckpt_mode=ckpt)
+    PU.assert_within(e, dtype)
+    assert st["flags_or"] == 0
+
+
+def test_per_problem_hyperparameters_and_sum_property():
+    wl = _mixed_workload("f64", seed=6)
+    ref = PU.oracle_reference(wl)
+    cots = PU.full_cotangent(wl, ref)
+    a = PU.gpu_run(wl, cots, per_problem=True)
+    b = PU.gpu_run(wl, cots, per_problem=False)
+    PU.assert_within(PU.compare(wl, ref, a, True), "f64")
+    PU.assert_within(PU.compare(wl, ref, b, False), "f64")
+    np.testing.assert_allclose(a["g_rho"].sum(1), b["g_rho"], rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(a["g_alpha"].sum(1), b["g_alpha"], rtol=1e-12, atol=1e-14)
+
+
+def test_host_io_matches_device_io_bitwise():
+    wl = _mixed_workload("f32", seed=7)
+    ref = PU.oracle_reference(wl)
+    cots = PU.full_cotangent(wl, ref)
+    a = PU.gpu_run(wl, cots, host=False)
+    b = PU.gpu_run(wl, cots, host=True)
+    for k in ("xK", "sK", "yK", "g_x0", "g_s0", "g_y0"):
+        for u, v in zip(a[k], b[k]):
+            assert np.array_equal(u, v)
+    assert np.array_equal(a["g_rho"], b["g_rho"]) and a["g_sigma"] == b["g_sigma"]
+
+
+def test_runs_are_deterministic():
+    wl = W.make_config(2, batch=5, p=14, K=10)
+    ref = PU.oracle_reference(wl, problems=[0])
+    cots = PU.full_cotangent(wl, ref)
+    a, b = PU.gpu_run(wl, cots), PU.gpu_run(wl, cots)
+    assert np.array_equal(a["g_rho"], b["g_rho"]) and all(np.array_equal(u, v) for u, v in zip(a["xK"], b["xK"]))
+
+
+# ---- degenerate and edge cases ------------------------------------------------------------------------------
+def test_edge_cases_psd1_soc1_odd_order_single_step():
+    cones = ((PSD, 1), (SOC, 1), (PSD, 7), (NONNEG, 1), (SOC, 2))
+    for dtype in ("f64", "f32"):
+        wl = _mixed_workload(dtype, seed=8, B=2, K=1, cones=cones, n=6)
+        e, _ = PU.check(wl)
+        PU.assert_within(e, dtype)
+
+
+def test_zero_cotangent_gives_zero_gradients_and_no_nan():
+    wl = _mixed_workload("f32", seed=10)
+    res = PU.gpu_run(wl, None)
+    for k in ("g_x0", "g_s0", "g_y0"):
+        assert all(np.all(v == 0.0) for v in res[k])
+    assert np.all(res["g_rho"] == 0.0) and np.all(res["g_alpha"] == 0.0) and res["g_sigma"] == 0.0
+
+
+def test_repeated_eigenvalues_in_the_unroll_stay_finite():
+    """Isotropic target: the projected matrix has an exactly degenerate spectrum."""
+    import scipy.sparse as sp
+    from oracle import cones as C
+    p = 6
+    n = W.svec_dim(p)
+    pr = Problem(P=sp.identity(n, format="csr"), q=-C.svec(2.0 * np.eye(p)), A=-sp.identity(n, format="csr"), b=np.zeros(n), cones=[(PSD, p)])
+    for dtype in ("f64", "f32"):
+        wl = Workload("iso", dtype, [_round_problem(pr, dtype)] * 2, 6, np.ones(6), np.full(6, PU.round_to(1.6, dtype)), 1e-6,
+                      [np.zeros(n)] * 2, [np.zeros(n)] * 2, [np.zeros(n)] * 2)
+        e, st = PU.check(wl)
+        PU.assert_within(e, dtype)
+
+
+def test_error_codes():
+    import torch
+    import paper_2606_13825_b200 as cdu
+    wl = W.make_config(1)
+    pk = W.pack_batch(wl.problems, wl.dtype)
+    h = cdu.cdu_create(pk, K_max=4)
+    rho = torch.ones(8, dtype=torch.float64, device="cuda")
+    with pytest.raises(cdu.CduError) as ei:
+        h.backward()
+    assert ei.value.status == cdu.CDU_ESTATE
+    with pytest.raises(cdu.CduError) as ei:
+        h.forward(5, rho, rho, 1e-6)
+    assert ei.value.status == cdu.CDU_EINVAL
+    with pytest.raises(cdu.CduError):
+        h.forward(2, rho, rho, -1.0)
+    with pytest.raises(cdu.CduError):      # host-side validation: alpha outside (0, 2)
+        h.forward(2, np.ones(2), np.full(2, 2.5), 1e-6, host=True)
+    h.close()
+    bad = dict(pk); bad["cones"] = pk["cones"].copy(); bad["cones"][0, 1] += 1     # cones no longer tile the rows
+    with pytest.raises(cdu.CduError) as ei:
+        cdu.cdu_create(bad, K_max=4)
+    assert ei.value.status == cdu.CDU_EINVAL
+    with pytest.raises(cdu.CduError):
+        cdu.cdu_create(pk, K_max=0)
+
+
+# ---- down-scaled configs: several tiles, ragged tails ------------------------------------------------------------
+@pytest.mark.parametrize("cfg,kw", [
+    (2, dict(batch=4, p=21, K=20)),
+    (3, dict(batch=4, p=40, K=30)),
+    (4, dict(batch=3, p=16, K=30)),
+    (4, dict(batch=2, p=33, K=25)),
+])
+def test_downscaled_configs(cfg, kw):
+    wl = W.make_config(cfg, **kw)
+    e, st = PU.check(wl)
+    PU.assert_within(e, wl.dtype)
+    assert st["flags_or"] == 0
+
+
+@pytest.mark.parametrize("ckpt", [0, 1])
+def test_large_block_path_downscaled(ckpt):
+    wl = W.make_config(5, batch=2, p=24, K=10)
+    e, st = PU.check(wl, ckpt_mode=ckpt, psd_small_max=8)       # force the global-memory path
+    PU.assert_within(e, wl.dtype)
+    wl = W.make_config(5, batch=2, p=140, K=6)
+    e, st = PU.check(wl, ckpt_mode=ckpt)
+    PU.assert_within(e, wl.dtype)
+
+
+# ---- full sizes, in the launch configuration bench.py times; sampled problems against the oracle --------------
+FULL = {2: [0, 101, 255], 3: [0, 1, 511, 1023], 4: [0, 63], 5: [3]}
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4])
+def test_full_size_configs_sampled(cfg):
+    wl = W.make_config(cfg)
+    e, st = PU.check(wl, problems=FULL[cfg], per_problem=True)
+    print(wl.name, e, st)
+    PU.assert_within(e, wl.dtype)
+    assert st["flags_or"] == 0
+
+
+def test_full_size_cfg5_sampled():
+    wl = W.make_config(5)
+    e, st = PU.check(wl, problems=FULL[5], per_problem=True)
+    print(wl.name, e, st)
+    PU.assert_within(e, wl.dtype)
+
+
+def test_full_size_shared_theta_equals_sum_of_per_problem():
+    wl = W.make_config(2)
+    rng = np.random.default_rng(3)
+    cots = [(rng.standard_normal(pr.n), rng.standard_normal(pr.m), rng.standard_normal(pr.m)) for pr in wl.problems]
+    a = PU.gpu_run(wl, cots, per_problem=True)
+    b = PU.gpu_run(wl, cots, per_problem=False)
+    assert PU.nrm_err(b["g_rho"], a["g_rho"].sum(1)) < 1e-5 and PU.nrm_err(b["g_alpha"], a["g_alpha"].sum(1)) < 1e-5

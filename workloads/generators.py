@@ -263,9 +263,10 @@ def lovasz_dual_feasible_start(pr: Problem):
 
 
 def make_config(cfg: int, batch: Optional[int] = None, K: Optional[int] = None,
-                p: Optional[int] = None) -> Workload:
+                p: Optional[int] = None, seed_offset: int = 0) -> Workload:
     """BASELINE.json configs[cfg-1] with the recipes of SURVEY.md 8(d). `batch`, `K`, `p` (graph order /
-    number of variables for cfg3) override the full sizes for down-scaled parity cases."""
+    number of variables for cfg3) override the full sizes for down-scaled parity cases; `seed_offset` shifts the
+    instance seeds (hyper-parameters stay shared) so that every rank of a weak-scaling run draws its own batch."""
     full = {1: (4, 20, 10), 2: (256, 50, 50), 3: (1024, 100, 200), 4: (64, 100, 100), 5: (8, 200, 512)}[cfg]
     B = batch if batch is not None else full[0]
     Kk = K if K is not None else full[1]
@@ -274,7 +275,7 @@ def make_config(cfg: int, batch: Optional[int] = None, K: Optional[int] = None,
     hrng = np.random.default_rng(BASE_SEED + 1000 * cfg + 999)
     problems = []
     for b in range(B):
-        rng = np.random.default_rng(BASE_SEED + 1000 * cfg + b)
+        rng = np.random.default_rng(BASE_SEED + 1000 * cfg + b + seed_offset)
         if cfg == 1:
             pr = maxcut_problem(erdos_renyi(rng, pp, 0.5, "unit"))
         elif cfg == 2:
