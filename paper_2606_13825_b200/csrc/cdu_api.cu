@@ -768,21 +768,16 @@ cdu_status psd_op_t(bool vjp, int count, int p, const void* in1, const void* in2
   T* d_one = pool.upload(one, st);
   if (pool.last != cudaSuccess || !W || !S1 || !Y1 || !GW || !part || !Gs || !Us || !Ls || !flags || !d_one) { err = "cudaMalloc (psd op)"; return CDU_ENOMEM; }
   Hyper<T> H; H.rho = d_one; H.alpha = d_one; H.kstride = 0; H.pstride = 0; H.sigma = 1.0;
-  const bool large = eng.n_large > 0;
   if (!vjp) {
     k_dense_to_svec<T><<<count, 256, 0, st>>>(p, (const T*)in1, W);
     PsdFwdArgs A; A.W = W; A.S1 = S1; A.Y1 = Y1; A.Ustore = Us; A.Lstore = Ls; A.sweeps_max = eng.sweeps_max; A.flags = flags; A.sweeps_sum = eng.sweeps_sum;
     s = eng.forward(H, 0, A, st);
     if (s != CDU_OK) { err = eng.err; return s; }
     k_svec_to_dense<T><<<count, 256, 0, st>>>(p, S1, (T*)out1);
-    if (out2) {
-      if (large) k_transpose_batched<T><<<count, 256, 0, st>>>(p, Us, (T*)out2);
-      else CU_OK(cudaMemcpyAsync(out2, Us, (size_t)count * p * p * sizeof(T), cudaMemcpyDeviceToDevice, st));
-    }
+    if (out2) k_transpose_batched<T><<<count, 256, 0, st>>>(p, Us, (T*)out2);   // both paths store eigenvectors as rows
     if (out3) CU_OK(cudaMemcpyAsync(out3, Ls, (size_t)count * p * sizeof(T), cudaMemcpyDeviceToDevice, st));
   } else {
-    if (large) k_transpose_batched<T><<<count, 256, 0, st>>>(p, (const T*)in1, Us);
-    else CU_OK(cudaMemcpyAsync(Us, in1, (size_t)count * p * p * sizeof(T), cudaMemcpyDeviceToDevice, st));
+    k_transpose_batched<T><<<count, 256, 0, st>>>(p, (const T*)in1, Us);
     CU_OK(cudaMemcpyAsync(Ls, in2, (size_t)count * p * sizeof(T), cudaMemcpyDeviceToDevice, st));
     k_dense_to_svec<T><<<count, 256, 0, st>>>(p, (const T*)in3, Gs);
     PsdBwdArgs A; A.W = W; A.Yk = Y1; A.S1 = S1; A.Gs = Gs; A.Gy = W /* zeros */; A.GW = GW; A.part = part;
