@@ -129,7 +129,7 @@ struct PsdEngine {
   int* rotflags = nullptr;
   int* sweeps_max = nullptr;
   unsigned long long* sweeps_sum = nullptr;
-  int small_threads = 256;
+  PsdSmallCfg scfg{1, 96};
   int use_tc = 0;
   long long launches = 0;
   Prof* prof = nullptr;
@@ -160,7 +160,6 @@ struct PsdEngine {
     d_small_list = pool.upload(small_list, st);
     sweeps_max = pool.zeros<int>(1, st);
     sweeps_sum = pool.zeros<unsigned long long>(1, st);
-    small_threads = pmax_small <= 64 ? 256 : 512;
     if (n_large) {
       lt.nblk = n_large; lt.pmax = pmax_large;
       lt.gblk = pool.upload(gblk, st); lt.moff = pool.upload(moff, st); lt.voff = pool.upload(voff, st); lt.pvec = pool.upload(lp, st);
@@ -174,12 +173,29 @@ struct PsdEngine {
     }
     if (pool.last != cudaSuccess) { err = std::string("PSD tables: ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
     if (n_small) {
-      const size_t sf = psd_small_smem_fwd(pmax_small, sizeof(T)), sb = psd_small_smem_bwd(pmax_small, sizeof(T));
-      if (sb > 227 * 1024) { err = "psd_small_max too large for shared memory"; return CDU_EINVAL; }
-      CU_OK(cudaFuncSetAttribute(k_psd_fwd_small<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sf));
-      CU_OK(cudaFuncSetAttribute(k_psd_bwd_small<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb));
+      const size_t sb = psd_small_smem_bytes(pmax_small, sizeof(T));
+      scfg = psd_small_cfg(pmax_small, sizeof(T));
+      if (sb > 227 * 1024 || scfg.maxi > PSD_SMALL_MAXI) { err = "psd_small_max too large for shared memory"; return CDU_EINVAL; }
+      const void* fn[8] = {(const void*)k_psd_fwd_small<T, 1>, (const void*)k_psd_fwd_small<T, 2>, (const void*)k_psd_fwd_small<T, 3>,
+                           (const void*)k_psd_fwd_small<T, 4>, (const void*)k_psd_bwd_small<T, 1>, (const void*)k_psd_bwd_small<T, 2>,
+                           (const void*)k_psd_bwd_small<T, 3>, (const void*)k_psd_bwd_small<T, 4>};
+      for (const void* f : fn) CU_OK(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb));
     }
     return CDU_OK;
+  }
+  void launch_small_fwd(const Hyper<T>& H, int k, const PsdFwdArgs& A, cudaStream_t st) {
+    const size_t sm = psd_small_smem_bytes(pmax_small, sizeof(T));
+    if (scfg.maxi == 1) k_psd_fwd_small<T, 1><<<n_small, scfg.threads, sm, st>>>(tab, H, k, A, d_small_list);
+    else if (scfg.maxi == 2) k_psd_fwd_small<T, 2><<<n_small, scfg.threads, sm, st>>>(tab, H, k, A, d_small_list);
+    else if (scfg.maxi == 3) k_psd_fwd_small<T, 3><<<n_small, scfg.threads, sm, st>>>(tab, H, k, A, d_small_list);
+    else k_psd_fwd_small<T, 4><<<n_small, scfg.threads, sm, st>>>(tab, H, k, A, d_small_list);
+  }
+  void launch_small_bwd(const Hyper<T>& H, int k, const PsdBwdArgs& A, cudaStream_t st) {
+    const size_t sm = psd_small_smem_bytes(pmax_small, sizeof(T));
+    if (scfg.maxi == 1) k_psd_bwd_small<T, 1><<<n_small, scfg.threads, sm, st>>>(tab, H, k, A, d_small_list);
+    else if (scfg.maxi == 2) k_psd_bwd_small<T, 2><<<n_small, scfg.threads, sm, st>>>(tab, H, k, A, d_small_list);
+    else if (scfg.maxi == 3) k_psd_bwd_small<T, 3><<<n_small, scfg.threads, sm, st>>>(tab, H, k, A, d_small_list);
+    else k_psd_bwd_small<T, 4><<<n_small, scfg.threads, sm, st>>>(tab, H, k, A, d_small_list);
   }
 
   cdu_status gemm(const T* A, int ta, const T* Bm, int tb, T* C, const T* kscale, int relu, cudaStream_t st) {
@@ -230,7 +246,7 @@ struct PsdEngine {
   cdu_status forward(const Hyper<T>& H, int k, const PsdFwdArgs& A, cudaStream_t st) {
     if (n_small) {
       pb(PC_PSD_FWD_SMALL, st);
-      k_psd_fwd_small<T><<<n_small, small_threads, psd_small_smem_fwd(pmax_small, sizeof(T)), st>>>(tab, H, k, A, d_small_list);
+      launch_small_fwd(H, k, A, st);
       pe(st);
       ++launches;
       CU_OK(cudaGetLastError());
@@ -257,7 +273,7 @@ struct PsdEngine {
   cdu_status backward(const Hyper<T>& H, int k, const PsdBwdArgs& A, cudaStream_t st) {
     if (n_small) {
       pb(PC_PSD_BWD_SMALL, st);
-      k_psd_bwd_small<T><<<n_small, small_threads, psd_small_smem_bwd(pmax_small, sizeof(T)), st>>>(tab, H, k, A, d_small_list);
+      launch_small_bwd(H, k, A, st);
       pe(st);
       ++launches;
       CU_OK(cudaGetLastError());

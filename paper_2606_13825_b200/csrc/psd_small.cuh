@@ -49,41 +49,60 @@ template <typename T> __device__ __forceinline__ T gamma_relu(T li, T lj) {
 //     plane 0: (top,top)  1: (top,bottom)  2: (bottom,top)  3: (bottom,bottom),   each h x ldh, ldh odd,
 // double-buffered: block (q1,q2) is read from the current buffer with unit-stride, conflict-free loads, rotated
 // (rows by pair q1, columns by pair q2) and its four entries are scattered to their next-round seats in the
-// other buffer; only q1 <= q2 is computed, the mirror image is written too. Eigenvectors are kept transposed
-// (Vt[player][coordinate], "player" = initial position), updated in place with lanes along the coordinate, and
-// found through the small position->player table plr. No index arithmetic of the pairing is left in the loop.
+// other buffer; only q1 <= q2 is computed, the mirror image is written too. Because seats never change, every
+// thread owns the same <= MAXI blocks and eigenvector slices in every round and keeps their source and
+// destination offsets in registers: no index arithmetic of the pairing is left in the loop.
+// Eigenvectors are kept transposed (Vt[player][coordinate], "player" = initial position), updated in place
+// with 16-byte accesses along the coordinate, and found through the small position->player table plr.
+// The last two warps of the CTA are "angle" warps: while the work warps apply round r they evaluate, from the
+// three entries involved, the pivots round r+1 will meet and write that round's rotations, so a round costs
+// one barrier and the rotation set-up is off the critical path of the updates.
 // ---------------------------------------------------------------------------------------------------------
+template <typename T> struct VecT;
+template <> struct VecT<float> { using type = float4; static constexpr int W = 4; };
+template <> struct VecT<double> { using type = double2; static constexpr int W = 2; };
+constexpr int JACOBI_ANGLE_THREADS = 64;
+
 template <typename T> struct JacobiWs {
   T* P0; int pstride;    // 2 x (4 planes x h x ldh); buffer c at P0 + c * pstride
-  T* Vt;                 // pe x pe
-  T* cs;                 // 3 h  (sin, tau = sin/(1+cos), tan)
+  T* Vt; int ldv;        // pe x ldv, ldv = pe rounded up to the 16-byte vector width
+  T* cs0;                // 2 x h x 4  (sin, tau = sin/(1+cos), tan, -); buffer c at cs0 + c * 4 h
   int* plr0; int pe;     // 2 x pe   player at position; buffer c at plr0 + c * pe
-  int4* mv;              // h        next-round seat offsets of pair q: (row-top, row-bottom, col-top, col-bottom)
-  unsigned short* blk;   // h(h+1)/2 (q1 << 8 | q2), q1 <= q2, row after row
 };
+__host__ __device__ inline int jacobi_ldv(int pe, size_t sz) { const int vw = (int)(16 / sz); return (pe + vw - 1) / vw * vw; }
 template <typename T> __host__ __device__ inline size_t jacobi_ws_bytes(int pe) {
-  const size_t h = pe >> 1, ldh = h | 1;
-  size_t b = (2 * 4 * h * ldh + (size_t)pe * pe + 3 * h) * sizeof(T);
+  const size_t h = pe >> 1, ldh = h | 1, ldv = jacobi_ldv(pe, sizeof(T));
+  size_t b = (((2 * 4 * h * ldh) * sizeof(T)) + 15) & ~(size_t)15;
+  b += (size_t)pe * ldv * sizeof(T) + 2 * h * 4 * sizeof(T);
   b = (b + 15) & ~(size_t)15;
-  b += h * sizeof(int4) + 2 * (size_t)pe * sizeof(int) + ((h * (h + 1) / 2 + 1) & ~(size_t)1) * sizeof(unsigned short);
+  b += 2 * (size_t)pe * sizeof(int);
   return (b + 15) & ~(size_t)15;
 }
 template <typename T> __device__ __forceinline__ JacobiWs<T> jacobi_ws_carve(unsigned char* base, int pe) {
-  const size_t h = pe >> 1, ldh = h | 1;
+  const size_t h = pe >> 1, ldh = h | 1, ldv = jacobi_ldv(pe, sizeof(T));
   JacobiWs<T> w;
-  T* t = reinterpret_cast<T*>(base);
-  w.P0 = t; w.pstride = (int)(4 * h * ldh); w.Vt = t + 8 * h * ldh; w.cs = w.Vt + (size_t)pe * pe;
-  size_t off = ((2 * 4 * h * ldh + (size_t)pe * pe + 3 * h) * sizeof(T) + 15) & ~(size_t)15;
-  w.mv = reinterpret_cast<int4*>(base + off); off += h * sizeof(int4);
-  w.plr0 = reinterpret_cast<int*>(base + off); w.pe = pe; off += 2 * (size_t)pe * sizeof(int);
-  w.blk = reinterpret_cast<unsigned short*>(base + off);
+  w.P0 = reinterpret_cast<T*>(base); w.pstride = (int)(4 * h * ldh);
+  size_t off = (((2 * 4 * h * ldh) * sizeof(T)) + 15) & ~(size_t)15;
+  w.Vt = reinterpret_cast<T*>(base + off); w.ldv = (int)ldv; off += (size_t)pe * ldv * sizeof(T);
+  w.cs0 = reinterpret_cast<T*>(base + off); off += 2 * h * 4 * sizeof(T);
+  off = (off + 15) & ~(size_t)15;
+  w.plr0 = reinterpret_cast<int*>(base + off); w.pe = pe;
   return w;
 }
 
-__device__ __forceinline__ int seat_after(int pos, int h) {   // position after one round of the circle
+__host__ __device__ inline int seat_after(int pos, int h) {   // position after one round of the circle
   const int q = pos >> 1;
   if (!(pos & 1)) return q == 0 ? 0 : (q < h - 1 ? pos + 2 : 2 * (h - 1) + 1);
   return q == 0 ? (h > 1 ? 2 : 1) : pos - 2;
+}
+__device__ __forceinline__ int seat_before(int pos, int h) {  // inverse of seat_after
+  const int q = pos >> 1;
+  if (h == 1) return pos;
+  if (!(pos & 1)) return q == 0 ? 0 : (q == 1 ? 1 : pos - 2);          // top 1 <- bottom 0, top q <- top q-1
+  return q == h - 1 ? 2 * (h - 1) : pos + 2;                            // bottom h-1 <- top h-1, bottom q <- bottom q+1
+}
+__device__ __forceinline__ int seat_offset(int rowpos, int colpos, int psz, int ldh) {   // plane offset of entry (rowpos, colpos)
+  return ((rowpos & 1) * 2 + (colpos & 1)) * psz + (rowpos >> 1) * ldh + (colpos >> 1);
 }
 
 template <typename T> __device__ __forceinline__ void jacobi_angle(T aii, T ajj, T aij, T skip, T& sn, T& tau, T& tt) {
@@ -96,6 +115,16 @@ template <typename T> __device__ __forceinline__ void jacobi_angle(T aii, T ajj,
     const T c = (T)1 / sqrt((T)1 + t * t);
     sn = t * c; tau = sn / ((T)1 + c); tt = t;
   }
+}
+template <typename T> __device__ __forceinline__ void rot2(T s, T tau, T& x, T& y) {
+  const T nx = x - s * (y + tau * x), ny = y + s * (x - tau * y);
+  x = nx; y = ny;
+}
+__device__ __forceinline__ void rot_vec(float s, float tau, float4& x, float4& y) {
+  rot2(s, tau, x.x, y.x); rot2(s, tau, x.y, y.y); rot2(s, tau, x.z, y.z); rot2(s, tau, x.w, y.w);
+}
+__device__ __forceinline__ void rot_vec(double s, double tau, double2& x, double2& y) {
+  rot2(s, tau, x.x, y.x); rot2(s, tau, x.y, y.y);
 }
 
 // smat(v [+ sc v2]) -> planes of buffer 0, zero padded to pe. v, v2: svec (fp64).
@@ -111,45 +140,81 @@ __device__ __forceinline__ void load_smat_planes(int p, int pe, T* P0, const dou
       if (v2) x += sc * v2[idx];
       val = (T)(a == b ? x : x * 0.70710678118654752440);
     }
-    P0[((a & 1) * 2 + (b & 1)) * psz + (a >> 1) * ldh + (b >> 1)] = val;
+    P0[seat_offset(a, b, psz, ldh)] = val;
   }
 }
 
+// Work threads needed so that every thread owns at most `maxi` blocks / eigenvector slices (host side).
+inline int jacobi_need(int pe, size_t sz) {
+  const int h = pe >> 1, nblk = h * (h + 1) / 2, nvit = h * (jacobi_ldv(pe, sz) / (int)(16 / sz));
+  return nblk > nvit ? nblk : nvit;
+}
+
 // On entry buffer 0 holds the matrix. On exit: *cur_out = buffer holding the (numerically diagonal) matrix,
-// plr[*cur_out][pos] = player whose eigenvalue sits on the diagonal at pos, Vt[player][:] = its eigenvector.
-template <typename T>
+// plr0[*cur_out * pe + pos] = player whose eigenvalue sits on the diagonal at pos, Vt[player][:] = its eigenvector.
+// blockDim.x = work threads + JACOBI_ANGLE_THREADS; every thread of the CTA must call.
+template <typename T, int MAXI>
 __device__ int jacobi_planes(int pe, const JacobiWs<T>& w, double* shred, int max_sweeps, int* flag, int* cur_out) {
-  const int tid = threadIdx.x, nt = blockDim.x;
-  const int h = pe >> 1, ldh = h | 1, psz = h * ldh, nblk = h * (h + 1) / 2;
-  // ---- one-time tables ----
-  for (int t = tid; t < pe * pe; t += nt) { const int i = t / pe, a = t - i * pe; w.Vt[t] = (i == a) ? (T)1 : (T)0; }
+  using V4 = typename VecT<T>::type;
+  constexpr int VW = VecT<T>::W;
+  const int tid = threadIdx.x, nt = blockDim.x, ntw = nt - JACOBI_ANGLE_THREADS;
+  const int h = pe >> 1, ldh = h | 1, psz = h * ldh, ldv = w.ldv, nblk = h * (h + 1) / 2, nvc = ldv / VW, nvit = h * nvc;
+  // ---- one-time set-up ----
+  for (int t = tid; t < pe * ldv; t += nt) { const int i = t / ldv, a = t - i * ldv; w.Vt[t] = (i == a) ? (T)1 : (T)0; }
   for (int pos = tid; pos < pe; pos += nt) w.plr0[pos] = pos;
-  for (int q = tid; q < h; q += nt) {
-    const int nt_ = seat_after(2 * q, h), nb_ = seat_after(2 * q + 1, h);
-    int4 m;
-    m.x = 2 * (nt_ & 1) * psz + (nt_ >> 1) * ldh;   // as a row
-    m.y = 2 * (nb_ & 1) * psz + (nb_ >> 1) * ldh;
-    m.z = (nt_ & 1) * psz + (nt_ >> 1);             // as a column
-    m.w = (nb_ & 1) * psz + (nb_ >> 1);
-    w.mv[q] = m;
-  }
-  for (int q1 = tid; q1 < h; q1 += nt) {
-    int o = q1 * h - q1 * (q1 - 1) / 2;
-    for (int q2 = q1; q2 < h; ++q2) w.blk[o++] = (unsigned short)((q1 << 8) | q2);
-  }
   double acc[1] = {0.0};
   for (int t = tid; t < 4 * psz; t += nt) {
     const int r = t % ldh;
     if (r < h) { const double x = (double)w.P0[t]; acc[0] += x * x; }
   }
-  block_sum<1>(acc, shred);   // also publishes the tables
+  block_sum<1>(acc, shred);
   const double normF2 = acc[0];
   *cur_out = 0;
   if (!(normF2 > 0.0)) { if (normF2 != normF2) *flag |= FLAG_NONFINITE; return 0; }
   const double tol2 = 16.0 * (double)Eps<T>::v() * (double)Eps<T>::v() * normF2;
   const T skip = (T)(0.01 * sqrt(tol2) / pe);
-  // V-update items (pair q, coordinate a), t = q pe + a, stepped incrementally
-  const int vq0 = tid / pe, va0 = tid - vq0 * pe, dq = nt / pe, da = nt - dq * pe;
+
+  // per-thread constants (registers): blocks, eigenvector slices, or the pivot an angle thread prepares
+  int bsrc[MAXI], bq[MAXI], bdst[MAXI][8];
+  int vq[MAXI], va[MAXI];
+#pragma unroll
+  for (int i = 0; i < MAXI; ++i) { bq[i] = -1; vq[i] = -1; bsrc[i] = 0; va[i] = 0; }
+  int qu = 0, qv = 0, su = 0, sv = 0;
+  const bool worker = tid < ntw;
+  if (worker) {
+#pragma unroll
+    for (int i = 0; i < MAXI; ++i) {
+      const int t = tid + i * ntw;
+      if (t < nblk) {
+        int q1, q2;
+        if (t < h) { q1 = q2 = t; }
+        else {   // off-diagonal blocks, row after row: row q1 holds q2 = q1+1 .. h-1
+          int e = t - h; q1 = 0;
+          while (e >= h - 1 - q1) { e -= h - 1 - q1; ++q1; }
+          q2 = q1 + 1 + e;
+        }
+        const int r_t = seat_after(2 * q1, h), r_b = seat_after(2 * q1 + 1, h), c_t = seat_after(2 * q2, h), c_b = seat_after(2 * q2 + 1, h);
+        bq[i] = (q1 << 8) | q2; bsrc[i] = q1 * ldh + q2;
+        bdst[i][0] = seat_offset(r_t, c_t, psz, ldh); bdst[i][1] = seat_offset(r_t, c_b, psz, ldh);
+        bdst[i][2] = seat_offset(r_b, c_t, psz, ldh); bdst[i][3] = seat_offset(r_b, c_b, psz, ldh);
+        bdst[i][4] = seat_offset(c_t, r_t, psz, ldh); bdst[i][5] = seat_offset(c_b, r_t, psz, ldh);   // mirror block
+        bdst[i][6] = seat_offset(c_t, r_b, psz, ldh); bdst[i][7] = seat_offset(c_b, r_b, psz, ldh);
+      }
+      if (t < nvit) { vq[i] = t / nvc; va[i] = (t - vq[i] * nvc) * VW; }
+    }
+  } else {
+    const int j = tid - ntw;
+    if (j < h) { const int u = seat_before(2 * j, h), v = seat_before(2 * j + 1, h); qu = u >> 1; su = u & 1; qv = v >> 1; sv = v & 1; }
+  }
+  // rotations of the first round, straight from the diagonal blocks
+  for (int q = tid; q < h; q += nt) {
+    const int o = q * ldh + q;
+    T sn, tau, tt;
+    jacobi_angle<T>(w.P0[o], w.P0[3 * psz + o], w.P0[psz + o], skip, sn, tau, tt);
+    w.cs0[4 * q] = sn; w.cs0[4 * q + 1] = tau; w.cs0[4 * q + 2] = tt; w.cs0[4 * q + 3] = (T)0;
+  }
+  __syncthreads();
+
   int cur = 0, sweep = 0;
   for (; sweep < max_sweeps; ++sweep) {
     {   // off-diagonal mass
@@ -165,50 +230,69 @@ __device__ int jacobi_planes(int pe, const JacobiWs<T>& w, double* shred, int ma
       if (!(acc[0] > tol2)) break;
     }
     for (int r = 0; r < pe - 1; ++r) {
-      const T* Pc = w.P0 + cur * w.pstride;
-      T* Pn = w.P0 + (cur ^ 1) * w.pstride;
-      const int* plc = w.plr0 + cur * pe;
-      int* pln = w.plr0 + (cur ^ 1) * pe;
-      for (int q = tid; q < h; q += nt) {
-        const int o = q * ldh + q;
-        T sn, tau, tt;
-        jacobi_angle<T>(Pc[o], Pc[3 * psz + o], Pc[psz + o], skip, sn, tau, tt);
-        w.cs[3 * q] = sn; w.cs[3 * q + 1] = tau; w.cs[3 * q + 2] = tt;
-      }
-      __syncthreads();
-      for (int t = tid; t < nblk; t += nt) {
-        const int qq = w.blk[t], q1 = qq >> 8, q2 = qq & 255, o = q1 * ldh + q2;
-        const int4 m1 = w.mv[q1], m2 = w.mv[q2];
-        T a = Pc[o], d = Pc[3 * psz + o];
-        if (q1 == q2) {
-          const T g = w.cs[3 * q1 + 2] * Pc[psz + o];   // tan * a_ij
-          a -= g; d += g;
-          Pn[m1.x + m1.z] = a; Pn[m1.y + m1.w] = d; Pn[m1.x + m1.w] = (T)0; Pn[m1.y + m1.z] = (T)0;
-        } else {
-          const T b = Pc[psz + o], c = Pc[2 * psz + o];
-          const T s1 = w.cs[3 * q1], t1 = w.cs[3 * q1 + 1], s2 = w.cs[3 * q2], t2 = w.cs[3 * q2 + 1];
-          const T ra = a - s1 * (c + t1 * a), rc = c + s1 * (a - t1 * c);   // rows:  J1' S
-          const T rb = b - s1 * (d + t1 * b), rd = d + s1 * (b - t1 * d);
-          const T na = ra - s2 * (rb + t2 * ra), nb = rb + s2 * (ra - t2 * rb);   // cols: (.) J2
-          const T nc = rc - s2 * (rd + t2 * rc), nd = rd + s2 * (rc - t2 * rd);
-          Pn[m1.x + m2.z] = na; Pn[m1.x + m2.w] = nb; Pn[m1.y + m2.z] = nc; Pn[m1.y + m2.w] = nd;
-          Pn[m2.x + m1.z] = na; Pn[m2.y + m1.z] = nb; Pn[m2.x + m1.w] = nc; Pn[m2.y + m1.w] = nd;   // mirror block
+      const T* __restrict__ Pc = w.P0 + cur * w.pstride;
+      T* __restrict__ Pn = w.P0 + (cur ^ 1) * w.pstride;
+      const T* __restrict__ csc = w.cs0 + cur * 4 * h;
+      const int* __restrict__ plc = w.plr0 + cur * pe;
+      if (worker) {
+        // ---- eigenvector slices: load everything, then rotate and store (in place, slices are disjoint) ----
+        V4 x[MAXI], y[MAXI]; T vs[MAXI], vt[MAXI]; V4 *pi[MAXI], *pj[MAXI];
+#pragma unroll
+        for (int i = 0; i < MAXI; ++i)
+          if (vq[i] >= 0) {
+            vs[i] = csc[4 * vq[i]]; vt[i] = csc[4 * vq[i] + 1];
+            const int2 pl = *reinterpret_cast<const int2*>(plc + 2 * vq[i]);
+            pi[i] = reinterpret_cast<V4*>(w.Vt + pl.x * ldv + va[i]); pj[i] = reinterpret_cast<V4*>(w.Vt + pl.y * ldv + va[i]);
+            x[i] = *pi[i]; y[i] = *pj[i];
+          }
+        // ---- 2 x 2 blocks ----
+#pragma unroll
+        for (int i = 0; i < MAXI; ++i)
+          if (bq[i] >= 0) {
+            const int o = bsrc[i], q1 = bq[i] >> 8, q2 = bq[i] & 255;
+            const T a = Pc[o], b = Pc[psz + o], d = Pc[3 * psz + o];
+            if (q1 == q2) {
+              const T g = csc[4 * q1 + 2] * b;   // tan * a_ij
+              Pn[bdst[i][0]] = a - g; Pn[bdst[i][3]] = d + g; Pn[bdst[i][1]] = (T)0; Pn[bdst[i][2]] = (T)0;
+            } else {
+              const T c = Pc[2 * psz + o];
+              const T s1 = csc[4 * q1], t1 = csc[4 * q1 + 1], s2 = csc[4 * q2], t2 = csc[4 * q2 + 1];
+              const T ra = a - s1 * (c + t1 * a), rc = c + s1 * (a - t1 * c);   // rows:  J1' S
+              const T rb = b - s1 * (d + t1 * b), rd = d + s1 * (b - t1 * d);
+              const T na = ra - s2 * (rb + t2 * ra), nb = rb + s2 * (ra - t2 * rb);   // cols: (.) J2
+              const T nc = rc - s2 * (rd + t2 * rc), nd = rd + s2 * (rc - t2 * rd);
+              Pn[bdst[i][0]] = na; Pn[bdst[i][1]] = nb; Pn[bdst[i][2]] = nc; Pn[bdst[i][3]] = nd;
+              Pn[bdst[i][4]] = na; Pn[bdst[i][5]] = nb; Pn[bdst[i][6]] = nc; Pn[bdst[i][7]] = nd;
+            }
+          }
+#pragma unroll
+        for (int i = 0; i < MAXI; ++i)
+          if (vq[i] >= 0 && vs[i] != (T)0) { rot_vec(vs[i], vt[i], x[i], y[i]); *pi[i] = x[i]; *pj[i] = y[i]; }
+        for (int pos = tid; pos < pe; pos += ntw) w.plr0[(cur ^ 1) * pe + seat_after(pos, h)] = plc[pos];
+      } else {
+        // ---- angle threads: pivot of next round's pair j = entries (u,u), (v,v), (u,v) AFTER this round's rotations ----
+        const int j = tid - ntw;
+        if (j < h) {
+          const int ou = qu * ldh + qu, ov = qv * ldh + qv;
+          const T su_ = csc[4 * qu], tu_ = csc[4 * qu + 1], gu_ = csc[4 * qu + 2];
+          const T sv_ = csc[4 * qv], tv_ = csc[4 * qv + 1], gv_ = csc[4 * qv + 2];
+          const T suu = su ? Pc[3 * psz + ou] + gu_ * Pc[psz + ou] : Pc[ou] - gu_ * Pc[psz + ou];
+          const T svv = sv ? Pc[3 * psz + ov] + gv_ * Pc[psz + ov] : Pc[ov] - gv_ * Pc[psz + ov];
+          T suv = (T)0;
+          if (qu != qv) {
+            const int o = qu * ldh + qv;
+            const T a = Pc[o], b = Pc[psz + o], c = Pc[2 * psz + o], d = Pc[3 * psz + o];
+            const T ra = a - su_ * (c + tu_ * a), rc = c + su_ * (a - tu_ * c);
+            const T rb = b - su_ * (d + tu_ * b), rd = d + su_ * (b - tu_ * d);
+            const T x0 = su ? rc : ra, x1 = su ? rd : rb;                            // row su of J1' S
+            suv = sv ? x1 + sv_ * (x0 - tv_ * x1) : x0 - sv_ * (x1 + tv_ * x0);
+          }
+          T sn, tau, tt;
+          jacobi_angle<T>(suu, svv, suv, skip, sn, tau, tt);
+          T* csn = w.cs0 + (cur ^ 1) * 4 * h + 4 * j;
+          csn[0] = sn; csn[1] = tau; csn[2] = tt;
         }
       }
-      for (int q = vq0, a = va0; q < h; ) {
-        const T s = w.cs[3 * q];
-        if (s != (T)0) {
-          const T tau = w.cs[3 * q + 1];
-          T* vi = w.Vt + plc[2 * q] * pe + a;
-          T* vj = w.Vt + plc[2 * q + 1] * pe + a;
-          const T x = *vi, y = *vj;
-          *vi = x - s * (y + tau * x);
-          *vj = y + s * (x - tau * y);
-        }
-        q += dq; a += da;
-        if (a >= pe) { a -= pe; ++q; }
-      }
-      for (int pos = tid; pos < pe; pos += nt) pln[seat_after(pos, h)] = plc[pos];
       __syncthreads();
       cur ^= 1;
     }
@@ -255,6 +339,9 @@ __device__ __forceinline__ void load_smat(int p, int pe, int ld, T* S, const dou
   }
 }
 
+// CTA size cap per MAXI (more register-resident items per thread -> fewer threads, more registers each)
+__host__ __device__ constexpr int psd_small_max_threads(int maxi) { return maxi <= 1 ? 1024 : (maxi == 2 ? 768 : (maxi == 3 ? 640 : 608)); }
+
 struct PsdFwdArgs {
   const double* W;   // projection argument, all rows
   double* S1;        // s^{k+1} base (rows)
@@ -265,8 +352,8 @@ struct PsdFwdArgs {
   unsigned long long* sweeps_sum;   // total Jacobi sweeps over blocks (statistics for the ALU roofline)
 };
 
-template <typename T>
-__global__ void __launch_bounds__(512) k_psd_fwd_small(PsdTab tab, Hyper<T> H, int k, PsdFwdArgs A, const int* list) {
+template <typename T, int MAXI>
+__global__ void __launch_bounds__(psd_small_max_threads(MAXI)) k_psd_fwd_small(PsdTab tab, Hyper<T> H, int k, PsdFwdArgs A, const int* list) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int blk = list[blockIdx.x];
   const int p = tab.p[blk], pe = (p + 1) & ~1;
@@ -280,7 +367,8 @@ __global__ void __launch_bounds__(512) k_psd_fwd_small(PsdTab tab, Hyper<T> H, i
   load_smat_planes<T>(p, pe, ws.P0, w, 0.0, nullptr);
   __syncthreads();
   int flag = 0, cur = 0;
-  const int sweeps = jacobi_planes<T>(pe, ws, shred, 40, &flag, &cur);
+  const int sweeps = jacobi_planes<T, MAXI>(pe, ws, shred, 40, &flag, &cur);
+  const int ldv = ws.ldv;
   const int h = pe >> 1, ldh = h | 1, psz = h * ldh;
   T* U = reinterpret_cast<T*>(A.Ustore) + tab.uoff[blk];   // rows = eigenvectors
   T* L = reinterpret_cast<T*>(A.Lstore) + tab.loff[blk];
@@ -290,7 +378,7 @@ __global__ void __launch_bounds__(512) k_psd_fwd_small(PsdTab tab, Hyper<T> H, i
     lp[pl] = l > (T)0 ? l : (T)0;
     if (pl < p) L[pl] = l;
   }
-  for (int t = threadIdx.x; t < p * p; t += blockDim.x) { const int i = t / p, a = t - i * p; U[t] = ws.Vt[i * pe + a]; }
+  for (int t = threadIdx.x; t < p * p; t += blockDim.x) { const int i = t / p, a = t - i * p; U[t] = ws.Vt[i * ldv + a]; }
   __syncthreads();
   // rebuild (Eq. 7) + svec + dual update (Eq. 3e); only eigenpairs with lambda > 0 contribute
   const int nsv = p * (p + 1) / 2;
@@ -305,7 +393,7 @@ __global__ void __launch_bounds__(512) k_psd_fwd_small(PsdTab tab, Hyper<T> H, i
     T acc = (T)0;
     for (int i = 0; i < pe; ++i) {
       const T l = lp[i];
-      if (l > (T)0) acc += va[i * pe] * l * vb[i * pe];
+      if (l > (T)0) acc += va[i * ldv] * l * vb[i * ldv];
     }
     const double sp = (a == b) ? (double)acc : (double)acc * 1.41421356237309504880;
     s1[t] = sp;
@@ -331,8 +419,8 @@ struct PsdBwdArgs {
   int* flags;
 };
 
-template <typename T>
-__global__ void __launch_bounds__(512) k_psd_bwd_small(PsdTab tab, Hyper<T> H, int k, PsdBwdArgs A, const int* list) {
+template <typename T, int MAXI>
+__global__ void __launch_bounds__(psd_small_max_threads(MAXI)) k_psd_bwd_small(PsdTab tab, Hyper<T> H, int k, PsdBwdArgs A, const int* list) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int blk = list[blockIdx.x];
   const int p = tab.p[blk], pe = (p + 1) & ~1, ld = pe;
@@ -341,7 +429,8 @@ __global__ void __launch_bounds__(512) k_psd_bwd_small(PsdTab tab, Hyper<T> H, i
   double* shred = reinterpret_cast<double*>(smem_raw);                 // 64 doubles
   const JacobiWs<T> ws = jacobi_ws_carve<T>(smem_raw + 512, pe);
   T* lam = reinterpret_cast<T*>(smem_raw + 512 + jacobi_ws_bytes<T>(pe));
-  T* Vt = ws.Vt;            // Vt[i*pe + a] = V(a, i)
+  T* Vt = ws.Vt;            // Vt[i*ldv + a] = V(a, i)
+  const int ldv = ws.ldv;
   T* G = ws.P0;             // the two p x p work matrices alias the Jacobi planes (dead after a recompute)
   T* Tm = G + pe * pe;
   const double rho = H.rho_at(k, prob);
@@ -351,7 +440,7 @@ __global__ void __launch_bounds__(512) k_psd_bwd_small(PsdTab tab, Hyper<T> H, i
     load_smat_planes<T>(p, pe, ws.P0, w, 0.0, nullptr);
     __syncthreads();
     int cur = 0;
-    jacobi_planes<T>(pe, ws, shred, 40, &flag, &cur);
+    jacobi_planes<T, MAXI>(pe, ws, shred, 40, &flag, &cur);
     const int h = pe >> 1, ldh = h | 1, psz = h * ldh;
     for (int pos = threadIdx.x; pos < pe; pos += blockDim.x)
       lam[ws.plr0[cur * pe + pos]] = ws.P0[cur * ws.pstride + ((pos & 1) ? 3 * psz : 0) + (pos >> 1) * ldh + (pos >> 1)];
@@ -361,7 +450,7 @@ __global__ void __launch_bounds__(512) k_psd_bwd_small(PsdTab tab, Hyper<T> H, i
     const T* L = reinterpret_cast<const T*>(A.Lstore) + tab.loff[blk];
     for (int t = threadIdx.x; t < pe * pe; t += blockDim.x) {
       const int i = t / pe, a = t - i * pe;
-      Vt[t] = (a < p && i < p) ? U[i * p + a] : ((a == i) ? (T)1 : (T)0);
+      Vt[i * ldv + a] = (a < p && i < p) ? U[i * p + a] : ((a == i) ? (T)1 : (T)0);
     }
     for (int i = threadIdx.x; i < pe; i += blockDim.x) lam[i] = i < p ? L[i] : (T)0;
     __syncthreads();
@@ -370,18 +459,18 @@ __global__ void __launch_bounds__(512) k_psd_bwd_small(PsdTab tab, Hyper<T> H, i
   const double* gy = A.Gy + row0;
   load_smat<T>(p, pe, ld, G, gs, rho, gy);                 // G = smat(g_s+ + rho g_y+)
   __syncthreads();
-  smem_gemm<T>(pe, G, ld, 1, Vt, 1, pe, Tm, ld);           // Tm = G V
+  smem_gemm<T>(pe, G, ld, 1, Vt, 1, ldv, Tm, ld);           // Tm = G V
   __syncthreads();
-  smem_gemm<T>(pe, Vt, pe, 1, Tm, ld, 1, G, ld);           // C  = V' Tm
+  smem_gemm<T>(pe, Vt, ldv, 1, Tm, ld, 1, G, ld);           // C  = V' Tm
   __syncthreads();
   for (int t = threadIdx.x; t < pe * pe; t += blockDim.x) {
     const int i = t / pe, j = t - i * pe;
     G[i * ld + j] *= gamma_relu<T>(lam[i], lam[j]);
   }
   __syncthreads();
-  smem_gemm<T>(pe, Vt, 1, pe, G, ld, 1, Tm, ld);           // Tm = V C
+  smem_gemm<T>(pe, Vt, 1, ldv, G, ld, 1, Tm, ld);           // Tm = V C
   __syncthreads();
-  smem_gemm<T>(pe, Tm, ld, 1, Vt, pe, 1, G, ld);           // out = Tm V'
+  smem_gemm<T>(pe, Tm, ld, 1, Vt, ldv, 1, G, ld);           // out = Tm V'
   __syncthreads();
   const int nsv = p * (p + 1) / 2;
   const double* yk = A.Yk + row0;
@@ -413,7 +502,18 @@ static inline size_t psd_small_smem_bytes(int p, size_t sz) {
   const size_t ws = sz == 4 ? jacobi_ws_bytes<float>(pe) : jacobi_ws_bytes<double>(pe);
   return 512 + ws + (((size_t)pe * sz + 15) & ~(size_t)15);
 }
-static inline size_t psd_small_smem_fwd(int p, size_t sz) { return psd_small_smem_bytes(p, sz); }
-static inline size_t psd_small_smem_bwd(int p, size_t sz) { return psd_small_smem_bytes(p, sz); }
+
+// Launch shape of the small-block kernels for blocks up to order pmax: every work thread owns at most `maxi`
+// 2x2 blocks and eigenvector slices (register resident), plus the angle warps. maxi <= PSD_SMALL_MAXI.
+constexpr int PSD_SMALL_MAXI = 4;
+struct PsdSmallCfg { int maxi, threads; };
+static inline PsdSmallCfg psd_small_cfg(int pmax, size_t sz) {
+  const int pe = (pmax + 1) & ~1, need = jacobi_need(pe, sz);
+  int maxi = 1;
+  while (maxi <= PSD_SMALL_MAXI && need > maxi * (psd_small_max_threads(maxi) - JACOBI_ANGLE_THREADS)) ++maxi;
+  int ntw = (((need + maxi - 1) / maxi) + 31) & ~31;
+  if (ntw < 32) ntw = 32;
+  return PsdSmallCfg{maxi, ntw + JACOBI_ANGLE_THREADS};
+}
 
 }  // namespace cdu
