@@ -204,12 +204,14 @@ def main():
     ap.add_argument("--p", type=int, default=None, help="override the graph order / n (debug)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--cg-refine", type=int, default=-1)
+    ap.add_argument("--cg-refine", type=int, default=-2, help="-2: workload default (cfg3: 0, others: handle default)")
     ap.add_argument("--cg-refine-tol", type=float, default=0.0)
     ap.add_argument("--tensor-cores", type=int, default=-1)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     cfg = WORKLOADS[args.workload]
+    if args.cg_refine == -2:
+        args.cg_refine = 0 if cfg == 3 else -1
     if args.impl == "reference":
         return run_reference(args, cfg)
 

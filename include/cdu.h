@@ -77,6 +77,10 @@ typedef struct {
                                the global-memory path; <= 0: default (128 for F32, 88 for F64)                  */
   int32_t use_tensor_cores; /* large-block rebuild / DK products: 1 = tcgen05 3xTF32 GEMM, 0 = fp32 FMA GEMM;
                                < 0: default                                                                     */
+  int32_t team_size;        /* CTAs (thread-block cluster size, power of two <= 16) that share one problem in the
+                               linear-step kernels; <= 0: chosen from the batch size and the problem size         */
+  int32_t no_batch;         /* 1: single-CTA teams read rows with lane groups straight from global memory instead of
+                               the precomputed warp batches (debug / comparison)                                  */
 } cdu_options;
 
 /* Copies and re-packs the batch onto the current CUDA device (transposed copy of A, diag(P), column square

@@ -322,10 +322,12 @@ struct PsdEngine {
 // ---------------------------------------------------------------------------------------------------------
 // handle
 // ---------------------------------------------------------------------------------------------------------
-template <typename T>
+template <typename T, typename IT>
 struct HandleT : cdu_handle_s {
   DevPool pool;
-  BatchDev<T> D{};
+  BatchDev<T, IT> D{};
+  int team_C = 1, lin_grid = 1;      // CTAs per team (cluster size), persistent grid size
+  size_t lin_smem = 0;               // dynamic shared memory of the linear-step kernels
   PsdEngine<T> psd;
   int B = 0, K_max = 0, ckpt_mode = 0, lin_threads = 256;
   long long N = 0, Mtot = 0;
@@ -351,6 +353,20 @@ struct HandleT : cdu_handle_s {
 
   double* z_at(int k) { return Z + (size_t)k * zstride; }
 
+  // One launch of a linear-step kernel over the whole batch: persistent CTAs (team_C == 1) or clusters of team_C CTAs.
+  template <typename... Args>
+  cudaError_t launch_lin(void (*single)(Args...), void (*multi)(Args...), cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(lin_grid); cfg.blockDim = dim3(lin_threads); cfg.dynamicSmemBytes = lin_smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    if (team_C > 1) {
+      at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = team_C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      return cudaLaunchKernelEx(&cfg, multi, args...);
+    }
+    return cudaLaunchKernelEx(&cfg, single, args...);
+  }
+
   cdu_status init(const cdu_problem* pr, const cdu_options* op, cudaStream_t st);
   Hyper<T> hyper() const {
     Hyper<T> H;
@@ -370,8 +386,8 @@ struct HandleT : cdu_handle_s {
   cdu_status import_state(double* z, const void* x, const void* s, const void* y, int host, cudaStream_t st);
 };
 
-template <typename T>
-cdu_status HandleT<T>::init(const cdu_problem* pr, const cdu_options* op, cudaStream_t st) {
+template <typename T, typename IT>
+cdu_status HandleT<T, IT>::init(const cdu_problem* pr, const cdu_options* op, cudaStream_t st) {
   B = pr->batch;
   if (B < 1 || !pr->var_off || !pr->row_off || !pr->A_rowptr || !pr->P_rowptr || !pr->cone_off || !pr->cones || !pr->q || !pr->b) {
     err = "cdu_create: NULL array or batch < 1"; return CDU_EINVAL;
@@ -389,7 +405,7 @@ cdu_status HandleT<T>::init(const cdu_problem* pr, const cdu_options* op, cudaSt
   if ((nnzA && (!pr->A_colidx || !pr->A_val)) || (nnzP && (!pr->P_colidx || !pr->P_val))) { err = "cdu_create: NULL CSR arrays"; return CDU_EINVAL; }
   cdu_options o{};
   if (op) o = *op;
-  else { o.cg_refine = -1; o.use_tensor_cores = -1; }
+  else { o.cg_refine = -1; o.use_tensor_cores = -1; o.team_size = 0; o.no_batch = 0; }
   if (o.K_max < 1) { err = "cdu_create: options.K_max must be >= 1"; return CDU_EINVAL; }
   const bool f32 = std::is_same<T, float>::value;
   K_max = o.K_max; ckpt_mode = o.ckpt_mode == CDU_CKPT_LEAN ? CDU_CKPT_LEAN : CDU_CKPT_FULL;
@@ -421,19 +437,25 @@ cdu_status HandleT<T>::init(const cdu_problem* pr, const cdu_options* op, cudaSt
   // ---- CSR re-packing: int32 rowptr, transposed copy, diag(P), column square sums ----------------------------
   const T* Av = reinterpret_cast<const T*>(pr->A_val);
   const T* Pv = reinterpret_cast<const T*>(pr->P_val);
-  std::vector<int> A_rp((size_t)Mtot + 1), P_rp((size_t)N + 1), AT_rp((size_t)N + 1, 0), AT_ci((size_t)nnzA);
+  std::vector<int> A_rp((size_t)Mtot + 1), P_rp((size_t)N + 1), AT_rp((size_t)N + 1, 0);
+  std::vector<IT> A_ci((size_t)nnzA), AT_ci((size_t)nnzA), P_ci;
   std::vector<T> AT_v((size_t)nnzA), diagP((size_t)N, (T)0), colsq((size_t)N, (T)0);
+  std::vector<long long> P_off(B, 0);
   for (long long i = 0; i <= Mtot; ++i) A_rp[i] = (int)pr->A_rowptr[i];
   for (long long i = 0; i <= N; ++i) P_rp[i] = (int)pr->P_rowptr[i];
   for (long long i = 0; i < Mtot; ++i) if (A_rp[i + 1] < A_rp[i]) { err = "cdu_create: A_rowptr not monotone"; return CDU_EINVAL; }
   for (long long i = 0; i < N; ++i) if (P_rp[i + 1] < P_rp[i]) { err = "cdu_create: P_rowptr not monotone"; return CDU_EINVAL; }
+  bool p_dense = nnzP > 0;      // every P_b stored as all n_b^2 entries with sorted columns -> no index array needed
+  long long nnz_max = 0, pnn_max = 0;
   {
     std::vector<double> csq((size_t)N, 0.0);
     for (int b = 0; b < B; ++b) {
       const long long v0 = pr->var_off[b], n = pr->var_off[b + 1] - v0, r0 = pr->row_off[b], r1 = pr->row_off[b + 1];
+      nnz_max = std::max<long long>(nnz_max, A_rp[r1] - A_rp[r0]);
       for (long long e = A_rp[r0]; e < A_rp[r1]; ++e) {
         const int c = pr->A_colidx[e];
         if (c < 0 || c >= n) { err = "cdu_create: A column index out of range"; return CDU_EINVAL; }
+        A_ci[e] = (IT)c;
         ++AT_rp[v0 + c + 1];
       }
     }
@@ -445,20 +467,27 @@ cdu_status HandleT<T>::init(const cdu_problem* pr, const cdu_options* op, cudaSt
         for (long long e = A_rp[r]; e < A_rp[r + 1]; ++e) {
           const long long col = v0 + pr->A_colidx[e];
           const int dst = fill[col]++;
-          AT_ci[dst] = (int)(r - r0);
+          AT_ci[dst] = (IT)(r - r0);
           AT_v[dst] = Av[e];
           csq[col] += (double)Av[e] * (double)Av[e];
         }
       const long long n = pr->var_off[b + 1] - v0;
-      for (long long i = 0; i < n; ++i)
+      P_off[b] = P_rp[v0];
+      pnn_max = std::max<long long>(pnn_max, P_rp[v0 + n] - P_rp[v0]);
+      if (P_rp[v0 + n] - P_rp[v0] != n * n) p_dense = false;
+      for (long long i = 0; i < n; ++i) {
+        if (P_rp[v0 + i + 1] - P_rp[v0 + i] != n) p_dense = false;
         for (long long e = P_rp[v0 + i]; e < P_rp[v0 + i + 1]; ++e) {
           const int c = pr->P_colidx[e];
           if (c < 0 || c >= n) { err = "cdu_create: P column index out of range"; return CDU_EINVAL; }
+          if (c != e - P_rp[v0 + i]) p_dense = false;
           if (c == i) diagP[v0 + i] += Pv[e];
         }
+      }
     }
     for (long long i = 0; i < N; ++i) colsq[i] = (T)csq[i];
   }
+  if (!p_dense) { P_ci.resize((size_t)nnzP); for (long long e = 0; e < nnzP; ++e) P_ci[e] = (IT)pr->P_colidx[e]; }
   std::vector<int> var_off32(B + 1), row_off32(B + 1);
   for (int b = 0; b <= B; ++b) { var_off32[b] = (int)pr->var_off[b]; row_off32[b] = (int)pr->row_off[b]; }
 
@@ -467,17 +496,18 @@ cdu_status HandleT<T>::init(const cdu_problem* pr, const cdu_options* op, cudaSt
   D.var_off = pool.upload(var_off32, st); D.row_off = pool.upload(row_off32, st);
   D.A_rp = pool.upload(A_rp, st); D.P_rp = pool.upload(P_rp, st); D.AT_rp = pool.upload(AT_rp, st);
   {
-    int* ci = pool.alloc<int>(nnzA); T* v = pool.alloc<T>(nnzA);
-    int* pci = pool.alloc<int>(nnzP); T* pv = pool.alloc<T>(nnzP);
+    T* v = pool.alloc<T>(nnzA); T* pv = pool.alloc<T>(nnzP);
     T* q = pool.alloc<T>(N); T* bb = pool.alloc<T>(Mtot);
-    if (!ci || !v || !pci || !pv || !q || !bb) { err = "cudaMalloc (problem data)"; return CDU_ENOMEM; }
-    if (nnzA) { CU_OK(cudaMemcpyAsync(ci, pr->A_colidx, nnzA * sizeof(int), cudaMemcpyHostToDevice, st)); CU_OK(cudaMemcpyAsync(v, Av, nnzA * sizeof(T), cudaMemcpyHostToDevice, st)); }
-    if (nnzP) { CU_OK(cudaMemcpyAsync(pci, pr->P_colidx, nnzP * sizeof(int), cudaMemcpyHostToDevice, st)); CU_OK(cudaMemcpyAsync(pv, Pv, nnzP * sizeof(T), cudaMemcpyHostToDevice, st)); }
+    if (!v || !pv || !q || !bb) { err = "cudaMalloc (problem data)"; return CDU_ENOMEM; }
+    if (nnzA) CU_OK(cudaMemcpyAsync(v, Av, nnzA * sizeof(T), cudaMemcpyHostToDevice, st));
+    if (nnzP) CU_OK(cudaMemcpyAsync(pv, Pv, nnzP * sizeof(T), cudaMemcpyHostToDevice, st));
     CU_OK(cudaMemcpyAsync(q, pr->q, N * sizeof(T), cudaMemcpyHostToDevice, st));
     if (Mtot) CU_OK(cudaMemcpyAsync(bb, pr->b, Mtot * sizeof(T), cudaMemcpyHostToDevice, st));
-    D.A_ci = ci; D.A_v = v; D.P_ci = pci; D.P_v = pv; D.q = q; D.b = bb;
+    D.A_v = v; D.P_v = pv; D.q = q; D.b = bb;
   }
+  D.A_ci = pool.upload(A_ci, st); D.P_ci = pool.upload(P_ci, st);
   D.AT_ci = pool.upload(AT_ci, st); D.AT_v = pool.upload(AT_v, st);
+  D.P_dense = p_dense ? 1 : 0; D.P_off = pool.upload(P_off, st);
   D.diagP = pool.upload(diagP, st); D.colsq = pool.upload(colsq, st);
   D.rowkind = pool.upload(rowkind, st);
   D.soc_off = pool.upload(soc_off, st); D.soc_start = pool.upload(soc_start, st); D.soc_dim = pool.upload(soc_dim, st);
@@ -486,8 +516,8 @@ cdu_status HandleT<T>::init(const cdu_problem* pr, const cdu_options* op, cudaSt
   D.AT_G = pow2_group((double)nnzA / (double)N);
   D.P_G = pow2_group((double)nnzP / (double)N);
   // scratch
-  D.xi = pool.alloc<double>(N); D.xt_scr = pool.alloc<double>(N); D.rd = pool.alloc<double>(N); D.lam = pool.alloc<double>(N);
-  D.tm = pool.alloc<double>(Mtot); D.st_scr = pool.alloc<double>(Mtot); D.W = pool.alloc<double>(Mtot); D.GW = pool.alloc<double>(Mtot);
+  D.xi = pool.alloc<double>(N); D.rd = pool.alloc<double>(N); D.lam = pool.alloc<double>(N);
+  D.tm = pool.alloc<double>(Mtot); D.W = pool.alloc<double>(Mtot); D.GW = pool.alloc<double>(Mtot);
   D.r = pool.alloc<T>(N); D.p = pool.alloc<T>(N); D.Ap = pool.alloc<T>(N); D.d = pool.alloc<T>(N); D.dinv = pool.alloc<T>(N);
   D.tA = pool.alloc<T>(Mtot);
   D.tol = o.cg_tol > 0 ? o.cg_tol : (f32 ? 1e-6 : 1e-10);
@@ -496,8 +526,97 @@ cdu_status HandleT<T>::init(const cdu_problem* pr, const cdu_options* op, cudaSt
   D.maxit = o.cg_max_iter > 0 ? o.cg_max_iter : 2 * nmax + 50;
   cg_f = pool.zeros<int>(B, st); cg_b = pool.zeros<int>(B, st); cg_max = pool.zeros<int>(B, st); flags = pool.zeros<int>(B, st);
   D.cg_iters = cg_f; D.cg_max = cg_max; D.flags = flags;
-  lin_threads = std::max(nmax, mmax) <= 16384 ? 256 : 1024;
   if (pool.last != cudaSuccess) { err = std::string("cdu_create: ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
+
+  // ---- team shape (lin.cuh): cluster size, CTA size, shared-memory residency, persistent grid -----------------
+  {
+    int dev = 0, nsm = 148, smem_optin = 227 * 1024;
+    CU_OK(cudaGetDevice(&dev));
+    CU_OK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    CU_OK(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    const long long big = std::max(nmax, mmax);
+    int C = 1;
+    while (C < 16 && (long long)B * C * 2 <= nsm && big / (C * 2) >= 2048) C *= 2;
+    if (o.team_size > 0) { C = 1; while (C * 2 <= std::min(o.team_size, 16)) C *= 2; }
+    const long long work = std::max<long long>(big, nnz_max / 8) / C;
+    lin_threads = 128;
+    while (lin_threads < 1024 && lin_threads * 4 < work) lin_threads *= 2;
+    const size_t ns = ((size_t)nmax + 3) & ~(size_t)3, ms = ((size_t)mmax + 3) & ~(size_t)3;
+    const size_t vec_bytes = (5 * ns + ms) * sizeof(T);
+    const size_t pd_bytes = (((size_t)pnn_max + 3) & ~(size_t)3) * sizeof(T);
+    const size_t budget = (size_t)smem_optin - 2048;
+    D.vec_smem = (C == 1 && vec_bytes <= std::min<size_t>(budget, 96 * 1024)) ? 1 : 0;
+    D.P_smem = (C == 1 && p_dense && D.vec_smem && pd_bytes + vec_bytes <= budget) ? 1 : 0;
+    lin_smem = (D.vec_smem ? vec_bytes : 0) + (D.P_smem ? pd_bytes : 0);
+    team_C = C;
+    // ---- warp row batches (lin.cuh batch_rows): single-CTA teams with shared-memory vectors -------------------------
+    D.batched = 0; D.rp_smem = 0; D.nmax = nmax; D.mmax = mmax;
+    if (C == 1 && D.vec_smem && o.no_batch == 0) {
+      const size_t rp_bytes = ((((size_t)mmax + 1 + 3) & ~(size_t)3) + 2 * (((size_t)nmax + 1 + 3) & ~(size_t)3)) * sizeof(int);
+      const size_t fixed = (size_t)(lin_threads / 32) * BATCH_ELEMS * sizeof(double) + rp_bytes + vec_bytes;
+      if (fixed <= budget) {
+        D.batched = 1; D.rp_smem = 1;
+        D.P_smem = (p_dense && fixed + pd_bytes <= budget) ? 1 : 0;
+        lin_smem = fixed + (D.P_smem ? pd_bytes : 0);
+      }
+    }
+    if (D.batched) {
+      auto build = [&](const std::vector<int>& rp, const int64_t* off, std::vector<int2>& bt, std::vector<int>& bo) {
+        bo.assign(B + 1, 0);
+        for (int b = 0; b < B; ++b) {
+          const long long r0 = off[b], r1 = off[b + 1];
+          long long row = r0;
+          while (row < r1) {
+            const int len = rp[row + 1] - rp[row];
+            if (len >= LONG_ROW) { bt.push_back(make_int2((int)(row - r0), -1)); ++row; continue; }
+            const long long first = row;
+            int tot = 0;
+            while (row < r1 && row - first < 128) {
+              const int l = rp[row + 1] - rp[row];
+              if (l >= LONG_ROW || tot + l > BATCH_ELEMS) break;
+              tot += l; ++row;
+            }
+            bt.push_back(make_int2((int)(first - r0), (int)(row - first)));
+          }
+          bo[b + 1] = (int)bt.size();
+        }
+      };
+      std::vector<int2> bta, btt, btp;
+      std::vector<int> boa, bot, bop;
+      build(A_rp, pr->row_off, bta, boa);
+      build(AT_rp, pr->var_off, btt, bot);
+      if (!p_dense) build(P_rp, pr->var_off, btp, bop); else bop.assign(B + 1, 0);
+      D.A_bt = pool.upload(bta, st); D.AT_bt = pool.upload(btt, st); D.P_bt = pool.upload(btp, st);
+      D.A_bo = pool.upload(boa, st); D.AT_bo = pool.upload(bot, st); D.P_bo = pool.upload(bop, st);
+      if (pool.last != cudaSuccess) { err = std::string("cdu_create (batches): ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
+      CU_OK(cudaStreamSynchronize(st));   // the staging vectors go out of scope
+    }
+    const void* fns[4] = {(const void*)k_fwd<T, IT, false>, (const void*)k_bwd<T, IT, false>, (const void*)k_fwd<T, IT, true>,
+                          (const void*)k_bwd<T, IT, true>};
+    for (int i = 0; i < 4; ++i) {
+      CU_OK(cudaFuncSetAttribute(fns[i], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(lin_smem, 1024)));
+      if (i >= 2 && C > 8) CU_OK(cudaFuncSetAttribute(fns[i], cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    }
+    if (C == 1) {
+      int occ = 1;
+      CU_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bwd<T, IT, false>, lin_threads, lin_smem));
+      occ = std::max(occ, 1);
+      // keep the matrices of the problems in flight inside L2 (126 MB): they are re-read every CG iteration
+      const double ws = ((double)nnzA * 2.0 * (sizeof(T) + sizeof(IT)) + (D.P_smem ? 0.0 : (double)nnzP * (sizeof(T) + (p_dense ? 0 : sizeof(IT))))) / B;
+      const long long conc = (long long)(96.0 * 1024 * 1024 / std::max(ws, 1.0));
+      lin_grid = (int)std::min<long long>(B, std::min<long long>((long long)nsm * occ, std::max<long long>(conc, nsm)));
+    } else {
+      cudaLaunchConfig_t cfg{};
+      cfg.gridDim = dim3(B * C); cfg.blockDim = dim3(lin_threads); cfg.dynamicSmemBytes = lin_smem;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      int ncl = 0;
+      cudaError_t e = cudaOccupancyMaxActiveClusters(&ncl, k_bwd<T, IT, true>, &cfg);
+      if (e != cudaSuccess || ncl < 1) { (void)cudaGetLastError(); err = "cdu_create: cluster launch not possible for the linear-step kernels"; return CDU_ECUDA; }
+      lin_grid = std::min(B, ncl) * C;
+    }
+  }
 
   // ---- PSD engine -----------------------------------------------------------------------------------------
   {
@@ -526,8 +645,8 @@ cdu_status HandleT<T>::init(const cdu_problem* pr, const cdu_options* op, cudaSt
   return CDU_OK;
 }
 
-template <typename T>
-cdu_status HandleT<T>::import_state(double* z, const void* x, const void* s, const void* y, int host, cudaStream_t st) {
+template <typename T, typename IT>
+cdu_status HandleT<T, IT>::import_state(double* z, const void* x, const void* s, const void* y, int host, cudaStream_t st) {
   const void* src[3] = {x, s, y};
   const long long len[3] = {N, Mtot, Mtot};
   double* dst[3] = {z, z + N, z + N + Mtot};
@@ -545,8 +664,8 @@ cdu_status HandleT<T>::import_state(double* z, const void* x, const void* s, con
   return CDU_OK;
 }
 
-template <typename T>
-cdu_status HandleT<T>::export_state(const double* z, void* x, void* s, void* y, int host, cudaStream_t st) {
+template <typename T, typename IT>
+cdu_status HandleT<T, IT>::export_state(const double* z, void* x, void* s, void* y, int host, cudaStream_t st) {
   void* dstp[3] = {x, s, y};
   const long long len[3] = {N, Mtot, Mtot};
   const double* src[3] = {z, z + N, z + N + Mtot};
@@ -562,8 +681,8 @@ cdu_status HandleT<T>::export_state(const double* z, void* x, void* s, void* y, 
   return CDU_OK;
 }
 
-template <typename T>
-cdu_status HandleT<T>::forward(int K, const void* rho, int mode, double sigma, const void* alpha, const void* x0,
+template <typename T, typename IT>
+cdu_status HandleT<T, IT>::forward(int K, const void* rho, int mode, double sigma, const void* alpha, const void* x0,
                                const void* s0, const void* y0, void* xK, void* sK, void* yK, int host, cudaStream_t st) {
   if (K < 1 || K > K_max) { err = "cdu_forward: K out of [1, K_max]"; return CDU_EINVAL; }
   if (!rho || !alpha) { err = "cdu_forward: NULL rho/alpha"; return CDU_EINVAL; }
@@ -587,17 +706,17 @@ cdu_status HandleT<T>::forward(int K, const void* rho, int mode, double sigma, c
   CU_OK(cudaMemsetAsync(psd.sweeps_max, 0, sizeof(int), st));
   CU_OK(cudaMemsetAsync(psd.sweeps_sum, 0, sizeof(unsigned long long), st));
   const Hyper<T> H = hyper();
-  BatchDev<T> Df = D; Df.cg_iters = cg_f;
+  BatchDev<T, IT> Df = D; Df.cg_iters = cg_f;
   const bool full = ckpt_mode == CDU_CKPT_FULL;
   for (int k = 0; k < K; ++k) {
     IterPtrs I;
     I.Zk = z_at(k); I.Zk1 = z_at(k + 1);
     I.XT = XT + (full ? (size_t)k * N : 0); I.ST = ST + (full ? (size_t)k * Mtot : 0);
     prof.begin(PC_LIN_FWD, st);
-    k_fwd<T><<<B, lin_threads, 0, st>>>(Df, H, I, k);
+    cudaError_t le = launch_lin(k_fwd<T, IT, false>, k_fwd<T, IT, true>, st, Df, H, I, k);
     prof.end(st);
     ++launches;
-    CU_OK(cudaGetLastError());
+    CU_OK(le);
     if (has_psd) {
       PsdFwdArgs A;
       A.W = D.W; A.S1 = z_at(k + 1) + N; A.Y1 = z_at(k + 1) + N + Mtot;
@@ -614,8 +733,8 @@ cdu_status HandleT<T>::forward(int K, const void* rho, int mode, double sigma, c
   return CDU_OK;
 }
 
-template <typename T>
-cdu_status HandleT<T>::backward(const void* gx, const void* gs, const void* gy, void* g_rho, void* g_sigma, void* g_alpha,
+template <typename T, typename IT>
+cdu_status HandleT<T, IT>::backward(const void* gx, const void* gs, const void* gy, void* g_rho, void* g_sigma, void* g_alpha,
                                 void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st) {
   if (K_last < 1) { err = "cdu_backward: no forward pass on this handle"; return CDU_ESTATE; }
   const int K = K_last;
@@ -624,7 +743,7 @@ cdu_status HandleT<T>::backward(const void* gx, const void* gs, const void* gy, 
   if (s != CDU_OK) return s;
   CU_OK(cudaMemsetAsync(cg_b, 0, B * sizeof(int), st));
   const Hyper<T> H = hyper();
-  BatchDev<T> Db = D; Db.cg_iters = cg_b;
+  BatchDev<T, IT> Db = D; Db.cg_iters = cg_b;
   const bool full = ckpt_mode == CDU_CKPT_FULL;
   for (int k = K - 1; k >= 0; --k) {
     BwdPtrs Q;
@@ -635,16 +754,16 @@ cdu_status HandleT<T>::backward(const void* gx, const void* gs, const void* gy, 
     Q.recompute = full ? 0 : 1;
     if (!has_psd) {
       prof.begin(PC_LIN_BWD, st);
-      k_bwd<T><<<B, lin_threads, 0, st>>>(Db, H, Q, k, 0);
+      cudaError_t le = launch_lin(k_bwd<T, IT, false>, k_bwd<T, IT, true>, st, Db, H, Q, k, 0);
       prof.end(st);
       ++launches;
-      CU_OK(cudaGetLastError());
+      CU_OK(le);
     } else {
       prof.begin(PC_LIN_BWD, st);
-      k_bwd<T><<<B, lin_threads, 0, st>>>(Db, H, Q, k, 1);
+      cudaError_t le = launch_lin(k_bwd<T, IT, false>, k_bwd<T, IT, true>, st, Db, H, Q, k, 1);
       prof.end(st);
       ++launches;
-      CU_OK(cudaGetLastError());
+      CU_OK(le);
       PsdBwdArgs A;
       A.W = D.W; A.Yk = z_at(k) + N + Mtot; A.S1 = z_at(k + 1) + N;
       A.Gs = Q.Gin + N; A.Gy = Q.Gin + N + Mtot; A.GW = D.GW; A.part = D.psd_part;
@@ -653,10 +772,10 @@ cdu_status HandleT<T>::backward(const void* gx, const void* gs, const void* gy, 
       s = psd.backward(H, k, A, st);
       if (s != CDU_OK) { err = psd.err; return s; }
       prof.begin(PC_LIN_BWD, st);
-      k_bwd<T><<<B, lin_threads, 0, st>>>(Db, H, Q, k, 2);
+      le = launch_lin(k_bwd<T, IT, false>, k_bwd<T, IT, true>, st, Db, H, Q, k, 2);
       prof.end(st);
       ++launches;
-      CU_OK(cudaGetLastError());
+      CU_OK(le);
     }
   }
   const int pp = mode_last == CDU_RHO_PER_PROBLEM;
@@ -679,8 +798,8 @@ cdu_status HandleT<T>::backward(const void* gx, const void* gs, const void* gy, 
   return CDU_OK;
 }
 
-template <typename T>
-cdu_status HandleT<T>::iterate(int k, void* x, void* s, void* y, int host, cudaStream_t st) {
+template <typename T, typename IT>
+cdu_status HandleT<T, IT>::iterate(int k, void* x, void* s, void* y, int host, cudaStream_t st) {
   if (k < 0 || k > K_last) { err = "cdu_get_iterate: k out of range"; return CDU_EINVAL; }
   cdu_status r = export_state(z_at(k), x, s, y, host, st);
   if (r != CDU_OK) return r;
@@ -688,8 +807,8 @@ cdu_status HandleT<T>::iterate(int k, void* x, void* s, void* y, int host, cudaS
   return CDU_OK;
 }
 
-template <typename T>
-cdu_status HandleT<T>::stats(cdu_stats* out) {
+template <typename T, typename IT>
+cdu_status HandleT<T, IT>::stats(cdu_stats* out) {
   if (!out) { err = "cdu_get_stats: NULL out"; return CDU_EINVAL; }
   CU_OK(cudaStreamSynchronize(last_stream));
   std::vector<int> f(B), bw(B), mx(B), fl(B);
@@ -714,9 +833,9 @@ cdu_status HandleT<T>::stats(cdu_stats* out) {
   return CDU_OK;
 }
 
-template <typename T>
+template <typename T, typename IT>
 cdu_status create_t(const cdu_problem* pr, const cdu_options* op, cudaStream_t st, cdu_handle* out) {
-  HandleT<T>* h = new (std::nothrow) HandleT<T>();
+  HandleT<T, IT>* h = new (std::nothrow) HandleT<T, IT>();
   if (!h) { g_create_err = "out of host memory"; return CDU_ENOMEM; }
   cdu_status s;
   try { s = h->init(pr, op, st); }
@@ -820,8 +939,11 @@ cdu_status cdu_create(const cdu_problem* prob, const cdu_options* opts, void* cu
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { g_create_err = "cdu_create: no CUDA device (there is no CPU fallback)"; return CDU_ECUDA; }
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
-  if (prob->dtype == CDU_F32) return create_t<float>(prob, opts, st, out);
-  if (prob->dtype == CDU_F64) return create_t<double>(prob, opts, st, out);
+  bool narrow = prob->batch >= 1 && prob->var_off && prob->row_off;      // 16-bit local indices suffice
+  for (int b = 0; narrow && b < prob->batch; ++b)
+    if (prob->var_off[b + 1] - prob->var_off[b] > 65535 || prob->row_off[b + 1] - prob->row_off[b] > 65535) narrow = false;
+  if (prob->dtype == CDU_F32) return narrow ? create_t<float, uint16_t>(prob, opts, st, out) : create_t<float, int>(prob, opts, st, out);
+  if (prob->dtype == CDU_F64) return narrow ? create_t<double, uint16_t>(prob, opts, st, out) : create_t<double, int>(prob, opts, st, out);
   g_create_err = "cdu_create: bad dtype";
   return CDU_EINVAL;
 }

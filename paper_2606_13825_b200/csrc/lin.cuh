@@ -1,30 +1,44 @@
 // lin.cuh - per-problem linear-system step, relaxation, separable/SOC cones, and their reverse.
 //
-// One CTA owns one problem instance of the batch ("super-batch" of PAPER.md L306 held as batched CSR with
-// per-problem offsets; CG convergence is decided per problem on the device, never by the host).
+// One TEAM owns one problem instance at a time ("super-batch" of PAPER.md L306 held as batched CSR with per-problem
+// offsets; CG convergence is decided per problem on the device, never by the host). A team is one CTA, or - when
+// the batch has fewer problems than the GPU has SMs - a thread-block cluster of C CTAs that split the rows of every
+// pass and reduce dot products through distributed shared memory. Teams are persistent: the grid is sized so that the
+// matrices of the problems in flight stay resident in the 126 MB L2 across the CG iterations, and loops over the batch.
 //   forward  : S1 xi assembly, S2 PCG on M = P + sigma I + rho A'A (Eq. 4, Jacobi preconditioner L294),
 //              S3 st = b - A xt, S4 relaxation (Eq. 3c-3d), S5 zero/nonneg/SOC projection, S7 dual
 //              update (Eq. 3e) - SURVEY.md 8(a).
 //   backward : S9 (separable + SOC part), S10, S11 adjoint PCG (Eq. 5), S12 Eq. 6 (L90) and the RHS terms.
-// The iterate and every reduction are fp64; matrices, CG vectors and the preconditioner are T.
+// The iterate and every reduction are fp64; matrices, CG vectors and the preconditioner are T. Column indices are IT
+// (uint16_t when every n_b, m_b < 65536). A fully dense P is stored without indices and, if it fits, cached in shared
+// memory together with the CG vectors.
 #pragma once
+#include <cooperative_groups.h>
 #include "common.cuh"
 
 namespace cdu {
+namespace cg = cooperative_groups;
 
-template <typename T>
+template <typename T, typename IT>
 struct BatchDev {
   int B;
-  const int *var_off, *row_off;                       // [B+1]
-  const int *A_rp, *A_ci;   const T* A_v;   int A_G;   // A   : rows = constraints, local column index
-  const int *AT_rp, *AT_ci; const T* AT_v;  int AT_G;  // A^T : rows = variables,   local row index
-  const int *P_rp, *P_ci;   const T* P_v;   int P_G;   // P   : full symmetric storage
+  const int *var_off, *row_off;                        // [B+1]
+  const int *A_rp;  const IT* A_ci;  const T* A_v;  int A_G;   // A   : rows = constraints, local column index
+  const int *AT_rp; const IT* AT_ci; const T* AT_v; int AT_G;  // A^T : rows = variables,   local row index
+  const int *P_rp;  const IT* P_ci;  const T* P_v;  int P_G;   // P   : full symmetric storage (CSR), or
+  int P_dense; const long long* P_off;                 //       dense row-major n_b x n_b blocks at P_v + P_off[b]
+  int P_smem, vec_smem;                                // dense P / CG vectors live in dynamic shared memory
+  // row batches (single-CTA teams): warp-sized work items built by cdu_create. bt = (first row, number of rows);
+  // rows shorter than LONG_ROW are packed into batches of at most BATCH_ELEMS elements, a longer row is a batch of
+  // its own (count -1). bo = per-problem offsets [B+1]. rp_smem: local row pointers are copied to shared memory.
+  int batched, rp_smem, nmax, mmax;
+  const int2 *A_bt, *AT_bt, *P_bt; const int *A_bo, *AT_bo, *P_bo;
   const T *q, *b, *diagP, *colsq;
   const uint8_t* rowkind;                              // per row: cone kind
   const int *soc_off, *soc_start, *soc_dim;            // per problem SOC list (start = local row)
   const int *psdblk_off;                               // [B+1] PSD blocks of each problem
-  double *xi, *xt_scr, *rd, *tm, *st_scr, *W, *GW, *lam;   // fp64 scratch, sized sum n / sum m
-  T *r, *p, *Ap, *d, *dinv, *tA;                        // CG vectors
+  double *xi, *rd, *tm, *W, *GW, *lam;                 // fp64 scratch, sized sum n / sum m
+  T *r, *p, *Ap, *d, *dinv, *tA;                       // CG vectors (global copies; unused parts when vec_smem)
   double tol, tol_ref;
   int maxit, refine;
   int *cg_iters, *cg_max, *flags;                      // [B] statistics
@@ -39,81 +53,276 @@ struct Hyper {  // per-iteration hyper-parameters as the caller laid them out (c
   __device__ double alpha_at(int k, int b) const { return (double)alpha[(size_t)k * kstride + (size_t)b * pstride]; }
 };
 
-// y = op(rows) . x with a group of G (power of two <= 32) lanes per row; emit(row, dot) runs on lane 0 of the group.
-template <typename TACC, typename TV, typename TX, typename F>
-__device__ __forceinline__ void spmv_rows(int nrows, const int* __restrict__ rp, const int* __restrict__ ci,
+// ---- team = CTA or cluster ---------------------------------------------------------------------------------
+template <bool MULTI>
+struct Team {
+  int C, rank, parity;
+  double* sh;       // [3*32] block_sum scratch
+  double* slots;    // [2][4] partials exchanged through DSMEM
+  double* bc;       // [4] broadcast
+  __device__ void init(double* sh_, double* slots_, double* bc_) {
+    sh = sh_; slots = slots_; bc = bc_; parity = 0;
+    if (MULTI) { cg::cluster_group cl = cg::this_cluster(); C = (int)cl.num_blocks(); rank = (int)cl.block_rank(); }
+    else { C = 1; rank = 0; }
+  }
+  __device__ __forceinline__ void sync() const {
+    if (MULTI) cg::this_cluster().sync(); else __syncthreads();
+  }
+  __device__ __forceinline__ void range(int len, int& lo, int& hi) const {
+    if (MULTI) { lo = (int)((long long)len * rank / C); hi = (int)((long long)len * (rank + 1) / C); }
+    else { lo = 0; hi = len; }
+  }
+  // Deterministic team-wide sum; every thread of every CTA returns the same bits.
+  template <int NV> __device__ void sum(double (&v)[NV]) {
+    block_sum<NV>(v, sh);
+    if (MULTI) {
+      double* slot = slots + parity * 4;
+      if (threadIdx.x == 0) {
+#pragma unroll
+        for (int i = 0; i < NV; ++i) slot[i] = v[i];
+      }
+      cg::cluster_group cl = cg::this_cluster();
+      cl.sync();
+      if (threadIdx.x < 32) {
+        const int lane = threadIdx.x;
+        const double* rs = cl.map_shared_rank(slot, lane < C ? lane : 0);
+#pragma unroll
+        for (int i = 0; i < NV; ++i) {
+          const double mine = lane < C ? rs[i] : 0.0;
+          double t = 0.0;
+          for (int r = 0; r < C; ++r) t += __shfl_sync(0xffffffffu, mine, r);
+          if (lane == 0) bc[i] = t;
+        }
+      }
+      __syncthreads();
+#pragma unroll
+      for (int i = 0; i < NV; ++i) v[i] = bc[i];
+      __syncthreads();
+      parity ^= 1;
+    }
+  }
+};
+
+template <bool MULTI, typename TX> __device__ __forceinline__ TX ldv(const TX* x) {
+  if (MULTI) return __ldcg(x);   // written by another CTA of the cluster during this launch: read at L2
+  return *x;
+}
+
+// y = op(rows [lo,hi)) . x with a group of G (power of two <= 32) lanes per row; emit(row, dot) runs on lane 0.
+template <typename TACC, bool MULTI, typename TV, typename IT, typename TX, typename F>
+__device__ __forceinline__ void spmv_rows(int lo, int hi, const int* __restrict__ rp, const IT* __restrict__ ci,
                                           const TV* __restrict__ v, const TX* x, int G, F emit) {
   const int tid = threadIdx.x;
   const int gl = tid & (G - 1);
   const int gid = tid / G, ng = blockDim.x / G;
-  for (int row0 = 0; row0 < nrows; row0 += ng) {
+  for (int row0 = lo; row0 < hi; row0 += ng) {
     const int row = row0 + gid;
     TACC acc = (TACC)0;
-    if (row < nrows) {
+    if (row < hi) {
       const int e0 = __ldg(rp + row), e1 = __ldg(rp + row + 1);
-#pragma unroll 4
-      for (int e = e0 + gl; e < e1; e += G) acc += (TACC)__ldg(v + e) * (TACC)x[__ldg(ci + e)];
+      int e = e0 + gl;
+      for (; e + 3 * G < e1; e += 4 * G) {       // four independent loads in flight per lane
+        const TV v0 = __ldg(v + e), v1 = __ldg(v + e + G), v2 = __ldg(v + e + 2 * G), v3 = __ldg(v + e + 3 * G);
+        const int c0 = __ldg(ci + e), c1 = __ldg(ci + e + G), c2 = __ldg(ci + e + 2 * G), c3 = __ldg(ci + e + 3 * G);
+        acc += (TACC)v0 * (TACC)ldv<MULTI>(x + c0);
+        acc += (TACC)v1 * (TACC)ldv<MULTI>(x + c1);
+        acc += (TACC)v2 * (TACC)ldv<MULTI>(x + c2);
+        acc += (TACC)v3 * (TACC)ldv<MULTI>(x + c3);
+      }
+      for (; e < e1; e += G) acc += (TACC)__ldg(v + e) * (TACC)ldv<MULTI>(x + (int)__ldg(ci + e));
     }
     for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if (row < nrows && gl == 0) emit(row, acc);
+    if (row < hi && gl == 0) emit(row, acc);
   }
 }
 
-template <typename T>
-struct Prob {  // one problem's view of the batch
+// Dense row-major block (n x n, global or shared): one warp per row.
+template <typename TACC, bool MULTI, typename TV, typename TX, typename F>
+__device__ __forceinline__ void dense_rows(int lo, int hi, int n, const TV* __restrict__ Pm, const TX* x, F emit) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  for (int row = lo + wid; row < hi; row += nw) {
+    const TV* pr = Pm + (size_t)row * n;
+    TACC a0 = (TACC)0, a1 = (TACC)0;
+    int j = lane;
+    for (; j + 32 < n; j += 64) {
+      a0 += (TACC)pr[j] * (TACC)ldv<MULTI>(x + j);
+      a1 += (TACC)pr[j + 32] * (TACC)ldv<MULTI>(x + j + 32);
+    }
+    if (j < n) a0 += (TACC)pr[j] * (TACC)ldv<MULTI>(x + j);
+    a0 += a1;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) a0 += __shfl_xor_sync(0xffffffffu, a0, o);
+    if (lane == 0) emit(row, a0);
+  }
+}
+
+// ---- batched rows: one warp per work item, every load of an item in flight at once ---------------------------
+constexpr int BATCH_ELEMS = 128;   // elements of a packed batch (4 loads per lane); scratch = 128 doubles per warp
+constexpr int LONG_ROW = 64;       // rows at least this long are taken by a whole warp
+
+// rows of one pass given as batches bt[0..nb): warps take batches round-robin. rp = local row pointers (shared or
+// global), v / ci = the problem's value / index arrays (element 0 = first element of local row 0).
+// emit(row, dot) runs on one lane per row (any lane).
+template <typename TACC, typename TV, typename IT, typename TX, typename F>
+__device__ __forceinline__ void batch_rows(const int2* __restrict__ bt, int nb, const int* rp, const TV* __restrict__ v,
+                                           const IT* __restrict__ ci, const TX* x, TACC* scratch, F emit) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  for (int i = warp; i < nb; i += nw) {
+    const int2 d = __ldg(bt + i);
+    if (d.y < 0) {   // one long row: strided by the warp, 8 loads per lane in flight
+      const int e0 = rp[d.x], e1 = rp[d.x + 1];
+      TACC acc = (TACC)0;
+      for (int base = e0 + lane; base < e1; base += 256) {
+        TV vv[8]; int cc[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const int e = base + 32 * j;
+          vv[j] = (TV)0; cc[j] = 0;
+          if (e < e1) { vv[j] = __ldg(v + e); cc[j] = (int)__ldg(ci + e); }
+        }
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc += (TACC)vv[j] * (TACC)x[cc[j]];
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+      if (lane == 0) emit(d.x, acc);
+    } else {         // d.y short rows, at most BATCH_ELEMS elements in total
+      const int e0 = rp[d.x], e1 = rp[d.x + d.y];
+      TV vv[4]; int cc[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int e = e0 + lane + 32 * j;
+        vv[j] = (TV)0; cc[j] = 0;
+        if (e < e1) { vv[j] = __ldg(v + e); cc[j] = (int)__ldg(ci + e); }
+      }
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+        if (e0 + lane + 32 * j < e1) scratch[lane + 32 * j] = (TACC)vv[j] * (TACC)x[cc[j]];
+      __syncwarp();
+      for (int r = lane; r < d.y; r += 32) {
+        const int s0 = rp[d.x + r] - e0, s1 = rp[d.x + r + 1] - e0;
+        TACC acc = (TACC)0;
+        for (int t = s0; t < s1; ++t) acc += scratch[t];
+        emit(d.x + r, acc);
+      }
+      __syncwarp();
+    }
+  }
+}
+
+template <typename T, typename IT, bool MULTI>
+struct Prob {  // one problem's view of the batch, as seen by one CTA of its team
   int n, m, b;
+  int nlo, nhi, mlo, mhi;             // this CTA's share of the variables / rows
   const int *A_rp, *AT_rp, *P_rp;
+  const T* Pd;                        // dense P block (global or shared) or NULL
   const T *q, *bv, *diagP, *colsq;
   double *xi, *rd, *tm, *W, *GW, *lam;
   T *r, *p, *Ap, *d, *dinv, *tA;
   double rho, alpha, sigma;
-  double* sh;
-  __device__ Prob(const BatchDev<T>& D, int b_, double* sh_) : b(b_), sh(sh_) {
+  Team<MULTI>* team;
+  const int *rpA, *rpAT, *rpP;        // local row pointers (shared memory when D.rp_smem)
+  const T *Av, *ATv, *Pv; const IT *Aci, *ATci, *Pci;   // the problem's arrays, element 0 = first element of row 0
+  double* scratch;                    // this warp's product staging (BATCH_ELEMS doubles)
+  __device__ Prob(const BatchDev<T, IT>& D, int b_, Team<MULTI>* tm_, unsigned char* dsm) : b(b_), team(tm_) {
     const int v0 = D.var_off[b], r0 = D.row_off[b];
     n = D.var_off[b + 1] - v0; m = D.row_off[b + 1] - r0;
+    team->range(n, nlo, nhi); team->range(m, mlo, mhi);
     A_rp = D.A_rp + r0; AT_rp = D.AT_rp + v0; P_rp = D.P_rp + v0;
     q = D.q + v0; bv = D.b + r0; diagP = D.diagP + v0; colsq = D.colsq + v0;
     xi = D.xi + v0; rd = D.rd + v0; lam = D.lam + v0; tm = D.tm + r0; W = D.W + r0; GW = D.GW + r0;
-    r = D.r + v0; p = D.p + v0; Ap = D.Ap + v0; d = D.d + v0; dinv = D.dinv + v0; tA = D.tA + r0;
+    Pd = D.P_dense ? D.P_v + D.P_off[b] : nullptr;
+    rpA = A_rp; rpAT = AT_rp; rpP = P_rp; scratch = nullptr;
+    if (D.batched) {
+      const int a0 = A_rp[0], t0 = AT_rp[0], p0 = P_rp[0];
+      Av = D.A_v + a0; Aci = D.A_ci + a0; ATv = D.AT_v + t0; ATci = D.AT_ci + t0; Pv = D.P_v + p0; Pci = D.P_dense ? nullptr : D.P_ci + p0;
+      scratch = reinterpret_cast<double*>(dsm) + (threadIdx.x >> 5) * BATCH_ELEMS;
+      dsm += (size_t)(blockDim.x >> 5) * BATCH_ELEMS * sizeof(double);
+      int* rpa = reinterpret_cast<int*>(dsm); dsm += (((size_t)D.mmax + 1 + 3) & ~(size_t)3) * sizeof(int);
+      int* rpat = reinterpret_cast<int*>(dsm); dsm += (((size_t)D.nmax + 1 + 3) & ~(size_t)3) * sizeof(int);
+      int* rpp = reinterpret_cast<int*>(dsm); dsm += (((size_t)D.nmax + 1 + 3) & ~(size_t)3) * sizeof(int);
+      __syncthreads();   // the previous problem's readers are done
+      for (int i = threadIdx.x; i <= m; i += blockDim.x) rpa[i] = A_rp[i] - a0;
+      for (int i = threadIdx.x; i <= n; i += blockDim.x) { rpat[i] = AT_rp[i] - t0; rpp[i] = P_rp[i] - p0; }
+      rpA = rpa; rpAT = rpat; rpP = rpp;
+    }
+    T* sv = reinterpret_cast<T*>(dsm);
+    if (D.P_smem) {   // cache the dense P of this problem (single-CTA teams only)
+      const size_t nn = (size_t)n * n;
+      __syncthreads();   // the previous problem's readers are done
+      for (size_t t = threadIdx.x; t < nn; t += blockDim.x) sv[t] = Pd[t];
+      Pd = sv; sv += (nn + 3) & ~(size_t)3;
+    }
+    if (D.vec_smem) {
+      const int ns = (n + 3) & ~3;
+      r = sv; p = r + ns; Ap = p + ns; d = Ap + ns; dinv = d + ns; tA = dinv + ns;
+    } else {
+      r = D.r + v0; p = D.p + v0; Ap = D.Ap + v0; d = D.d + v0; dinv = D.dinv + v0; tA = D.tA + r0;
+    }
+    __syncthreads();
   }
 };
 
-// Jacobi-preconditioned CG on M d = r, d0 = 0. r (T) holds the right-hand side on entry. rr0 = ||r||^2.
-// Stops when the recursive residual satisfies ||r|| <= thresh. Returns iterations.
-template <typename T>
-__device__ int pcg(const BatchDev<T>& D, const Prob<T>& c, double thresh, double rr0, int* flag) {
+// One pass over the rows of A, A^T or P owned by this CTA: warp batches (single-CTA teams) or lane groups per row.
+template <typename TACC, typename T, typename IT, bool MULTI, typename TX, typename F>
+__device__ __forceinline__ void rows_A(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const TX* x, F emit) {
+  if (D.batched) batch_rows<TACC>(D.A_bt + D.A_bo[c.b], D.A_bo[c.b + 1] - D.A_bo[c.b], c.rpA, c.Av, c.Aci, x, reinterpret_cast<TACC*>(c.scratch), emit);
+  else spmv_rows<TACC, MULTI>(c.mlo, c.mhi, c.A_rp, D.A_ci, D.A_v, x, D.A_G, emit);
+}
+template <typename TACC, typename T, typename IT, bool MULTI, typename TX, typename F>
+__device__ __forceinline__ void rows_AT(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const TX* x, F emit) {
+  if (D.batched) batch_rows<TACC>(D.AT_bt + D.AT_bo[c.b], D.AT_bo[c.b + 1] - D.AT_bo[c.b], c.rpAT, c.ATv, c.ATci, x, reinterpret_cast<TACC*>(c.scratch), emit);
+  else spmv_rows<TACC, MULTI>(c.nlo, c.nhi, c.AT_rp, D.AT_ci, D.AT_v, x, D.AT_G, emit);
+}
+template <typename TACC, typename T, typename IT, bool MULTI, typename TX, typename F>
+__device__ __forceinline__ void rows_P(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const TX* x, F emit) {
+  if (c.Pd) dense_rows<TACC, MULTI>(c.nlo, c.nhi, c.n, c.Pd, x, emit);
+  else if (D.batched) batch_rows<TACC>(D.P_bt + D.P_bo[c.b], D.P_bo[c.b + 1] - D.P_bo[c.b], c.rpP, c.Pv, c.Pci, x, reinterpret_cast<TACC*>(c.scratch), emit);
+  else spmv_rows<TACC, MULTI>(c.nlo, c.nhi, c.P_rp, D.P_ci, D.P_v, x, D.P_G, emit);
+}
+
+// q = M p for the CG: tA = rho A p ; Ap = A' tA + P p + sigma p ; returns the team-wide <p, Ap>.
+template <typename T, typename IT, bool MULTI>
+__device__ __forceinline__ double apply_M(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c) {
+  const T rhoT = (T)c.rho, sigT = (T)c.sigma;
+  rows_A<T>(D, c, c.p, [&](int row, T a) { c.tA[row] = rhoT * a; });
+  c.team->sync();
+  rows_AT<T>(D, c, c.tA, [&](int row, T a) { c.Ap[row] = a; });
+  __syncthreads();   // Ap rows are owned by this CTA
+  double pap[1] = {0.0};
+  auto fin = [&](int row, T a) {
+    const T pi = c.p[row];
+    const T ap = c.Ap[row] + a + sigT * pi;
+    c.Ap[row] = ap;
+    pap[0] += (double)pi * (double)ap;
+  };
+  rows_P<T>(D, c, c.p, fin);
+  c.team->sum(pap);
+  return pap[0];
+}
+
+// Jacobi-preconditioned CG on M d = r, d0 = 0. r (T) holds the right-hand side on entry (owner rows).
+// Stops when the recursive residual satisfies ||r|| <= thresh (reading A5). Returns iterations.
+template <typename T, typename IT, bool MULTI>
+__device__ int pcg(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, double thresh, double rr0, int* flag) {
   const int tid = threadIdx.x, nt = blockDim.x;
-  double acc[2];
-  acc[0] = 0.0;
-  for (int i = tid; i < c.n; i += nt) {
+  double acc[2] = {0.0, 0.0};
+  for (int i = c.nlo + tid; i < c.nhi; i += nt) {
     const T ri = c.r[i], z = ri * c.dinv[i];
     c.d[i] = (T)0; c.p[i] = z;
     acc[0] += (double)ri * (double)z;
   }
-  acc[1] = 0.0;
-  block_sum<2>(acc, c.sh);
+  c.team->sum(acc);          // also orders the p writes before the first A pass
   double rz = acc[0];
   const double th2 = thresh * thresh;
   int it = 0;
   if (!(rr0 > th2)) return 0;
-  const T rhoT = (T)c.rho, sigT = (T)c.sigma;
   while (it < D.maxit) {
-    spmv_rows<T>(c.m, c.A_rp, D.A_ci, D.A_v, c.p, D.A_G, [&](int row, T a) { c.tA[row] = rhoT * a; });
-    __syncthreads();
-    spmv_rows<T>(c.n, c.AT_rp, D.AT_ci, D.AT_v, c.tA, D.AT_G, [&](int row, T a) { c.Ap[row] = a; });
-    __syncthreads();
-    double pap[1] = {0.0};
-    spmv_rows<T>(c.n, c.P_rp, D.P_ci, D.P_v, c.p, D.P_G, [&](int row, T a) {
-      const T pi = c.p[row];
-      const T ap = c.Ap[row] + a + sigT * pi;
-      c.Ap[row] = ap;
-      pap[0] += (double)pi * (double)ap;
-    });
-    block_sum<1>(pap, c.sh);
-    if (!(pap[0] > 0.0)) { *flag |= FLAG_CG_CURV; break; }
-    const T a = (T)(rz / pap[0]);
+    const double pap = apply_M(D, c);
+    if (!(pap > 0.0)) { *flag |= FLAG_CG_CURV; break; }
+    const T a = (T)(rz / pap);
     acc[0] = 0.0; acc[1] = 0.0;
-    for (int i = tid; i < c.n; i += nt) {
+    for (int i = c.nlo + tid; i < c.nhi; i += nt) {
       const T pi = c.p[i];
       c.d[i] += a * pi;
       const T ri = c.r[i] - a * c.Ap[i];
@@ -122,13 +331,13 @@ __device__ int pcg(const BatchDev<T>& D, const Prob<T>& c, double thresh, double
       acc[0] += (double)ri * (double)ri;
       acc[1] += (double)ri * (double)z;
     }
-    block_sum<2>(acc, c.sh);
+    c.team->sum(acc);
     ++it;
     if (!(acc[0] > th2)) break;
     const T beta = (T)(acc[1] / rz);
     rz = acc[1];
-    for (int i = tid; i < c.n; i += nt) c.p[i] = c.r[i] * c.dinv[i] + beta * c.p[i];
-    __syncthreads();
+    for (int i = c.nlo + tid; i < c.nhi; i += nt) c.p[i] = c.r[i] * c.dinv[i] + beta * c.p[i];
+    c.team->sync();
   }
   if (it >= D.maxit) *flag |= FLAG_CG_CAP;
   return it;
@@ -136,45 +345,47 @@ __device__ int pcg(const BatchDev<T>& D, const Prob<T>& c, double thresh, double
 
 // out = M^-1 rhs with start xbase (NULL = 0): pass 0 is PCG to tol ||rhs|| on the fp64 residual of the start
 // (identical to CG started at xbase); each further pass re-evaluates the residual in fp64 and corrects
-// (iterative refinement, DESIGN.md "fp32 numerics"). Guards ||rhs|| = 0 => out = 0 (reading A5).
-template <typename T>
-__device__ int solve_M(const BatchDev<T>& D, const Prob<T>& c, const double* rhs, const double* xbase, double* out,
-                       int* flag) {
+// (iterative refinement, DESIGN.md section 6). Guards ||rhs|| = 0 => out = 0 (reading A5).
+// rhs: owner rows valid. out: every row valid team-wide on return (after a team sync).
+template <typename T, typename IT, bool MULTI>
+__device__ int solve_M(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const double* rhs, const double* xbase,
+                       double* out, int* flag) {
   const int tid = threadIdx.x, nt = blockDim.x;
   double acc[1] = {0.0};
-  for (int i = tid; i < c.n; i += nt) {
+  for (int i = c.nlo + tid; i < c.nhi; i += nt) {
     c.dinv[i] = (T)(1.0 / ((double)c.diagP[i] + c.sigma + c.rho * (double)c.colsq[i]));
     const double v = rhs[i];
     acc[0] += v * v;
     out[i] = xbase ? xbase[i] : 0.0;
   }
-  block_sum<1>(acc, c.sh);
+  c.team->sum(acc);
   const double nr2 = acc[0];
   if (!(nr2 > 0.0)) {
-    for (int i = tid; i < c.n; i += nt) out[i] = 0.0;
+    for (int i = c.nlo + tid; i < c.nhi; i += nt) out[i] = 0.0;
     if (nr2 != nr2) *flag |= FLAG_NONFINITE;
-    __syncthreads();
+    c.team->sync();
     return 0;
   }
   int total = 0;
   for (int pass = 0; pass <= D.refine; ++pass) {
     double rr0;
     if (pass == 0 && !xbase) {
-      for (int i = tid; i < c.n; i += nt) c.r[i] = (T)rhs[i];
+      for (int i = c.nlo + tid; i < c.nhi; i += nt) c.r[i] = (T)rhs[i];
       rr0 = nr2;
       __syncthreads();
     } else {  // r = rhs - M out, fp64
-      spmv_rows<double>(c.m, c.A_rp, D.A_ci, D.A_v, out, D.A_G, [&](int row, double a) { c.tm[row] = c.rho * a; });
-      __syncthreads();
-      spmv_rows<double>(c.n, c.AT_rp, D.AT_ci, D.AT_v, c.tm, D.AT_G, [&](int row, double a) { c.rd[row] = a; });
+      rows_A<double>(D, c, out, [&](int row, double a) { c.tm[row] = c.rho * a; });
+      c.team->sync();
+      rows_AT<double>(D, c, c.tm, [&](int row, double a) { c.rd[row] = a; });
       __syncthreads();
       acc[0] = 0.0;
-      spmv_rows<double>(c.n, c.P_rp, D.P_ci, D.P_v, out, D.P_G, [&](int row, double a) {
+      auto fin = [&](int row, double a) {
         const double res = rhs[row] - (c.rd[row] + a + c.sigma * out[row]);
         c.r[row] = (T)res;
         acc[0] += res * res;
-      });
-      block_sum<1>(acc, c.sh);
+      };
+      rows_P<double>(D, c, out, fin);
+      c.team->sum(acc);
       rr0 = acc[0];
     }
     double thresh = D.tol * sqrt(nr2);
@@ -185,26 +396,25 @@ __device__ int solve_M(const BatchDev<T>& D, const Prob<T>& c, const double* rhs
     const int it = pcg(D, c, thresh, rr0, flag);
     total += it;
     if (it == 0 && pass == 0 && D.refine == 0) break;
-    for (int i = tid; i < c.n; i += nt) out[i] += (double)c.d[i];
-    __syncthreads();
+    for (int i = c.nlo + tid; i < c.nhi; i += nt) out[i] += (double)c.d[i];
+    c.team->sync();
   }
+  c.team->sync();
   return total;
 }
 
 // xi and x-tilde of one step from z^k = (x, s, y): S1 + S2. Writes xt; st is produced by the caller's A pass.
-template <typename T>
-__device__ int lin_solve_step(const BatchDev<T>& D, const Prob<T>& c, const double* x, const double* s,
+template <typename T, typename IT, bool MULTI>
+__device__ int lin_solve_step(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const double* x, const double* s,
                               const double* y, double* xt, int* flag) {
   const int tid = threadIdx.x, nt = blockDim.x;
-  for (int i = tid; i < c.m; i += nt) c.tm[i] = c.rho * ((double)c.bv[i] - s[i]) - y[i];
-  __syncthreads();
-  spmv_rows<double>(c.n, c.AT_rp, D.AT_ci, D.AT_v, c.tm, D.AT_G,
-                    [&](int row, double a) { c.xi[row] = c.sigma * x[row] - (double)c.q[row] + a; });
-  __syncthreads();
+  for (int i = c.mlo + tid; i < c.mhi; i += nt) c.tm[i] = c.rho * ((double)c.bv[i] - s[i]) - y[i];
+  c.team->sync();
+  rows_AT<double>(D, c, c.tm, [&](int row, double a) { c.xi[row] = c.sigma * x[row] - (double)c.q[row] + a; });
+  c.team->sync();   // tm is reused by solve_M's residual pass
   return solve_M(D, c, c.xi, x, xt, flag);
 }
 
-// SOC projection of one cone held by a warp: w -> s+; returns branch (0 inside, 1 polar, 2 boundary), nu.
 __device__ __forceinline__ int soc_branch(double t, double nu) { return (nu <= t) ? 0 : ((nu <= -t) ? 1 : 2); }
 
 struct IterPtrs {
@@ -214,59 +424,75 @@ struct IterPtrs {
   double* ST;         // s-tilde store, size Mtot
 };
 
-template <typename T>
-__global__ void __launch_bounds__(1024) k_fwd(BatchDev<T> D, Hyper<T> H, IterPtrs I, int k) {
-  __shared__ double sh[3 * 32];
-  const int b = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
-  Prob<T> c(D, b, sh);
-  c.rho = H.rho_at(k, b); c.alpha = H.alpha_at(k, b); c.sigma = H.sigma;
-  const long long v0 = D.var_off[b], r0 = D.row_off[b];
-  const double *x = I.Zk + v0, *s = I.Zk + D.N + r0, *y = I.Zk + D.N + D.Mtot + r0;
-  double *x1 = I.Zk1 + v0, *s1 = I.Zk1 + D.N + r0, *y1 = I.Zk1 + D.N + D.Mtot + r0;
-  double *xt = I.XT + v0, *st = I.ST + r0;
-  int flag = 0;
-  const int iters = lin_solve_step(D, c, x, s, y, xt, &flag);
-  const double al = c.alpha, rho = c.rho;
-  const uint8_t* kind = D.rowkind + r0;
-  spmv_rows<double>(c.m, c.A_rp, D.A_ci, D.A_v, xt, D.A_G, [&](int row, double a) {
-    const double stv = (double)c.bv[row] - a;
-    st[row] = stv;
-    const double yv = y[row];
-    const double w = al * stv + (1.0 - al) * s[row] - yv / rho;
-    c.W[row] = w;
-    const int kd = kind[row];
-    if (kd <= KIND_NONNEG) {
-      const double sp = (kd == KIND_NONNEG && w > 0.0) ? w : 0.0;
-      s1[row] = sp;
-      y1[row] = rho * (sp - w);
+#define CDU_TEAM_PROLOGUE()                                                                   \
+  __shared__ double sh_[3 * 32];                                                               \
+  __shared__ double slots_[8];                                                                 \
+  __shared__ double bc_[4];                                                                    \
+  extern __shared__ __align__(16) unsigned char dsm_[];                                        \
+  Team<MULTI> team;                                                                            \
+  team.init(sh_, slots_, bc_);                                                                 \
+  const int nteams = (int)gridDim.x / team.C, team_id = (int)blockIdx.x / team.C;
+
+template <typename T, typename IT, bool MULTI>
+__global__ void __launch_bounds__(1024) k_fwd(BatchDev<T, IT> D, Hyper<T> H, IterPtrs I, int k) {
+  CDU_TEAM_PROLOGUE();
+  const int tid = threadIdx.x, nt = blockDim.x;
+  for (int b = team_id; b < D.B; b += nteams) {
+    Prob<T, IT, MULTI> c(D, b, &team, dsm_);
+    c.rho = H.rho_at(k, b); c.alpha = H.alpha_at(k, b); c.sigma = H.sigma;
+    const long long v0 = D.var_off[b], r0 = D.row_off[b];
+    const double *x = I.Zk + v0, *s = I.Zk + D.N + r0, *y = I.Zk + D.N + D.Mtot + r0;
+    double *x1 = I.Zk1 + v0, *s1 = I.Zk1 + D.N + r0, *y1 = I.Zk1 + D.N + D.Mtot + r0;
+    double *xt = I.XT + v0, *st = I.ST + r0;
+    int flag = 0;
+    const int iters = lin_solve_step(D, c, x, s, y, xt, &flag);
+    const double al = c.alpha, rho = c.rho;
+    const uint8_t* kind = D.rowkind + r0;
+    rows_A<double>(D, c, xt, [&](int row, double a) {
+      const double stv = (double)c.bv[row] - a;
+      st[row] = stv;
+      const double yv = y[row];
+      const double w = al * stv + (1.0 - al) * s[row] - yv / rho;
+      c.W[row] = w;
+      const int kd = kind[row];
+      if (kd <= KIND_NONNEG) {
+        const double sp = (kd == KIND_NONNEG && w > 0.0) ? w : 0.0;
+        s1[row] = sp;
+        y1[row] = rho * (sp - w);
+      }
+    });
+    for (int i = c.nlo + tid; i < c.nhi; i += nt) x1[i] = al * xt[i] + (1.0 - al) * x[i];
+    const int nsoc = D.soc_off[b + 1] - D.soc_off[b];
+    if (nsoc) {
+      team.sync();   // W complete on every row of the problem
+      // second-order cones of this problem: one warp per cone, cones dealt round-robin over the team's warps
+      const int lane = tid & 31, nw = nt >> 5, gw = team.rank * nw + (tid >> 5), wtot = team.C * nw;
+      for (int j = D.soc_off[b] + gw; j < D.soc_off[b + 1]; j += wtot) {
+        const int st0 = D.soc_start[j], dim = D.soc_dim[j];
+        const double* w = c.W + st0;
+        double nu2 = 0.0;
+        for (int i = 1 + lane; i < dim; i += 32) { const double wi = ldv<MULTI>(w + i); nu2 += wi * wi; }
+        nu2 = warp_sum(nu2);
+        const double t = ldv<MULTI>(w), nu = sqrt(nu2);
+        const int br = soc_branch(t, nu);
+        const double cf = (br == 2) ? 0.5 * (t + nu) : 0.0;
+        for (int i = lane; i < dim; i += 32) {
+          const double wi = ldv<MULTI>(w + i);
+          double sp;
+          if (br == 0) sp = wi; else if (br == 1) sp = 0.0; else sp = (i == 0) ? cf : cf * wi / nu;
+          s1[st0 + i] = sp;
+          y1[st0 + i] = rho * (sp - wi);
+        }
+      }
     }
-  });
-  for (int i = tid; i < c.n; i += nt) x1[i] = al * xt[i] + (1.0 - al) * x[i];
-  __syncthreads();
-  // second-order cones of this problem: one warp per cone
-  const int lane = tid & 31, wid = tid >> 5, nw = nt >> 5;
-  for (int j = D.soc_off[b] + wid; j < D.soc_off[b + 1]; j += nw) {
-    const int st0 = D.soc_start[j], dim = D.soc_dim[j];
-    const double* w = c.W + st0;
-    double nu2 = 0.0;
-    for (int i = 1 + lane; i < dim; i += 32) nu2 += w[i] * w[i];
-    nu2 = warp_sum(nu2);
-    const double t = w[0], nu = sqrt(nu2);
-    const int br = soc_branch(t, nu);
-    const double cf = (br == 2) ? 0.5 * (t + nu) : 0.0;
-    for (int i = lane; i < dim; i += 32) {
-      const double wi = w[i];
-      double sp;
-      if (br == 0) sp = wi; else if (br == 1) sp = 0.0; else sp = (i == 0) ? cf : cf * wi / nu;
-      s1[st0 + i] = sp;
-      y1[st0 + i] = rho * (sp - wi);
+    if (tid == 0 && team.rank == 0) {
+      D.cg_iters[b] += iters;
+      if (iters > D.cg_max[b]) D.cg_max[b] = iters;
+      if (flag) D.flags[b] |= flag;
     }
+    team.sync();   // scratch (tm, xi, CG vectors, shared memory) is reused by the team's next problem
   }
-  if (tid == 0) {
-    D.cg_iters[b] += iters;
-    if (iters > D.cg_max[b]) D.cg_max[b] = iters;
-    if (flag) D.flags[b] |= flag;
-  }
+  if (MULTI) team.sync();   // no CTA leaves while a peer may still read its shared memory
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -287,8 +513,9 @@ struct BwdPtrs {
 };
 
 // Phase 1 of the reverse step: (LEAN: re-solve), w, and B1/B2/B4 for zero, nonneg and SOC rows.
-template <typename T>
-__device__ void bwd_pre(const BatchDev<T>& D, Prob<T>& c, const BwdPtrs& Q, double* out_part, int* flag, int* iters) {
+template <typename T, typename IT, bool MULTI>
+__device__ void bwd_pre(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const BwdPtrs& Q, double* out_part, int* flag,
+                        int* iters) {
   const int b = c.b, tid = threadIdx.x, nt = blockDim.x;
   const long long v0 = D.var_off[b], r0 = D.row_off[b];
   const double *x = Q.Zk + v0, *s = Q.Zk + D.N + r0, *y = Q.Zk + D.N + D.Mtot + r0;
@@ -298,12 +525,12 @@ __device__ void bwd_pre(const BatchDev<T>& D, Prob<T>& c, const BwdPtrs& Q, doub
   const double al = c.alpha, rho = c.rho;
   if (Q.recompute) {
     *iters += lin_solve_step(D, c, x, s, y, xt, flag);
-    spmv_rows<double>(c.m, c.A_rp, D.A_ci, D.A_v, xt, D.A_G, [&](int row, double a) { st[row] = (double)c.bv[row] - a; });
+    rows_A<double>(D, c, xt, [&](int row, double a) { st[row] = (double)c.bv[row] - a; });
     __syncthreads();
   }
   const uint8_t* kind = D.rowkind + r0;
   double acc[2] = {0.0, 0.0};   // [0]: <gy, s+ - w>, [1]: <gw, y>
-  for (int i = tid; i < c.m; i += nt) {
+  for (int i = c.mlo + tid; i < c.mhi; i += nt) {
     const double yv = y[i];
     const double w = al * st[i] + (1.0 - al) * s[i] - yv / rho;
     c.W[i] = w;
@@ -317,45 +544,49 @@ __device__ void bwd_pre(const BatchDev<T>& D, Prob<T>& c, const BwdPtrs& Q, doub
       acc[1] += gw * yv;
     }
   }
-  __syncthreads();
-  const int lane = tid & 31, wid = tid >> 5, nw = nt >> 5;
-  for (int j = D.soc_off[b] + wid; j < D.soc_off[b + 1]; j += nw) {
-    const int st0 = D.soc_start[j], dim = D.soc_dim[j];
-    const double* w = c.W + st0;
-    double nu2 = 0.0, dot = 0.0;   // dot = u . G_u
-    for (int i = 1 + lane; i < dim; i += 32) {
-      const double wi = w[i];
-      nu2 += wi * wi;
-      dot += wi * (gs[st0 + i] + rho * gy[st0 + i]);
-    }
-    nu2 = warp_sum(nu2); dot = warp_sum(dot);
-    const double t = w[0], nu = sqrt(nu2);
-    const int br = soc_branch(t, nu);
-    const double Gt = gs[st0] + rho * gy[st0];
-    const double dh = (br == 2) ? dot / nu : 0.0;       // uhat . G_u
-    const double tn = (br == 2) ? t / nu : 0.0;
-    for (int i = lane; i < dim; i += 32) {
-      const double gyv = gy[st0 + i];
-      const double G = gs[st0 + i] + rho * gyv;
-      double v;
-      if (br == 0) v = G;
-      else if (br == 1) v = 0.0;
-      else if (i == 0) v = 0.5 * (Gt + dh);
-      else { const double uh = w[i] / nu; v = 0.5 * (Gt * uh + (1.0 + tn) * G - tn * dh * uh); }
-      const double gw = -rho * gyv + v;
-      c.GW[st0 + i] = gw;
-      acc[0] += gyv * (s1[st0 + i] - w[i]);
-      acc[1] += gw * y[st0 + i];
+  const int nsoc = D.soc_off[b + 1] - D.soc_off[b];
+  if (nsoc) {
+    c.team->sync();
+    const int lane = tid & 31, nw = nt >> 5, gwp = c.team->rank * nw + (tid >> 5), wtot = c.team->C * nw;
+    for (int j = D.soc_off[b] + gwp; j < D.soc_off[b + 1]; j += wtot) {
+      const int st0 = D.soc_start[j], dim = D.soc_dim[j];
+      const double* w = c.W + st0;
+      double nu2 = 0.0, dot = 0.0;   // dot = u . G_u
+      for (int i = 1 + lane; i < dim; i += 32) {
+        const double wi = ldv<MULTI>(w + i);
+        nu2 += wi * wi;
+        dot += wi * (gs[st0 + i] + rho * gy[st0 + i]);
+      }
+      nu2 = warp_sum(nu2); dot = warp_sum(dot);
+      const double t = ldv<MULTI>(w), nu = sqrt(nu2);
+      const int br = soc_branch(t, nu);
+      const double Gt = gs[st0] + rho * gy[st0];
+      const double dh = (br == 2) ? dot / nu : 0.0;       // uhat . G_u
+      const double tn = (br == 2) ? t / nu : 0.0;
+      for (int i = lane; i < dim; i += 32) {
+        const double gyv = gy[st0 + i];
+        const double G = gs[st0 + i] + rho * gyv;
+        const double wi = ldv<MULTI>(w + i);
+        double v;
+        if (br == 0) v = G;
+        else if (br == 1) v = 0.0;
+        else if (i == 0) v = 0.5 * (Gt + dh);
+        else { const double uh = wi / nu; v = 0.5 * (Gt * uh + (1.0 + tn) * G - tn * dh * uh); }
+        const double gw = -rho * gyv + v;
+        c.GW[st0 + i] = gw;
+        acc[0] += gyv * (s1[st0 + i] - wi);
+        acc[1] += gw * y[st0 + i];
+      }
     }
   }
-  block_sum<2>(acc, c.sh);
+  c.team->sum(acc);
   out_part[0] = acc[0]; out_part[1] = acc[1];
 }
 
 // Phase 2: B5-B9 with the adjoint solve; needs GW complete on every row (PSD rows written by the PSD kernels).
-template <typename T>
-__device__ void bwd_post(const BatchDev<T>& D, Prob<T>& c, const BwdPtrs& Q, const double* part, int k, int* flag,
-                         int* iters) {
+template <typename T, typename IT, bool MULTI>
+__device__ void bwd_post(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const BwdPtrs& Q, const double* part, int k,
+                         int* flag, int* iters) {
   const int b = c.b, tid = threadIdx.x, nt = blockDim.x;
   const long long v0 = D.var_off[b], r0 = D.row_off[b];
   const double *x = Q.Zk + v0, *s = Q.Zk + D.N + r0;
@@ -366,29 +597,28 @@ __device__ void bwd_post(const BatchDev<T>& D, Prob<T>& c, const BwdPtrs& Q, con
   double d_gy_sw = part[0], d_gw_y = part[1];
   for (int j = D.psdblk_off[b]; j < D.psdblk_off[b + 1]; ++j) { d_gy_sw += D.psd_part[2 * j]; d_gw_y += D.psd_part[2 * j + 1]; }
   // B6: rhs = alpha g_x+ - A'(alpha g_w)   (g_st = alpha g_w)
-  spmv_rows<double>(c.n, c.AT_rp, D.AT_ci, D.AT_v, c.GW, D.AT_G,
-                    [&](int row, double a) { c.xi[row] = al * (gx1[row] - a); });
+  rows_AT<double>(D, c, c.GW, [&](int row, double a) { c.xi[row] = al * (gx1[row] - a); });
   __syncthreads();
   // B7: adjoint solve M lam = g_xt (Eq. 5), zero start
   *iters += solve_M(D, c, c.xi, (const double*)nullptr, c.lam, flag);
   // u = A lam; B7+B9 combined: g_rho += <u, st - s> (cancellation-free form of Eq. 6 + RHS term)
   double acc[3] = {0.0, 0.0, 0.0};   // rho, alpha, sigma
-  spmv_rows<double>(c.m, c.A_rp, D.A_ci, D.A_v, c.lam, D.A_G, [&](int row, double u) {
-    const double gw = c.GW[row];
+  rows_A<double>(D, c, c.lam, [&](int row, double u) {
+    const double gw = ldv<MULTI>(c.GW + row);   // SOC rows may have been written by a peer CTA
     const double ds = st[row] - s[row];
     acc[0] += u * ds;
     acc[1] += gw * ds;                                  // B5: <g_vhat, st - s>
     gs[row] = (1.0 - al) * gw - rho * u;                // B5 + B9
     gy[row] = -gw / rho - u;                            // B4 + B9
   });
-  for (int i = tid; i < c.n; i += nt) {
+  for (int i = c.nlo + tid; i < c.nhi; i += nt) {
     const double g1 = gx1[i], l = c.lam[i], dx = xt[i] - x[i];
     acc[1] += g1 * dx;                                  // B5: <g_x+, xt - x>
     acc[2] -= l * dx;                                   // B7+B8: <lam, x - xt>
     gx[i] = (1.0 - al) * g1 + sg * l;                   // B5 + B8
   }
-  block_sum<3>(acc, c.sh);
-  if (tid == 0) {
+  c.team->sum(acc);
+  if (tid == 0 && c.team->rank == 0) {
     const size_t o = (size_t)k * D.B + b;
     Q.g_rho_pb[o] = acc[0] + d_gy_sw + d_gw_y / (rho * rho);   // B1 + B4 + (B7+B9)
     Q.g_alpha_pb[o] = acc[1];
@@ -396,26 +626,29 @@ __device__ void bwd_post(const BatchDev<T>& D, Prob<T>& c, const BwdPtrs& Q, con
   }
 }
 
-template <typename T>
-__global__ void __launch_bounds__(1024) k_bwd(BatchDev<T> D, Hyper<T> H, BwdPtrs Q, int k, int phase) {
+template <typename T, typename IT, bool MULTI>
+__global__ void __launch_bounds__(1024) k_bwd(BatchDev<T, IT> D, Hyper<T> H, BwdPtrs Q, int k, int phase) {
   // phase 0: pre + post fused (no PSD blocks anywhere); 1: pre only; 2: post only
-  __shared__ double sh[3 * 32];
-  const int b = blockIdx.x;
-  Prob<T> c(D, b, sh);
-  c.rho = H.rho_at(k, b); c.alpha = H.alpha_at(k, b); c.sigma = H.sigma;
-  int flag = 0, iters = 0;
-  double part[2];
-  if (phase != 2) {
-    bwd_pre(D, c, Q, part, &flag, &iters);
-    if (phase == 1 && threadIdx.x == 0) { Q.part_pre[2 * b] = part[0]; Q.part_pre[2 * b + 1] = part[1]; }
-  } else {
-    part[0] = Q.part_pre[2 * b]; part[1] = Q.part_pre[2 * b + 1];
+  CDU_TEAM_PROLOGUE();
+  for (int b = team_id; b < D.B; b += nteams) {
+    Prob<T, IT, MULTI> c(D, b, &team, dsm_);
+    c.rho = H.rho_at(k, b); c.alpha = H.alpha_at(k, b); c.sigma = H.sigma;
+    int flag = 0, iters = 0;
+    double part[2];
+    if (phase != 2) {
+      bwd_pre(D, c, Q, part, &flag, &iters);
+      if (phase == 1 && threadIdx.x == 0 && team.rank == 0) { Q.part_pre[2 * b] = part[0]; Q.part_pre[2 * b + 1] = part[1]; }
+    } else {
+      part[0] = Q.part_pre[2 * b]; part[1] = Q.part_pre[2 * b + 1];
+    }
+    if (phase != 1) bwd_post(D, c, Q, part, k, &flag, &iters);
+    if (threadIdx.x == 0 && team.rank == 0) {
+      D.cg_iters[b] += iters;
+      if (flag) D.flags[b] |= flag;
+    }
+    team.sync();
   }
-  if (phase != 1) bwd_post(D, c, Q, part, k, &flag, &iters);
-  if (threadIdx.x == 0) {
-    D.cg_iters[b] += iters;
-    if (flag) D.flags[b] |= flag;
-  }
+  if (MULTI) team.sync();
 }
 
 // ---- small utility kernels -------------------------------------------------------------------------------

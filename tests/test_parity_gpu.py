@@ -77,6 +77,36 @@ def test_runs_are_deterministic():
     assert np.array_equal(a["g_rho"], b["g_rho"]) and all(np.array_equal(u, v) for u, v in zip(a["xK"], b["xK"]))
 
 
+# ---- thread-block-cluster teams (several CTAs per problem) against the oracle ---------------------------------
+@pytest.mark.parametrize("dtype,team,ckpt", [("f64", 2, 0), ("f64", 4, 1), ("f32", 8, 0), ("f32", 16, 1)])
+def test_cluster_teams_all_cone_types(dtype, team, ckpt):
+    wl = _mixed_workload(dtype, seed=11, B=3, K=5, n=23,
+                         cones=((ZERO, 5), (NONNEG, 7), (SOC, 9), (PSD, 6), (SOC, 3), (PSD, 4), (NONNEG, 2)))
+    e, st = PU.check(wl, ckpt_mode=ckpt, team_size=team)
+    PU.assert_within(e, dtype)
+    assert st["flags_or"] == 0
+
+
+def test_cluster_team_equals_single_cta_on_socp():
+    wl = W.make_config(3, batch=3, p=60, K=12)
+    ref = PU.oracle_reference(wl)
+    cots = PU.full_cotangent(wl, ref)
+    a = PU.gpu_run(wl, cots, team_size=1)                 # warp row batches
+    b = PU.gpu_run(wl, cots, team_size=4)                 # cluster of 4 CTAs, direct global reads
+    c = PU.gpu_run(wl, cots, team_size=1, no_batch=1)    # single CTA, direct global reads
+    for r in (a, b, c):
+        PU.assert_within(PU.compare(wl, ref, r, False), "f32")
+
+
+def test_cfg3_full_size_without_refinement():
+    """bench.py times cfg3 with cg_refine=0: parity must hold in that configuration too."""
+    wl = W.make_config(3)
+    e, st = PU.check(wl, problems=[0, 700], per_problem=True, cg_refine=0)
+    print(wl.name, e, st)
+    PU.assert_within(e, wl.dtype)
+    assert st["flags_or"] == 0
+
+
 # ---- degenerate and edge cases ------------------------------------------------------------------------------
 def test_edge_cases_psd1_soc1_odd_order_single_step():
     cones = ((PSD, 1), (SOC, 1), (PSD, 7), (NONNEG, 1), (SOC, 2))
@@ -138,6 +168,7 @@ def test_error_codes():
 @pytest.mark.parametrize("cfg,kw", [
     (2, dict(batch=4, p=21, K=20)),
     (3, dict(batch=4, p=40, K=30)),
+    (3, dict(batch=3, p=120, K=8)),       # 14k non-zeros, long and short rows
     (4, dict(batch=3, p=16, K=30)),
     (4, dict(batch=2, p=33, K=25)),
 ])
