@@ -15,6 +15,7 @@
 #include "cdu.h"
 #include "lin.cuh"
 #include "psd_large.cuh"
+#include "psd_bjacobi.cuh"
 #include "psd_small.cuh"
 #include "gemm_tc.cuh"
 
@@ -124,7 +125,12 @@ struct PsdEngine {
   int nblk = 0, n_small = 0, n_large = 0, pmax_small = 0, pmax_large = 0;
   int* d_small_list = nullptr;
   LargeTab lt{};
-  T *G = nullptr, *Vt = nullptr, *Tm = nullptr, *T2 = nullptr, *mu = nullptr, *lamL = nullptr;
+  T *G = nullptr, *Vt = nullptr, *Tm = nullptr, *T2 = nullptr, *mu = nullptr, *lamL = nullptr, *scaleL = nullptr;
+  T* lmaxL = nullptr;            // max |lambda| per large block, from the last eigendecomposition
+  double* wprev = nullptr;       // svec of the last matrix each large block decomposed
+  int eig_impl = 1;              // 1: blocked one-sided Jacobi (orders <= 512), 0: k_hestenes everywhere
+  bool warm = false;             // Vt holds the eigenvectors of the previous call (warm start of the next one)
+  int warm_enable = 1;
   float* tc_split = nullptr;   // hi/lo operand staging of the tcgen05 path
   int* rotflags = nullptr;
   int* sweeps_max = nullptr;
@@ -162,13 +168,16 @@ struct PsdEngine {
     sweeps_sum = pool.zeros<unsigned long long>(1, st);
     if (n_large) {
       lt.nblk = n_large; lt.pmax = pmax_large;
+      std::vector<long long> soff; long long so = 0;
+      for (int q : lp) { soff.push_back(so); so += (long long)q * (q + 1) / 2; }
+      lt.soff = pool.upload(soff, st); wprev = pool.zeros<double>((size_t)so, st);
       lt.gblk = pool.upload(gblk, st); lt.moff = pool.upload(moff, st); lt.voff = pool.upload(voff, st); lt.pvec = pool.upload(lp, st);
       G = pool.alloc<T>(mo); Vt = pool.alloc<T>(mo); Tm = pool.alloc<T>(mo); T2 = pool.alloc<T>(mo);
-      mu = pool.alloc<T>(n_large); lamL = pool.alloc<T>(vo);
+      mu = pool.alloc<T>(n_large); lamL = pool.alloc<T>(vo); scaleL = pool.alloc<T>(vo); lmaxL = pool.zeros<T>(n_large, st);
       rotflags = pool.zeros<int>((size_t)n_large * HESTENES_MAXSW, st);
-      use_tc = (want_tc != 0) && std::is_same<T, float>::value && gemm_tc_supported(pmax_large) ;
-      for (int q : lp) if (!gemm_tc_supported(q)) use_tc = 0;
-      if (use_tc) tc_split = pool.alloc<float>((size_t)mo * 4);
+      use_tc = (want_tc != 0) && std::is_same<T, float>::value && gemm_tc_supported(pmax_large) ? (want_tc < 0 ? 3 : want_tc) : 0;   // bit 0: rebuild, bit 1: DK products
+      for (int q : lp) if (q != pmax_large) use_tc = 0;      // the tensor maps assume one block order
+      if (use_tc) { tc_split = pool.alloc<float>((size_t)mo * 2); tcmaps.nblk = n_large; tcmaps.p = pmax_large; }
       if (!G || !Vt || !Tm || !T2 || !mu || !lamL || !rotflags) { err = "cudaMalloc (PSD large scratch)"; return CDU_ENOMEM; }
     }
     if (pool.last != cudaSuccess) { err = std::string("PSD tables: ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
@@ -205,11 +214,6 @@ struct PsdEngine {
     return s;
   }
   cdu_status gemm_(const T* A, int ta, const T* Bm, int tb, T* C, const T* kscale, int relu, cudaStream_t st) {
-    if (use_tc) {
-      cdu_status s = gemm_tc_batched(n_large, h_large_p.data(), lt.pvec, lt.moff, lt.voff, (const float*)A, ta,
-                                     (const float*)Bm, tb, (float*)C, (const float*)kscale, relu, tc_split, st, &launches, err);
-      return s;
-    }
     const int tiles = (pmax_large + 63) / 64;
     k_gemm_fma<T><<<dim3(tiles, tiles, n_large), 256, 0, st>>>(n_large, lt.pvec, lt.moff, lt.voff, A, ta, Bm, tb, C, kscale, relu);
     ++launches;
@@ -217,7 +221,73 @@ struct PsdEngine {
     return CDU_OK;
   }
 
-  cdu_status eig_large(cudaStream_t st) {   // G (shifted) , Vt = I  ->  Vt, lamL
+  // tcgen05 path (fp32 handles, uniform block order, multiple of 128): C = A Bt' per block, see gemm_tc.cuh
+  tc::Maps tcmaps;
+  cdu_status gemm_nt(const T* A, const T* Bt, T* C, const T* lam, cudaStream_t st) {
+    pb(PC_GEMM_LARGE, st);
+    cdu_status s = tc::gemm_nt(tcmaps, (const float*)A, (const float*)Bt, (float*)C, (const float*)lam, st, err);
+    pe(st);
+    ++launches;
+    return s;
+  }
+  cdu_status tc_transpose(const T* lam, cudaStream_t st) {   // tc_split[0] = V = Vt', tc_split[1] = V diag(lam+)
+    const int p = pmax_large;
+    pb(PC_LARGE_MISC, st);
+    tc::k_tc_transpose<<<dim3(p / 32, p / 32, n_large), 256, 0, st>>>(p, (const float*)Vt, (const float*)lam, tc_split,
+                                                                     lam ? tc_split + (size_t)n_large * p * p : nullptr);
+    pe(st);
+    ++launches;
+    CU_OK(cudaGetLastError());
+    return CDU_OK;
+  }
+
+  // blocked one-sided Jacobi (psd_bjacobi.cuh): RP rows per CTA and round, cluster size chosen from what the device can co-schedule
+  template <int RP> cdu_status eig_blocked(cudaStream_t st) {
+    const int BR = RP / 2, NB = (pmax_large + BR - 1) / BR, NP = ((NB + 1) & ~1) / 2;
+    const size_t smem = bj::smem_bytes<T, RP>(pmax_large);
+    auto kern = bj::k_bjacobi<T, RP>;
+    if (bj_C == 0) {
+      CU_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      CU_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+      long long best = -1;
+      for (int C = 16; C >= 1; C >>= 1) {
+        if (C > 1 && C / 2 >= NP) continue;                // smaller cluster already covers all pairs
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(n_large * C); cfg.blockDim = dim3(bj::THREADS); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int active = 0;
+        if (cudaOccupancyMaxActiveClusters(&active, kern, &cfg) != cudaSuccess || active < 1) { cudaGetLastError(); continue; }
+        const long long cost = (long long)((n_large + active - 1) / active) * ((NP + C - 1) / C);
+        if (best < 0 || cost < best) { best = cost; bj_C = C; }
+      }
+      if (bj_C == 0) { err = "k_bjacobi: no launchable cluster size"; return CDU_ECUDA; }
+    }
+    CU_OK(cudaMemsetAsync(rotflags, 0, (size_t)n_large * bj::MAXSW * sizeof(int), st));
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(n_large * bj_C); cfg.blockDim = dim3(bj::THREADS); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = bj_C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    const double tol = std::is_same<T, float>::value ? 3e-7 : 1e-15;
+    int nl = n_large, maxsw = bj::MAXSW - 1;
+    const int* pv = lt.pvec; const long long* mo = lt.moff; const int* vo = lt.voff;
+    T *g = G, *v = Vt, *l = lamL; const T* m = mu; int* rf = rotflags; int* sw = sweeps_max; unsigned long long* ss = sweeps_sum;
+    pb(PC_EIG_LARGE, st);
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, nl, pv, mo, vo, g, v, m, l, rf, sw, ss, maxsw, tol);
+    pe(st);
+    ++launches;
+    CU_OK(e);
+    return CDU_OK;
+  }
+  int bj_C = 0;
+
+  cdu_status eig_large(cudaStream_t st) {   // G = Vt (S + mu I), Vt orthonormal (I on a cold start)  ->  Vt, lamL
+    if (eig_impl == 1 && pmax_large <= 512) {
+      if (std::is_same<T, float>::value) return eig_blocked<32>(st);
+      return eig_blocked<16>(st);
+    }
     CU_OK(cudaMemsetAsync(rotflags, 0, (size_t)n_large * HESTENES_MAXSW * sizeof(int), st));
     const int C = 8;
     cudaLaunchConfig_t cfg{};
@@ -243,6 +313,34 @@ struct PsdEngine {
     return CDU_OK;
   }
 
+  // Eigendecomposition of smat(w) for every large block. Cold: G = S + mu I, Vt = I. Warm (Vt = eigenvectors left by
+  // the previous call, nearby because consecutive ADMM iterates are): Tm = S + mu I, G = Vt Tm, so the Jacobi sweeps
+  // start from an almost orthogonal G.
+  cdu_status eig_of_w(const Hyper<T>& H, int k, const double* Wv, cudaStream_t st) {
+    const bool w = warm && warm_enable;
+    pb(PC_LARGE_MISC, st);
+    if (w) k_large_smat<T><<<n_large, 1024, 0, st>>>(tab, lt, Wv, nullptr, H, k, 0, 2, Tm, nullptr, mu, wprev, lmaxL);
+    else k_large_smat<T><<<n_large, 1024, 0, st>>>(tab, lt, Wv, nullptr, H, k, 0, 1, G, Vt, mu, wprev, lmaxL);
+    pe(st);
+    ++launches;
+    CU_OK(cudaGetLastError());
+    cdu_status s;
+    if (w) {
+      if (use_tc) s = gemm_nt(Vt, Tm, G, nullptr, st);       // Tm is symmetric: Vt Tm = Vt Tm'
+      else s = gemm(Vt, 0, Tm, 0, G, nullptr, 0, st);
+      if (s != CDU_OK) return s;
+    }
+    s = eig_large(st);
+    if (s != CDU_OK) return s;
+    pb(PC_LARGE_MISC, st);
+    k_large_post<T><<<n_large, 256, 0, st>>>(lt.pvec, lt.voff, lamL, scaleL, lmaxL);
+    pe(st);
+    ++launches;
+    CU_OK(cudaGetLastError());
+    warm = true;
+    return CDU_OK;
+  }
+
   cdu_status forward(const Hyper<T>& H, int k, const PsdFwdArgs& A, cudaStream_t st) {
     if (n_small) {
       pb(PC_PSD_FWD_SMALL, st);
@@ -252,14 +350,14 @@ struct PsdEngine {
       CU_OK(cudaGetLastError());
     }
     if (n_large) {
-      pb(PC_LARGE_MISC, st);
-      k_large_smat<T><<<n_large, 1024, 0, st>>>(tab, lt, A.W, nullptr, H, k, 0, 1, G, Vt, mu);
-      pe(st);
-      ++launches;
-      CU_OK(cudaGetLastError());
-      cdu_status s = eig_large(st);
+      cdu_status s = eig_of_w(H, k, A.W, st);
       if (s != CDU_OK) return s;
-      s = gemm(Vt, 1, Vt, 0, Tm, lamL, 1, st);          // Tm = Vt' diag(lam+) Vt
+      if (use_tc & 1) {
+        if ((s = tc_transpose(scaleL, st)) != CDU_OK) return s;
+        s = gemm_nt((const T*)(tc_split + (size_t)n_large * pmax_large * pmax_large), (const T*)tc_split, Tm, nullptr, st);   // Tm = (V diag(lam+)) V'
+      } else {
+        s = gemm(Vt, 1, Vt, 0, Tm, scaleL, 0, st);        // Tm = Vt' diag(scale) Vt
+      }
       if (s != CDU_OK) return s;
       pb(PC_LARGE_MISC, st);
       k_large_finish_fwd<T><<<dim3(64, n_large), 256, 0, st>>>(tab, lt, H, k, Tm, Vt, lamL, A);
@@ -280,12 +378,7 @@ struct PsdEngine {
     }
     if (n_large) {
       if (A.recompute) {
-        pb(PC_LARGE_MISC, st);
-      k_large_smat<T><<<n_large, 1024, 0, st>>>(tab, lt, A.W, nullptr, H, k, 0, 1, G, Vt, mu);
-      pe(st);
-        ++launches;
-        CU_OK(cudaGetLastError());
-        cdu_status s = eig_large(st);
+        cdu_status s = eig_of_w(H, k, A.W, st);
         if (s != CDU_OK) return s;
       } else {
         pb(PC_LARGE_MISC, st);
@@ -295,11 +388,25 @@ struct PsdEngine {
         CU_OK(cudaGetLastError());
       }
       pb(PC_LARGE_MISC, st);
-      k_large_smat<T><<<n_large, 1024, 0, st>>>(tab, lt, A.Gs, A.Gy, H, k, 1, 0, G, nullptr, nullptr);   // G = smat(g_s + rho g_y)
+      k_large_smat<T><<<n_large, 1024, 0, st>>>(tab, lt, A.Gs, A.Gy, H, k, 1, 0, G, nullptr, nullptr, nullptr, nullptr);   // G = smat(g_s + rho g_y)
       pe(st);
       ++launches;
       CU_OK(cudaGetLastError());
       cdu_status s;
+      if (use_tc & 2) {   // every product as A Bt' with both operands row-major: G and C o Gamma are symmetric, V = Vt'
+        const T* V = (const T*)tc_split;
+        if ((s = tc_transpose(nullptr, st)) != CDU_OK) return s;
+        if ((s = gemm_nt(Vt, G, Tm, nullptr, st)) != CDU_OK) return s;         // Tm = Vt G
+        if ((s = gemm_nt(Tm, Vt, G, lamL, st)) != CDU_OK) return s;            // C  = (Tm Vt') o Gamma   (Hadamard in the epilogue)
+        if ((s = gemm_nt(V, G, Tm, nullptr, st)) != CDU_OK) return s;          // Tm = Vt' C
+        if ((s = gemm_nt(Tm, V, G, nullptr, st)) != CDU_OK) return s;          // out = Tm Vt
+        pb(PC_LARGE_MISC, st);
+        k_large_finish_bwd<T><<<n_large, 1024, 0, st>>>(tab, lt, H, k, G, A);
+        pe(st);
+        ++launches;
+        CU_OK(cudaGetLastError());
+        return CDU_OK;
+      }
       if ((s = gemm(Vt, 0, G, 0, Tm, nullptr, 0, st)) != CDU_OK) return s;     // Tm = Vt G
       if ((s = gemm(Tm, 0, Vt, 1, G, nullptr, 0, st)) != CDU_OK) return s;     // C  = Tm Vt'
       pb(PC_LARGE_MISC, st);
@@ -708,6 +815,7 @@ cdu_status HandleT<T, IT>::forward(int K, const void* rho, int mode, double sigm
   const Hyper<T> H = hyper();
   BatchDev<T, IT> Df = D; Df.cg_iters = cg_f;
   const bool full = ckpt_mode == CDU_CKPT_FULL;
+  psd.warm = false;        // every unroll starts cold: results do not depend on the handle's history
   for (int k = 0; k < K; ++k) {
     IterPtrs I;
     I.Zk = z_at(k); I.Zk1 = z_at(k + 1);
@@ -745,6 +853,7 @@ cdu_status HandleT<T, IT>::backward(const void* gx, const void* gs, const void* 
   const Hyper<T> H = hyper();
   BatchDev<T, IT> Db = D; Db.cg_iters = cg_b;
   const bool full = ckpt_mode == CDU_CKPT_FULL;
+  psd.warm = false;
   for (int k = K - 1; k >= 0; --k) {
     BwdPtrs Q;
     Q.Zk = z_at(k); Q.Zk1 = z_at(k + 1);

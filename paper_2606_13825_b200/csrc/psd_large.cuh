@@ -22,14 +22,22 @@ struct LargeTab {
   const long long* moff; // offset of the block's p x p scratch matrices (elements)
   const int* voff;       // offset of the block's length-p scratch vectors
   const int* pvec;       // order of each large block
+  const long long* soff; // offset of the block's svec in the engine's own svec buffers
   int pmax;
 };
 
-// G = smat(v [+ scale v2]) + mu I with mu = ||smat||_F (shift = 1) or mu = 0; optionally Vt = I. One CTA per block.
+// G = smat(v [+ scale v2]) + mu I; optionally Vt = I. One CTA per block. The shift mu >= ||S||_2 makes G >= 0:
+//   shift = 0: mu = 0;   shift = 1: mu = ||S||_F (svec is an isometry, so this is ||svec||_2);
+//   shift = 2: warm call - Weyl's inequality against the previous matrix of this block, whose svec is kept in wprev
+//              and whose largest |eigenvalue| is lmax: ||S||_2 <= lmax + ||S - S_prev||_F. mu = 1.5 x that bound
+//              (capped by ||S||_F): between ADMM iterates the difference is small, so mu ~ 1.5 ||S||_2 instead of
+//              ~ sqrt(p) ||S||_2, and the rounding error of the Jacobi sweeps (eps (mu + ||S||_2)) shrinks with it.
+// shift >= 1 also refreshes wprev.
 template <typename T>
 __global__ void __launch_bounds__(1024) k_large_smat(PsdTab tab, LargeTab lt, const double* v, const double* v2,
-                                                     Hyper<T> H, int k, int use_rho_scale, int shift, T* G, T* Vt, T* mu) {
-  __shared__ double sh[32];
+                                                     Hyper<T> H, int k, int use_rho_scale, int shift, T* G, T* Vt, T* mu,
+                                                     double* wprev, const T* lmax) {
+  __shared__ double sh[64];
   const int lb = blockIdx.x, blk = lt.gblk[lb];
   const int p = tab.p[blk];
   const long long row0 = tab.row0[blk];
@@ -37,16 +45,23 @@ __global__ void __launch_bounds__(1024) k_large_smat(PsdTab tab, LargeTab lt, co
   T* g = G + lt.moff[lb];
   const double* a = v + row0;
   const double* a2 = v2 ? v2 + row0 : nullptr;
-  double acc[1] = {0.0};
+  double* wp = (wprev && shift) ? wprev + lt.soff[lb] : nullptr;
+  double acc[2] = {0.0, 0.0};
   const int nsv = p * (p + 1) / 2;
   for (int t = threadIdx.x; t < nsv; t += blockDim.x) {
     double x = a[t];
     if (a2) x += sc * a2[t];
-    acc[0] += x * x;       // svec is an isometry: ||smat||_F = ||svec||_2
+    acc[0] += x * x;
+    if (wp) { const double d = x - wp[t]; acc[1] += d * d; wp[t] = x; }
   }
-  block_sum<1>(acc, sh);
-  const double m = shift ? sqrt(acc[0]) : 0.0;
+  block_sum<2>(acc, sh);
+  double m = shift ? sqrt(acc[0]) : 0.0;
+  if (shift == 2) {
+    const double weyl = 1.5 * (1.02 * (double)lmax[lb] + sqrt(acc[1])) + 1e-30;
+    if (weyl < m) m = weyl;
+  }
   if (threadIdx.x == 0 && mu) mu[lb] = (T)m;
+  m = mu ? (double)(T)m : m;     // the value the eigenvalue pass subtracts
   for (long long t = threadIdx.x; t < (long long)p * p; t += blockDim.x) {
     const int r = (int)(t / p), c = (int)(t - (long long)r * p);
     const int idx = r <= c ? svec_idx(r, c) : svec_idx(c, r);
@@ -206,6 +221,29 @@ __global__ void k_large_hadamard(int nblk, const int* pvec, const long long* mof
   for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < (long long)p * p; t += (long long)gridDim.x * blockDim.x) {
     const int i = (int)(t / p), j = (int)(t - (long long)i * p);
     c[t] *= gamma_relu<T>(l[i], l[j]);
+  }
+}
+
+// After an eigendecomposition: scale[k] = max(lam_k, 0) (the rebuild's column scaling) and lmax = max |lam_k|
+// (the spectral radius the next warm call's shift is derived from).
+template <typename T>
+__global__ void __launch_bounds__(256) k_large_post(const int* pvec, const int* voff, const T* lam, T* scale, T* lmax) {
+  __shared__ double sh[32];
+  const int lb = blockIdx.x, p = pvec[lb];
+  const T* l = lam + voff[lb];
+  double mx = 0.0;
+  for (int i = threadIdx.x; i < p; i += blockDim.x) {
+    const T x = l[i];
+    scale[voff[lb] + i] = x > (T)0 ? x : (T)0;
+    mx = fmax(mx, fabs((double)x));
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = mx;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) mx = fmax(mx, sh[w]);
+    lmax[lb] = (T)mx;
   }
 }
 

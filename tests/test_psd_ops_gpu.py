@@ -7,8 +7,10 @@ from oracle import cones as C
 
 pytestmark = pytest.mark.gpu
 
-CASES = [("f32", 10, 1), ("f32", 50, 1), ("f32", 100, 1), ("f32", 128, 1), ("f32", 33, 2), ("f32", 140, 2), ("f32", 512, 2),
-         ("f64", 10, 1), ("f64", 51, 1), ("f64", 64, 2), ("f64", 140, 2)]
+# (dtype, order, path, tensor cores): path 1 = shared-memory Jacobi, 2 = large-block path; tc = tcgen05 3xTF32 products
+CASES = [("f32", 10, 1, 0), ("f32", 50, 1, 0), ("f32", 100, 1, 0), ("f32", 128, 1, 0), ("f32", 33, 2, 0), ("f32", 140, 2, 0),
+         ("f32", 512, 2, 0), ("f32", 128, 2, 1), ("f32", 256, 2, 1), ("f32", 512, 2, 1),
+         ("f64", 10, 1, 0), ("f64", 51, 1, 0), ("f64", 64, 2, 0), ("f64", 140, 2, 0)]
 
 
 def _sym(rng, cnt, p):
@@ -16,8 +18,8 @@ def _sym(rng, cnt, p):
     return 0.5 * (S + S.transpose(0, 2, 1))
 
 
-@pytest.mark.parametrize("dtype,p,path", CASES)
-def test_projection_and_vjp_match_oracle(dtype, p, path):
+@pytest.mark.parametrize("dtype,p,path,tc", CASES)
+def test_projection_and_vjp_match_oracle(dtype, p, path, tc):
     import torch
     import paper_2606_13825_b200 as cdu
     tdt = torch.float32 if dtype == "f32" else torch.float64
@@ -25,12 +27,12 @@ def test_projection_and_vjp_match_oracle(dtype, p, path):
     cnt = 3
     S = _sym(rng, cnt, p)
     S = S.astype(np.float32).astype(np.float64) if dtype == "f32" else S
-    Pi, U, lam = cdu.cdu_psd_project(torch.as_tensor(S, dtype=tdt, device="cuda"), path=path)
+    Pi, U, lam = cdu.cdu_psd_project(torch.as_tensor(S, dtype=tdt, device="cuda"), path=path, use_tensor_cores=tc)
     Pi, U, lam = (t.double().cpu().numpy() for t in (Pi, U, lam))
     G = _sym(rng, cnt, p)
     G = G.astype(np.float32).astype(np.float64) if dtype == "f32" else G
     Sb = cdu.cdu_psd_vjp(torch.as_tensor(U, dtype=tdt, device="cuda"), torch.as_tensor(lam, dtype=tdt, device="cuda"),
-                         torch.as_tensor(G, dtype=tdt, device="cuda"), path=path).double().cpu().numpy()
+                         torch.as_tensor(G, dtype=tdt, device="cuda"), path=path, use_tensor_cores=tc).double().cpu().numpy()
     tolp, tolv = (2e-5, 2e-4) if dtype == "f32" else (1e-12, 1e-11)
     for i in range(cnt):
         ref = C.smat(C.proj_psd(C.svec(S[i]))[0])
