@@ -126,6 +126,7 @@ struct PsdEngine {
   int* d_small_list = nullptr;
   LargeTab lt{};
   T *G = nullptr, *Vt = nullptr, *Tm = nullptr, *T2 = nullptr, *mu = nullptr, *lamL = nullptr, *scaleL = nullptr;
+  double* chunk_scr = nullptr; unsigned* chunk_tick = nullptr;   // partials / tickets of the chunked glue kernels
   T* lmaxL = nullptr;            // max |lambda| per large block, from the last eigendecomposition
   double* wprev = nullptr;       // svec of the last matrix each large block decomposed
   int eig_impl = 1;              // 1: blocked one-sided Jacobi (orders <= 512), 0: k_hestenes everywhere
@@ -174,6 +175,7 @@ struct PsdEngine {
       lt.gblk = pool.upload(gblk, st); lt.moff = pool.upload(moff, st); lt.voff = pool.upload(voff, st); lt.pvec = pool.upload(lp, st);
       G = pool.alloc<T>(mo); Vt = pool.alloc<T>(mo); Tm = pool.alloc<T>(mo); T2 = pool.alloc<T>(mo);
       mu = pool.alloc<T>(n_large); lamL = pool.alloc<T>(vo); scaleL = pool.alloc<T>(vo); lmaxL = pool.zeros<T>(n_large, st);
+      chunk_scr = pool.zeros<double>((size_t)n_large * LARGE_NCH * 2, st); chunk_tick = pool.zeros<unsigned>(n_large, st);
       rotflags = pool.zeros<int>((size_t)n_large * HESTENES_MAXSW, st);
       use_tc = (want_tc != 0) && std::is_same<T, float>::value && gemm_tc_supported(pmax_large) ? (want_tc < 0 ? 3 : want_tc) : 0;   // bit 0: rebuild, bit 1: DK products
       for (int q : lp) if (q != pmax_large) use_tc = 0;      // the tensor maps assume one block order
@@ -319,8 +321,9 @@ struct PsdEngine {
   cdu_status eig_of_w(const Hyper<T>& H, int k, const double* Wv, cudaStream_t st) {
     const bool w = warm && warm_enable;
     pb(PC_LARGE_MISC, st);
-    if (w) k_large_smat<T><<<n_large, 1024, 0, st>>>(tab, lt, Wv, nullptr, H, k, 0, 2, Tm, nullptr, mu, wprev, lmaxL);
-    else k_large_smat<T><<<n_large, 1024, 0, st>>>(tab, lt, Wv, nullptr, H, k, 0, 1, G, Vt, mu, wprev, lmaxL);
+    const bool rq = eig_impl == 1 && pmax_large <= 512;   // blocked Jacobi: eigenvalues by Rayleigh quotient afterwards
+    if (w) k_large_smat<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, Wv, nullptr, H, k, 0, 2, Tm, nullptr, mu, wprev, lmaxL, rq ? T2 : nullptr, chunk_scr, chunk_tick);
+    else k_large_smat<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, Wv, nullptr, H, k, 0, 1, G, Vt, mu, wprev, lmaxL, rq ? T2 : nullptr, chunk_scr, chunk_tick);
     pe(st);
     ++launches;
     CU_OK(cudaGetLastError());
@@ -332,6 +335,15 @@ struct PsdEngine {
     }
     s = eig_large(st);
     if (s != CDU_OK) return s;
+    if (rq) {
+      if (use_tc) s = gemm_nt(Vt, T2, G, nullptr, st);       // R = Vt S (S symmetric)
+      else s = gemm(Vt, 0, T2, 0, G, nullptr, 0, st);
+      if (s != CDU_OK) return s;
+      pb(PC_LARGE_MISC, st);
+      k_large_rayleigh<T><<<dim3(16, n_large), 256, 0, st>>>(lt.pvec, lt.moff, lt.voff, G, Vt, lamL);
+      pe(st);
+      ++launches;
+    }
     pb(PC_LARGE_MISC, st);
     k_large_post<T><<<n_large, 256, 0, st>>>(lt.pvec, lt.voff, lamL, scaleL, lmaxL);
     pe(st);
@@ -388,7 +400,7 @@ struct PsdEngine {
         CU_OK(cudaGetLastError());
       }
       pb(PC_LARGE_MISC, st);
-      k_large_smat<T><<<n_large, 1024, 0, st>>>(tab, lt, A.Gs, A.Gy, H, k, 1, 0, G, nullptr, nullptr, nullptr, nullptr);   // G = smat(g_s + rho g_y)
+      k_large_smat<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, A.Gs, A.Gy, H, k, 1, 0, G, nullptr, nullptr, nullptr, nullptr, nullptr, chunk_scr, chunk_tick);   // G = smat(g_s + rho g_y)
       pe(st);
       ++launches;
       CU_OK(cudaGetLastError());
@@ -401,7 +413,7 @@ struct PsdEngine {
         if ((s = gemm_nt(V, G, Tm, nullptr, st)) != CDU_OK) return s;          // Tm = Vt' C
         if ((s = gemm_nt(Tm, V, G, nullptr, st)) != CDU_OK) return s;          // out = Tm Vt
         pb(PC_LARGE_MISC, st);
-        k_large_finish_bwd<T><<<n_large, 1024, 0, st>>>(tab, lt, H, k, G, A);
+        k_large_finish_bwd<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, H, k, G, A, chunk_scr, chunk_tick);
         pe(st);
         ++launches;
         CU_OK(cudaGetLastError());
@@ -417,7 +429,7 @@ struct PsdEngine {
       if ((s = gemm(Vt, 1, G, 0, Tm, nullptr, 0, st)) != CDU_OK) return s;     // Tm = Vt' C
       if ((s = gemm(Tm, 0, Vt, 0, G, nullptr, 0, st)) != CDU_OK) return s;     // out = Tm Vt
       pb(PC_LARGE_MISC, st);
-      k_large_finish_bwd<T><<<n_large, 1024, 0, st>>>(tab, lt, H, k, G, A);
+      k_large_finish_bwd<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, H, k, G, A, chunk_scr, chunk_tick);
       pe(st);
       ++launches;
       CU_OK(cudaGetLastError());

@@ -34,18 +34,16 @@ template <> struct V4<double> { using type = double2; static constexpr int W = 2
 
 // shared-memory plan for RP = 2 BR rows of length p
 template <typename T, int RP> struct Plan {
-  int ldx;           // row stride of X / Y (elements); columns [p, ldx) stay zero
-  size_t off_y, off_part, off_w, off_q, off_rot, off_red, bytes;
+  int ldx;           // row stride of X (elements); columns [p, ldx) stay zero
+  size_t off_part, off_w, off_q, off_red, off_pairs, bytes;
   __host__ __device__ explicit Plan(int p) {
-    constexpr int VW = V4<T>::W;
     ldx = ((p + 3) / 4) * 4 + 4;     // multiple of 4 (16-byte rows for float), +4: rows 0..7 start in distinct bank groups
     size_t o = (size_t)RP * ldx * sizeof(T);
-    off_y = o; o += (size_t)RP * ldx * sizeof(T);
-    off_part = o; o += (size_t)KSL * RP * (RP + 1) * sizeof(T);
+    off_part = o; o += (size_t)KSL * RP * (RP + 1) * sizeof(T);   // Gram partials; later the second W buffer and Q'
     off_w = o; o += (size_t)RP * (RP + 1) * sizeof(T);
     off_q = o; o += (size_t)RP * (RP + 4) * sizeof(T);
-    off_rot = o; o += (size_t)(RP / 2) * 4 * sizeof(T);
     off_red = (o + 15) & ~(size_t)15; o = off_red + 64 * sizeof(double);
+    off_pairs = o; o += (size_t)(RP - 1) * (RP / 2) * sizeof(int);
     bytes = o;
   }
 };
@@ -161,78 +159,132 @@ __device__ __forceinline__ double gram_reduce(const T* part, T* W, double* red) 
   return mx;
 }
 
-// One cyclic sweep (RP - 1 rounds of RP / 2 disjoint rotations) of two-sided Jacobi on W; Q (RP x RP, row stride
-// RP + 4) accumulates the rotations: on exit row i of Q holds the combination of the old rows that makes new row i.
+// Rotation (sin, tau = sin / (1 + cos)) that annihilates w_ij, or the identity when |w_ij| <= thresh sqrt(w_ii w_jj).
+__device__ __forceinline__ void sweep_angle(float a, float b, float c, float thresh, float& sn, float& tau) {
+  // approximate reciprocals / square roots: they only perturb the angle and scale the row pair by 1 + O(eps s^2);
+  // eigenvalues are Rayleigh quotients taken afterwards and eigenvectors are the normalised rows, so neither matters.
+  sn = 0.f; tau = 0.f;
+  if (c * c > thresh * thresh * a * b) {
+    const float th = __fdividef(b - a, 2.f * c);
+    const float h2 = 1.f + th * th;
+    const float t = __fdividef(th >= 0.f ? 1.f : -1.f, fabsf(th) + h2 * rsqrtf(h2));
+    const float cs = rsqrtf(1.f + t * t);
+    sn = t * cs; tau = __fdividef(sn, 1.f + cs);
+  }
+}
+__device__ __forceinline__ void sweep_angle(double a, double b, double c, double thresh, double& sn, double& tau) {
+  sn = 0.0; tau = 0.0;
+  if (fabs(c) > thresh * sqrt(a * b)) {
+    const double th = (b - a) / (2.0 * c);
+    const double t = (th >= 0.0 ? 1.0 : -1.0) / (fabs(th) + sqrt(1.0 + th * th));
+    const double cs = 1.0 / sqrt(1.0 + t * t);
+    sn = t * cs; tau = sn / (1.0 + cs);
+  }
+}
+
+// One cyclic sweep (RP - 1 rounds of RP / 2 disjoint rotations) of two-sided Jacobi on W (double buffered: W0 holds
+// the matrix on entry, the result is in the buffer returned). Q (RP x RP, row stride RP + 4) accumulates the
+// rotations: row i of Q = the combination of the old rows that makes new row i. One barrier per round: warp q owns
+// row pair q; every lane derives the rotation of pair (lane mod RP/2) from the current buffer itself, the warp's own
+// rotation comes by shuffle; lanes < RP/2 update the 2 x 2 block (pair q rows, pair lane columns), all lanes the Q rows.
 template <typename T, int RP>
-__device__ __forceinline__ void inner_sweep(T* W, T* Q, T* rot, T thresh) {
+__device__ __forceinline__ T* inner_sweep(T* W0, T* W1, T* Q, T thresh, const int* pairs) {
   constexpr int H = RP / 2, LW = RP + 1, LQ = RP + 4;
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   for (int t = tid; t < RP * RP; t += blockDim.x) { const int i = t / RP, j = t - i * RP; Q[i * LQ + j] = (i == j) ? (T)1 : (T)0; }
   __syncthreads();
+  T* Wc = W0; T* Wn = W1;
   for (int r = 0; r < RP - 1; ++r) {
-    if (tid < H) {
-      int i, j; rr_pair(r, tid, RP, i, j);
-      const T a = W[i * LW + i], b = W[j * LW + j], c = W[i * LW + j];
-      T sn = (T)0, tau = (T)0;
-      if (fabs(c) > thresh * sqrt(a * b)) {
-        const T th = (b - a) / ((T)2 * c);
-        const T t = ((th >= (T)0) ? (T)1 : (T)-1) / (fabs(th) + sqrt((T)1 + th * th));
-        const T cs = (T)1 / sqrt((T)1 + t * t);
-        sn = t * cs; tau = sn / ((T)1 + cs);
+    if (warp < H) {
+      const int q2 = lane % H;
+      const int pr = pairs[r * H + q2], i2 = pr & 0xffff, j2 = pr >> 16;
+      T s2, t2;
+      sweep_angle(Wc[i2 * LW + i2], Wc[j2 * LW + j2], Wc[i2 * LW + j2], thresh, s2, t2);
+      const T s1 = __shfl_sync(0xffffffffu, s2, warp), t1 = __shfl_sync(0xffffffffu, t2, warp);
+      const int i1 = __shfl_sync(0xffffffffu, i2, warp), j1 = __shfl_sync(0xffffffffu, j2, warp);
+      if (lane < H) {
+        T a = Wc[i1 * LW + i2], b = Wc[i1 * LW + j2], c = Wc[j1 * LW + i2], d = Wc[j1 * LW + j2];
+        rot2(s1, t1, a, c); rot2(s1, t1, b, d);      // rows i1, j1
+        rot2(s2, t2, a, b); rot2(s2, t2, c, d);      // columns i2, j2
+        Wn[i1 * LW + i2] = a; Wn[i1 * LW + j2] = b; Wn[j1 * LW + i2] = c; Wn[j1 * LW + j2] = d;
       }
-      rot[2 * tid] = sn; rot[2 * tid + 1] = tau;
+      for (int col = lane; col < RP; col += 32) {
+        T x = Q[i1 * LQ + col], y = Q[j1 * LQ + col];
+        rot2(s1, t1, x, y);
+        Q[i1 * LQ + col] = x; Q[j1 * LQ + col] = y;
+      }
     }
     __syncthreads();
-    // W <- J' W J on 2 x 2 blocks (rows pair q1, columns pair q2); Q <- J' Q on row pairs
-    for (int t = tid; t < H * H; t += blockDim.x) {
-      const int q1 = t / H, q2 = t - q1 * H;
-      int i1, j1, i2, j2; rr_pair(r, q1, RP, i1, j1); rr_pair(r, q2, RP, i2, j2);
-      const T s1 = rot[2 * q1], t1 = rot[2 * q1 + 1], s2 = rot[2 * q2], t2 = rot[2 * q2 + 1];
-      T a = W[i1 * LW + i2], b = W[i1 * LW + j2], c = W[j1 * LW + i2], d = W[j1 * LW + j2];
-      rot2(s1, t1, a, c); rot2(s1, t1, b, d);      // rows i1, j1
-      rot2(s2, t2, a, b); rot2(s2, t2, c, d);      // columns i2, j2
-      W[i1 * LW + i2] = a; W[i1 * LW + j2] = b; W[j1 * LW + i2] = c; W[j1 * LW + j2] = d;
-    }
-    for (int t = tid; t < H * RP; t += blockDim.x) {
-      const int q = t / RP, col = t - q * RP;
-      int i, j; rr_pair(r, q, RP, i, j);
-      T x = Q[i * LQ + col], y = Q[j * LQ + col];
-      rot2(rot[2 * q], rot[2 * q + 1], x, y);
-      Q[i * LQ + col] = x; Q[j * LQ + col] = y;
-    }
-    __syncthreads();
+    T* tmp = Wc; Wc = Wn; Wn = tmp;
   }
+  return Wc;
 }
 
-// X <- Q X for the columns [0, p): one thread per column, Q read as broadcast vectors.
+// rows of the pair -> global: new row i = sum_k Q[i][k] X[k][:], written straight to the matrix (rows [0, BR) of the
+// pair live at rowA.., rows [BR, RP) at rowB..). Qt = Q' (row stride RP + 4). 4 x 4 register tiles.
 template <typename T, int RP>
-__device__ __forceinline__ void apply_q(const T* Q, T* X, int ldx, int p) {
-  constexpr int LQ = RP + 4;
-  for (int k = threadIdx.x; k < p; k += blockDim.x) {
-    T x[RP];
+__device__ __forceinline__ void apply_store(const T* Qt, const T* X, int ldx, int p, T* g, int rowA, int rowB) {
+  constexpr int LQ = RP + 4, NRG = RP / 4, TPT = (NRG + 3) / 4, BR = RP / 2;
+  const int cl = threadIdx.x & 127, rl = threadIdx.x >> 7;
+  const int ncg = (p + 3) >> 2;
+  for (int cgi = cl; cgi < ncg; cgi += 128) {
+    T acc[TPT][4][4];
 #pragma unroll
-    for (int j = 0; j < RP; ++j) x[j] = X[(size_t)j * ldx + k];
+    for (int u = 0; u < TPT; ++u)
+#pragma unroll
+      for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) acc[u][a][b] = (T)0;
 #pragma unroll 4
-    for (int i = 0; i < RP; ++i) {
-      T o = (T)0;
+    for (int k = 0; k < RP; ++k) {
+      T x[4];
+      load4(X + (size_t)k * ldx + 4 * cgi, x);
 #pragma unroll
-      for (int j = 0; j < RP; j += 4) {
-        T q[4];
-        load4(Q + i * LQ + j, q);
-        o += q[0] * x[j] + q[1] * x[j + 1] + q[2] * x[j + 2] + q[3] * x[j + 3];
+      for (int u = 0; u < TPT; ++u) {
+        const int rg = rl + 4 * u;
+        if (rg < NRG) {
+          T q[4];
+          load4(Qt + k * LQ + 4 * rg, q);
+#pragma unroll
+          for (int a = 0; a < 4; ++a)
+#pragma unroll
+            for (int b = 0; b < 4; ++b) acc[u][a][b] += q[a] * x[b];
+        }
       }
-      X[(size_t)i * ldx + k] = o;       // rows < i are already overwritten: x[] holds the old column
+    }
+#pragma unroll
+    for (int u = 0; u < TPT; ++u) {
+      const int rg = rl + 4 * u;
+      if (rg < NRG) {
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+          const int i = 4 * rg + a;
+          const int grow = i < BR ? rowA + i : rowB + (i - BR);
+          if (grow < p) {
+            T* dst = g + (size_t)grow * p + 4 * cgi;
+            if ((p & 3) == 0) {
+              if (sizeof(T) == 4) __stcg(reinterpret_cast<float4*>(dst), make_float4((float)acc[u][a][0], (float)acc[u][a][1], (float)acc[u][a][2], (float)acc[u][a][3]));
+              else { __stcg(reinterpret_cast<double2*>(dst), make_double2((double)acc[u][a][0], (double)acc[u][a][1])); __stcg(reinterpret_cast<double2*>(dst) + 1, make_double2((double)acc[u][a][2], (double)acc[u][a][3])); }
+            } else {
+#pragma unroll
+              for (int b = 0; b < 4; ++b) if (4 * cgi + b < p) __stcg(dst + b, acc[u][a][b]);
+            }
+          }
+        }
+      }
     }
   }
 }
 
-// One cluster per matrix; CTA `rank` takes block pairs rank, rank + C, ... of every round. G, Vt: p x p row-major,
-// row i = (S + mu I) v_i resp. v_i. rotflags[lb][sweep] is raised by any CTA that met a pair above the tolerance.
+// One cluster per matrix; CTA `rank` takes block pairs rank, rank + C, ... of every round. G: p x p row-major, row i
+// = v_i' (S + mu I) for an orthonormal set {v_i} that is never formed: a rotation of the rows of G rotates the v_i
+// with it, and once the rows are mutually orthogonal v_i = g_i / ||g_i|| and lambda_i = ||g_i|| - mu.
+// rotflags[lb][sweep] is raised by any CTA that met a pair above the tolerance.
 template <typename T, int RP>
 __global__ void __launch_bounds__(THREADS, 1)
 k_bjacobi(int nblk, const int* pvec, const long long* moff, const int* voff, T* G, T* Vt, const T* mu, T* lam, int* rotflags,
           int* sweeps_out, unsigned long long* sweeps_sum, int max_sweeps, double tol) {
-  constexpr int BR = RP / 2;
+  constexpr int BR = RP / 2, LQ = RP + 4;
   extern __shared__ __align__(16) unsigned char smem_bj[];
   cg::cluster_group cluster = cg::this_cluster();
   const int C = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
@@ -240,23 +292,25 @@ k_bjacobi(int nblk, const int* pvec, const long long* moff, const int* voff, T* 
   const int p = pvec[lb];
   const Plan<T, RP> pl(p);
   T* X = reinterpret_cast<T*>(smem_bj);
-  T* Y = reinterpret_cast<T*>(smem_bj + pl.off_y);
   T* part = reinterpret_cast<T*>(smem_bj + pl.off_part);
   T* W = reinterpret_cast<T*>(smem_bj + pl.off_w);
   T* Q = reinterpret_cast<T*>(smem_bj + pl.off_q);
-  T* rot = reinterpret_cast<T*>(smem_bj + pl.off_rot);
+  T* W1 = part;                                  // free once gram_reduce has consumed the partials
+  T* Qt = part + RP * (RP + 1) + 3;              // 16-byte aligned below
+  Qt = reinterpret_cast<T*>((reinterpret_cast<uintptr_t>(Qt)) & ~(uintptr_t)15);
   double* red = reinterpret_cast<double*>(smem_bj + pl.off_red);
   T* g = G + moff[lb];
-  T* vt = Vt + moff[lb];
   int* rf = rotflags + lb * MAXSW;
   const int ldx = pl.ldx;
   const int NB = (p + BR - 1) / BR, NBe = (NB + 1) & ~1, NP = NBe >> 1;
-  for (int t = threadIdx.x; t < 2 * RP * ldx; t += blockDim.x) X[t] = (T)0;    // X and Y are contiguous; pads stay zero
+  int* pairs = reinterpret_cast<int*>(smem_bj + pl.off_pairs);              // pair (i | j << 16) of round r, table q
+  for (int t = threadIdx.x; t < (RP - 1) * BR; t += blockDim.x) { int i, j; rr_pair(t / BR, t % BR, RP, i, j); pairs[t] = i | (j << 16); }
+  for (int t = threadIdx.x; t < RP * ldx; t += blockDim.x) X[t] = (T)0;    // the pads stay zero
   __syncthreads();
   const T thresh = (T)(0.25 * tol);
   int sweep = 0;
   for (; sweep < max_sweeps; ++sweep) {
-    for (int r = 0; r < NBe - 1 || (NBe == 2 && r == 0); ++r) {
+    for (int r = 0; r < NBe - 1; ++r) {
       for (int q = rank; q < NP; q += C) {
         int bi, bj2; rr_pair(r, q, NBe, bi, bj2);
         load_rows<T, BR>(g, p, bi * BR, X, ldx, 0);
@@ -266,41 +320,31 @@ k_bjacobi(int nblk, const int* pvec, const long long* moff, const int* voff, T* 
         __syncthreads();
         const double mx = gram_reduce<T, RP>(part, W, red);
         if (mx > tol) {
-          load_rows<T, BR>(vt, p, bi * BR, Y, ldx, 0);          // in flight while the sweep runs
-          load_rows<T, BR>(vt, p, bj2 * BR, Y, ldx, BR);
-          inner_sweep<T, RP>(W, Q, rot, thresh);
-          apply_q<T, RP>(Q, X, ldx, p);
-          apply_q<T, RP>(Q, Y, ldx, p);
+          const T* Wf = inner_sweep<T, RP>(W, W1, Q, thresh, pairs);
+          (void)Wf;
+          for (int t = threadIdx.x; t < RP * RP; t += blockDim.x) { const int i = t / RP, k = t - i * RP; Qt[k * LQ + i] = Q[i * LQ + k]; }
           __syncthreads();
-          store_rows<T, BR>(g, p, bi * BR, X, ldx, 0);
-          store_rows<T, BR>(g, p, bj2 * BR, X, ldx, BR);
-          store_rows<T, BR>(vt, p, bi * BR, Y, ldx, 0);
-          store_rows<T, BR>(vt, p, bj2 * BR, Y, ldx, BR);
+          apply_store<T, RP>(Qt, X, ldx, p, g, bi * BR, bj2 * BR);
           if (threadIdx.x == 0) __stcg(rf + sweep, 1);
         }
         __syncthreads();
       }
       cluster.sync();
-      if (NBe == 2) break;
     }
     if (!__ldcg(rf + sweep)) break;
   }
-  // eigenvalues; Vt <- normalised rows of G
+  // eigenvalues and eigenvectors
   const int lane = threadIdx.x & 31, nw = blockDim.x >> 5;
   const double m = (double)mu[lb];
+  T* vt = Vt + moff[lb];
   for (int i = rank * nw + (threadIdx.x >> 5); i < p; i += C * nw) {
-    double a = 0.0, b = 0.0;
-    for (int c = lane; c < p; c += 32) {
-      const double x = (double)ld_cg(g + (size_t)i * p + c), y = (double)ld_cg(vt + (size_t)i * p + c);
-      a += x * x; b += y * y;
-    }
-    a = warp_sum(a); b = warp_sum(b);
+    double a = 0.0;
+    for (int c = lane; c < p; c += 32) { const double x = (double)ld_cg(g + (size_t)i * p + c); a += x * x; }
+    a = warp_sum(a);
     const double na = sqrt(a);
-    if (lane == 0) lam[voff[lb] + i] = (T)((b > 0.0 ? na / sqrt(b) : 0.0) - m);
-    if (na > 0.0) {
-      const double inv = 1.0 / na;
-      for (int c = lane; c < p; c += 32) vt[(size_t)i * p + c] = (T)((double)ld_cg(g + (size_t)i * p + c) * inv);
-    }
+    if (lane == 0) lam[voff[lb] + i] = (T)(na - m);
+    const double inv = na > 0.0 ? 1.0 / na : 0.0;
+    for (int c = lane; c < p; c += 32) vt[(size_t)i * p + c] = (T)((double)ld_cg(g + (size_t)i * p + c) * inv);
   }
   if (rank == 0 && threadIdx.x == 0) { atomicMax(sweeps_out, sweep); if (sweeps_sum) atomicAdd(sweeps_sum, (unsigned long long)sweep); }
 }

@@ -26,19 +26,25 @@ struct LargeTab {
   int pmax;
 };
 
-// G = smat(v [+ scale v2]) + mu I; optionally Vt = I. One CTA per block. The shift mu >= ||S||_2 makes G >= 0:
+// G = smat(v [+ scale v2]) + mu I; optionally Vt = I and an unshifted copy. The shift mu >= ||S||_2 makes G >= 0:
 //   shift = 0: mu = 0;   shift = 1: mu = ||S||_F (svec is an isometry, so this is ||svec||_2);
 //   shift = 2: warm call - Weyl's inequality against the previous matrix of this block, whose svec is kept in wprev
 //              and whose largest |eigenvalue| is lmax: ||S||_2 <= lmax + ||S - S_prev||_F. mu = 1.5 x that bound
 //              (capped by ||S||_F): between ADMM iterates the difference is small, so mu ~ 1.5 ||S||_2 instead of
 //              ~ sqrt(p) ||S||_2, and the rounding error of the Jacobi sweeps (eps (mu + ||S||_2)) shrinks with it.
 // shift >= 1 also refreshes wprev.
+constexpr int LARGE_NCH = 32;   // CTAs per block in the chunked glue kernels
+
+// Chunked over gridDim.x CTAs per block (blockIdx.y = block). The reductions (||svec||^2, ||svec - wprev||^2) go
+// through per-chunk partials in `scr` ([nblk][LARGE_NCH][2] doubles + one ticket per block in `tick`); the last CTA
+// to finish sums them in chunk order (deterministic), sets mu and adds it to the diagonal.
 template <typename T>
-__global__ void __launch_bounds__(1024) k_large_smat(PsdTab tab, LargeTab lt, const double* v, const double* v2,
-                                                     Hyper<T> H, int k, int use_rho_scale, int shift, T* G, T* Vt, T* mu,
-                                                     double* wprev, const T* lmax) {
+__global__ void __launch_bounds__(256) k_large_smat(PsdTab tab, LargeTab lt, const double* v, const double* v2,
+                                                    Hyper<T> H, int k, int use_rho_scale, int shift, T* G, T* Vt, T* mu,
+                                                    double* wprev, const T* lmax, T* Splain, double* scr, unsigned* tick) {
   __shared__ double sh[64];
-  const int lb = blockIdx.x, blk = lt.gblk[lb];
+  __shared__ unsigned last;
+  const int lb = blockIdx.y, blk = lt.gblk[lb], nch = gridDim.x, ch = blockIdx.x;
   const int p = tab.p[blk];
   const long long row0 = tab.row0[blk];
   const double sc = use_rho_scale ? H.rho_at(k, tab.prob[blk]) : 0.0;
@@ -46,29 +52,76 @@ __global__ void __launch_bounds__(1024) k_large_smat(PsdTab tab, LargeTab lt, co
   const double* a = v + row0;
   const double* a2 = v2 ? v2 + row0 : nullptr;
   double* wp = (wprev && shift) ? wprev + lt.soff[lb] : nullptr;
+  // 32 x 32 tiles of the lower triangle (tile row bi >= tile column bj): the svec entries of matrix row R, columns
+  // Cc <= R are contiguous (idx = R (R + 1) / 2 + Cc), so reads are coalesced along Cc; the tile and its mirror image
+  // are written from shared memory, both coalesced.
+  __shared__ T tile[32][33];
+  const int ntr = (p + 31) >> 5, ntiles = ntr * (ntr + 1) / 2;
+  const int lane = threadIdx.x & 31, wy = threadIdx.x >> 5, nwy = blockDim.x >> 5;
   double acc[2] = {0.0, 0.0};
-  const int nsv = p * (p + 1) / 2;
-  for (int t = threadIdx.x; t < nsv; t += blockDim.x) {
-    double x = a[t];
-    if (a2) x += sc * a2[t];
-    acc[0] += x * x;
-    if (wp) { const double d = x - wp[t]; acc[1] += d * d; wp[t] = x; }
+  for (int tl = ch; tl < ntiles; tl += nch) {
+    int bi = (int)((sqrt(8.0 * tl + 1.0) - 1.0) * 0.5);
+    while (bi * (bi + 1) / 2 > tl) --bi;
+    while ((bi + 1) * (bi + 2) / 2 <= tl) ++bi;
+    const int bj = tl - bi * (bi + 1) / 2;
+    const int Cc = bj * 32 + lane;
+    for (int rr = wy; rr < 32; rr += nwy) {
+      const int R = bi * 32 + rr;
+      T val = (T)0;
+      if (R < p && Cc < p && Cc <= R) {
+        const int idx = svec_idx(Cc, R);
+        double x = a[idx];
+        if (a2) x += sc * a2[idx];
+        acc[0] += x * x;
+        if (wp) { const double d = x - wp[idx]; acc[1] += d * d; wp[idx] = x; }
+        val = (T)(R == Cc ? x : x * 0.70710678118654752440);
+      }
+      tile[rr][lane] = val;
+    }
+    __syncthreads();
+    for (int rr = wy; rr < 32; rr += nwy) {
+      const int R = bi * 32 + rr;
+      if (R < p && Cc < p && (bi != bj || lane <= rr)) {
+        const long long t = (long long)R * p + Cc;
+        const T val = tile[rr][lane];
+        g[t] = val;
+        if (Splain) Splain[lt.moff[lb] + t] = val;
+        if (Vt) Vt[lt.moff[lb] + t] = (R == Cc) ? (T)1 : (T)0;
+      }
+      // mirror image: element (row Cm, column Rm) = tile[lane][rr] with Rm = bi * 32 + lane, Cm = bj * 32 + rr
+      const int Rm = bi * 32 + lane, Cm = bj * 32 + rr;
+      if (Rm < p && Cm < p && (bi != bj ? true : rr < lane)) {
+        const long long t = (long long)Cm * p + Rm;
+        const T val = tile[lane][rr];
+        g[t] = val;
+        if (Splain) Splain[lt.moff[lb] + t] = val;
+        if (Vt) Vt[lt.moff[lb] + t] = (T)0;
+      }
+    }
+    __syncthreads();
   }
+  if (!shift) return;
   block_sum<2>(acc, sh);
-  double m = shift ? sqrt(acc[0]) : 0.0;
+  if (threadIdx.x == 0) {
+    scr[((size_t)lb * LARGE_NCH + ch) * 2] = acc[0]; scr[((size_t)lb * LARGE_NCH + ch) * 2 + 1] = acc[1];
+    __threadfence();
+    last = (atomicAdd(tick + lb, 1u) == (unsigned)nch - 1) ? 1u : 0u;
+  }
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  double n2 = 0.0, d2 = 0.0;
+  for (int c = 0; c < nch; ++c) { n2 += __ldcg(scr + ((size_t)lb * LARGE_NCH + c) * 2); d2 += __ldcg(scr + ((size_t)lb * LARGE_NCH + c) * 2 + 1); }
+  double m = sqrt(n2);
   if (shift == 2) {
-    const double weyl = 1.5 * (1.02 * (double)lmax[lb] + sqrt(acc[1])) + 1e-30;
+    const double weyl = 1.5 * (1.02 * (double)lmax[lb] + sqrt(d2)) + 1e-30;
     if (weyl < m) m = weyl;
   }
-  if (threadIdx.x == 0 && mu) mu[lb] = (T)m;
-  m = mu ? (double)(T)m : m;     // the value the eigenvalue pass subtracts
-  for (long long t = threadIdx.x; t < (long long)p * p; t += blockDim.x) {
-    const int r = (int)(t / p), c = (int)(t - (long long)r * p);
-    const int idx = r <= c ? svec_idx(r, c) : svec_idx(c, r);
-    double x = a[idx];
-    if (a2) x += sc * a2[idx];
-    g[t] = (T)(r == c ? x + m : x * 0.70710678118654752440);
-    if (Vt) Vt[lt.moff[lb] + t] = (r == c) ? (T)1 : (T)0;
+  const T mT = (T)m;
+  if (threadIdx.x == 0) { if (mu) mu[lb] = mT; tick[lb] = 0; }
+  for (int i = threadIdx.x; i < p; i += blockDim.x) {
+    T* d = g + (long long)i * p + i;
+    *d = (T)((double)__ldcg(d) + (double)mT);
   }
 }
 
@@ -224,6 +277,23 @@ __global__ void k_large_hadamard(int nblk, const int* pvec, const long long* mof
   }
 }
 
+// lam_i = <R_i, v_i> / <v_i, v_i> with R = Vt S (rows): Rayleigh quotients against the UNSHIFTED matrix, so the
+// eigenvalues carry an error of eps ||S||, not eps mu, and do not see how the sweeps scaled the rows of G.
+template <typename T>
+__global__ void __launch_bounds__(256) k_large_rayleigh(const int* pvec, const long long* moff, const int* voff, const T* R,
+                                                        const T* Vt, T* lam) {
+  const int lb = blockIdx.y, p = pvec[lb];
+  const int lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+  const T* r = R + moff[lb];
+  const T* v = Vt + moff[lb];
+  for (int i = blockIdx.x * nw + (threadIdx.x >> 5); i < p; i += gridDim.x * nw) {
+    double a = 0.0, b = 0.0;
+    for (int c = lane; c < p; c += 32) { const double x = (double)v[(long long)i * p + c]; a += (double)r[(long long)i * p + c] * x; b += x * x; }
+    a = warp_sum(a); b = warp_sum(b);
+    if (lane == 0) lam[voff[lb] + i] = (T)(b > 0.0 ? a / b : 0.0);
+  }
+}
+
 // After an eigendecomposition: scale[k] = max(lam_k, 0) (the rebuild's column scaling) and lmax = max |lam_k|
 // (the spectral radius the next warm call's shift is derived from).
 template <typename T>
@@ -286,12 +356,14 @@ __global__ void k_large_fetch(PsdTab tab, LargeTab lt, const T* Ustore, const T*
   for (long long t = t0; t < p; t += stride) lam[lt.voff[lb] + t] = L[t];
 }
 
-// g_w = -rho g_y + svec(Out); partial dots for g_rho.
+// g_w = -rho g_y + svec(Out); partial dots for g_rho. Chunked like k_large_smat; the last CTA of a block sums the
+// chunk partials in order into A.part.
 template <typename T>
-__global__ void __launch_bounds__(1024) k_large_finish_bwd(PsdTab tab, LargeTab lt, Hyper<T> H, int k, const T* Out,
-                                                           PsdBwdArgs A) {
+__global__ void __launch_bounds__(256) k_large_finish_bwd(PsdTab tab, LargeTab lt, Hyper<T> H, int k, const T* Out,
+                                                          PsdBwdArgs A, double* scr, unsigned* tick) {
   __shared__ double sh[64];
-  const int lb = blockIdx.x, blk = lt.gblk[lb];
+  __shared__ unsigned last;
+  const int lb = blockIdx.y, blk = lt.gblk[lb], nch = gridDim.x, ch = blockIdx.x;
   const int p = tab.p[blk];
   const long long row0 = tab.row0[blk];
   const double rho = H.rho_at(k, tab.prob[blk]);
@@ -299,7 +371,9 @@ __global__ void __launch_bounds__(1024) k_large_finish_bwd(PsdTab tab, LargeTab 
   const double *w = A.W + row0, *yk = A.Yk + row0, *s1 = A.S1 + row0, *gy = A.Gy + row0;
   double* gw = A.GW + row0;
   double acc[2] = {0.0, 0.0};
-  for (long long t = threadIdx.x; t < (long long)p * p; t += blockDim.x) {
+  const long long tot = (long long)p * p;
+  const long long t0 = tot * ch / nch, t1 = tot * (ch + 1) / nch;
+  for (long long t = t0 + threadIdx.x; t < t1; t += blockDim.x) {
     const int r = (int)(t / p), c = (int)(t - (long long)r * p);
     if (r <= c) {
       const double ov = (r == c) ? (double)o[t] : 0.5 * ((double)o[t] + (double)o[(long long)c * p + r]) * 1.41421356237309504880;
@@ -312,7 +386,18 @@ __global__ void __launch_bounds__(1024) k_large_finish_bwd(PsdTab tab, LargeTab 
     }
   }
   block_sum<2>(acc, sh);
-  if (threadIdx.x == 0) { A.part[2 * blk] = acc[0]; A.part[2 * blk + 1] = acc[1]; }
+  if (threadIdx.x == 0) {
+    scr[((size_t)lb * LARGE_NCH + ch) * 2] = acc[0]; scr[((size_t)lb * LARGE_NCH + ch) * 2 + 1] = acc[1];
+    __threadfence();
+    last = (atomicAdd(tick + lb, 1u) == (unsigned)nch - 1) ? 1u : 0u;
+  }
+  __syncthreads();
+  if (!last || threadIdx.x != 0) return;
+  __threadfence();
+  double p0 = 0.0, p1 = 0.0;
+  for (int c = 0; c < nch; ++c) { p0 += __ldcg(scr + ((size_t)lb * LARGE_NCH + c) * 2); p1 += __ldcg(scr + ((size_t)lb * LARGE_NCH + c) * 2 + 1); }
+  A.part[2 * blk] = p0; A.part[2 * blk + 1] = p1;
+  tick[lb] = 0;
 }
 
 }  // namespace cdu
