@@ -841,6 +841,7 @@ cdu_status HandleT<T, IT>::forward(int K, const void* rho, int mode, double sigm
       PsdFwdArgs A;
       A.W = D.W; A.S1 = z_at(k + 1) + N; A.Y1 = z_at(k + 1) + N + Mtot;
       A.Ustore = Ustore + (full ? (size_t)k * psd.sum_p2 : 0); A.Lstore = Lstore + (full ? (size_t)k * psd.sum_p : 0);
+      A.Uprev = (k > 0 && psd.warm_enable) ? (const void*)(Ustore + (full ? (size_t)(k - 1) * psd.sum_p2 : 0)) : nullptr;
       A.sweeps_max = psd.sweeps_max; A.flags = flags; A.sweeps_sum = psd.sweeps_sum;
       s = psd.forward(H, k, A, st);
       if (s != CDU_OK) { err = psd.err; return s; }
@@ -1026,7 +1027,7 @@ cdu_status psd_op_t(bool vjp, int count, int p, const void* in1, const void* in2
   Hyper<T> H; H.rho = d_one; H.alpha = d_one; H.kstride = 0; H.pstride = 0; H.sigma = 1.0;
   if (!vjp) {
     k_dense_to_svec<T><<<count, 256, 0, st>>>(p, (const T*)in1, W);
-    PsdFwdArgs A; A.W = W; A.S1 = S1; A.Y1 = Y1; A.Ustore = Us; A.Lstore = Ls; A.sweeps_max = eng.sweeps_max; A.flags = flags; A.sweeps_sum = eng.sweeps_sum;
+    PsdFwdArgs A; A.W = W; A.S1 = S1; A.Y1 = Y1; A.Ustore = Us; A.Lstore = Ls; A.Uprev = nullptr; A.sweeps_max = eng.sweeps_max; A.flags = flags; A.sweeps_sum = eng.sweeps_sum;
     s = eng.forward(H, 0, A, st);
     if (s != CDU_OK) { err = eng.err; return s; }
     k_svec_to_dense<T><<<count, 256, 0, st>>>(p, S1, (T*)out1);

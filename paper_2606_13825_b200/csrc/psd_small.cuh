@@ -154,13 +154,15 @@ inline int jacobi_need(int pe, size_t sz) {
 // plr0[*cur_out * pe + pos] = player whose eigenvalue sits on the diagonal at pos, Vt[player][:] = its eigenvector.
 // blockDim.x = work threads + JACOBI_ANGLE_THREADS; every thread of the CTA must call.
 template <typename T, int MAXI>
-__device__ int jacobi_planes(int pe, const JacobiWs<T>& w, double* shred, int max_sweeps, int* flag, int* cur_out) {
+__device__ int jacobi_planes(int pe, const JacobiWs<T>& w, double* shred, int max_sweeps, int* flag, int* cur_out,
+                             bool keep_vt = false) {
   using V4 = typename VecT<T>::type;
   constexpr int VW = VecT<T>::W;
   const int tid = threadIdx.x, nt = blockDim.x, ntw = nt - JACOBI_ANGLE_THREADS;
   const int h = pe >> 1, ldh = h | 1, psz = h * ldh, ldv = w.ldv, nblk = h * (h + 1) / 2, nvc = ldv / VW, nvit = h * nvc;
   // ---- one-time set-up ----
-  for (int t = tid; t < pe * ldv; t += nt) { const int i = t / ldv, a = t - i * ldv; w.Vt[t] = (i == a) ? (T)1 : (T)0; }
+  if (!keep_vt)   // warm start: Vt already holds an orthonormal basis in which the matrix was expressed
+    for (int t = tid; t < pe * ldv; t += nt) { const int i = t / ldv, a = t - i * ldv; w.Vt[t] = (i == a) ? (T)1 : (T)0; }
   for (int pos = tid; pos < pe; pos += nt) w.plr0[pos] = pos;
   double acc[1] = {0.0};
   for (int t = tid; t < 4 * psz; t += nt) {
@@ -348,6 +350,7 @@ struct PsdFwdArgs {
   double* Y1;        // y^{k+1} base (rows)
   void* Ustore;      // eigenvector store of this iteration (or scratch)
   void* Lstore;
+  const void* Uprev; // eigenvectors of the previous iterate (same layout as Ustore) or NULL: warm start
   int* sweeps_max; int* flags;
   unsigned long long* sweeps_sum;   // total Jacobi sweeps over blocks (statistics for the ALU roofline)
 };
@@ -364,12 +367,36 @@ __global__ void __launch_bounds__(psd_small_max_threads(MAXI)) k_psd_fwd_small(P
   T* lp = reinterpret_cast<T*>(smem_raw + 512 + jacobi_ws_bytes<T>(pe));   // pe: max(lambda, 0) by player
   const double rho = H.rho_at(k, prob);
   const double* w = A.W + row0;
-  load_smat_planes<T>(p, pe, ws.P0, w, 0.0, nullptr);
-  __syncthreads();
-  int flag = 0, cur = 0;
-  const int sweeps = jacobi_planes<T, MAXI>(pe, ws, shred, 40, &flag, &cur);
   const int ldv = ws.ldv;
   const int h = pe >> 1, ldh = h | 1, psz = h * ldh;
+  const bool warmst = A.Uprev != nullptr;
+  if (warmst) {
+    // Warm start: consecutive ADMM iterates have nearby eigenbases, so S is first expressed in the previous
+    // iterate's basis, A' = U' S U (two shared-memory products), which leaves it almost diagonal; the sweeps then
+    // rotate that basis (Vt keeps U instead of the identity) and 2-3 of them suffice instead of 6-8.
+    const T* Up = reinterpret_cast<const T*>(A.Uprev) + tab.uoff[blk];
+    T* Tm = ws.P0;                    // buffer 0: S U
+    T* Sd = ws.P0 + ws.pstride;       // buffer 1: S, then A'
+    for (int t = threadIdx.x; t < pe * ldv; t += blockDim.x) {
+      const int i = t / ldv, a = t - i * ldv;
+      ws.Vt[t] = (i < p && a < p) ? Up[i * p + a] : ((i == a) ? (T)1 : (T)0);
+    }
+    load_smat<T>(p, pe, pe, Sd, w, 0.0, nullptr);
+    __syncthreads();
+    smem_gemm<T>(pe, Sd, pe, 1, ws.Vt, 1, ldv, Tm, pe);        // Tm(a,i) = sum_b S(a,b) U(b,i)
+    __syncthreads();
+    smem_gemm<T>(pe, ws.Vt, ldv, 1, Tm, pe, 1, Sd, pe);        // A'(i,j) = sum_a U(a,i) Tm(a,j)
+    __syncthreads();
+    for (int t = threadIdx.x; t < pe * pe; t += blockDim.x) {
+      const int b = t / pe, a = t - b * pe;
+      ws.P0[seat_offset(a, b, psz, ldh)] = (T)0.5 * (Sd[a * pe + b] + Sd[b * pe + a]);
+    }
+  } else {
+    load_smat_planes<T>(p, pe, ws.P0, w, 0.0, nullptr);
+  }
+  __syncthreads();
+  int flag = 0, cur = 0;
+  const int sweeps = jacobi_planes<T, MAXI>(pe, ws, shred, 40, &flag, &cur, warmst);
   T* U = reinterpret_cast<T*>(A.Ustore) + tab.uoff[blk];   // rows = eigenvectors
   T* L = reinterpret_cast<T*>(A.Lstore) + tab.loff[blk];
   for (int pos = threadIdx.x; pos < pe; pos += blockDim.x) {
