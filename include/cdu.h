@@ -75,8 +75,9 @@ typedef struct {
   double  cg_refine_tol;    /* each refinement pass reduces the true residual by this factor; <= 0: 1e-4        */
   int32_t psd_small_max;    /* PSD blocks of order <= this run in the shared-memory Jacobi kernel, larger ones in
                                the global-memory path; <= 0: default (128 for F32, 88 for F64)                  */
-  int32_t use_tensor_cores; /* large-block rebuild / DK products: 1 = tcgen05 3xTF32 GEMM, 0 = fp32 FMA GEMM;
-                               < 0: default                                                                     */
+  int32_t use_tensor_cores; /* large-block products on tcgen05 (3xTF32, fp32 handles, block order a multiple of 128):
+                               bit 0 = rebuild U max(L,0) U', bit 1 = the four Dalecki-Krein products; 0 = fp32 FMA
+                               GEMM for both; < 0: default (3)                                                  */
   int32_t team_size;        /* CTAs (thread-block cluster size, power of two <= 16) that share one problem in the
                                linear-step kernels; <= 0: chosen from the batch size and the problem size         */
   int32_t no_batch;         /* 1: single-CTA teams read rows with lane groups straight from global memory instead of

@@ -1,21 +1,24 @@
 // psd_bjacobi.cuh - eigendecomposition of the large PSD blocks: blocked one-sided Jacobi in shared memory.
 //
-// Same fixed point as k_hestenes (psd_large.cuh): the rows g_i = (S + mu I) v_i of G are made mutually orthogonal by
-// plane rotations applied to (G, Vt) alike; then v_i are eigenvectors of S and lambda_i = ||g_i|| / ||v_i|| - mu
-// (Eq. 7: only U max(L,0) U' is compared with the oracle, never U - reading A15). What changes is
-// the schedule, which is built for the SM instead of for L2 latency:
+// Same fixed point as k_hestenes (psd_large.cuh): the rows g_i = v_i' (S + mu I) of G, for an orthonormal set {v_i},
+// are made mutually orthogonal by plane rotations; then v_i = g_i / ||g_i|| are eigenvectors of S (Eq. 7,
+// L102: only U max(L,0) U' is compared with the oracle, never U - reading A15). The v_i are never formed: rotating
+// the rows of G rotates them implicitly, so only G is carried. What changes against k_hestenes is the schedule,
+// built for the SM instead of for L2 latency:
 //   * rows are grouped in blocks of BR; one round of a round-robin tournament over the NB blocks pairs every block
 //     with one other, and one CTA of the matrix's thread-block cluster takes one pair: it brings the 2 BR rows of G
-//     and of Vt (2 BR x p each) into shared memory, forms their Gram matrix W = X X' (2 BR x 2 BR, register-tiled,
-//     k split over 8 thread groups), runs ONE cyclic sweep of two-sided Jacobi on W in shared memory (rotation
-//     threshold relative to sqrt(w_ii w_jj), de Rijk), accumulating the rotations in Q, and applies Q to both row
-//     sets (X <- Q X, Y <- Q Y; one thread per column, Q broadcast from shared memory). Rows go back to L2 and the
-//     cluster meets at one barrier per ROUND OF BLOCKS (NB - 1 per sweep) instead of one per round of rows (p - 1);
+//     (2 BR x p) into shared memory, forms their Gram matrix W = X X' (2 BR x 2 BR, register-tiled, k split over 8
+//     thread groups), runs ONE cyclic sweep of two-sided Jacobi on W in shared memory (rotation threshold relative to
+//     sqrt(w_ii w_jj), de Rijk), accumulating the rotations in Q, and writes Q X straight back to L2 (4 x 4 register
+//     tiles). The cluster meets at one barrier per ROUND OF BLOCKS (NB - 1 per sweep) instead of one per round of
+//     rows (p - 1);
 //   * a pair whose Gram matrix is already diagonal to the tolerance costs a load and the Gram product only;
-//   * the sweep count falls further with a warm start: the caller may pass Vt = the previous iterate's eigenvectors
-//     and G = Vt (S + mu I) (one GEMM), since consecutive ADMM iterates have nearby eigenbases.
-// On exit Vt holds the normalised rows of G (orthonormal to the convergence tolerance whatever rounding did to the
-// accumulated rotations), lam the eigenvalues.
+//   * the sweep count falls further with a warm start: the caller passes G = V_prev' (S + mu I) (one GEMM) for the
+//     previous iterate's eigenvectors, since consecutive ADMM iterates have nearby eigenbases, and a mu from Weyl's
+//     inequality (k_large_smat) instead of ||S||_F.
+// On exit Vt holds the normalised rows of G (orthonormal to the convergence tolerance by construction) and lam =
+// ||g_i|| - mu, which the caller replaces by Rayleigh quotients against the unshifted S (k_large_rayleigh): the
+// approximate reciprocals in the rotation set-up scale row pairs by 1 + O(eps), which the quotient does not see.
 #pragma once
 #include <cooperative_groups.h>
 #include "common.cuh"
@@ -160,16 +163,18 @@ __device__ __forceinline__ double gram_reduce(const T* part, T* W, double* red) 
 }
 
 // Rotation (sin, tau = sin / (1 + cos)) that annihilates w_ij, or the identity when |w_ij| <= thresh sqrt(w_ii w_jj).
+__device__ __forceinline__ float rcp_approx(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float rsqrt_approx(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ void sweep_angle(float a, float b, float c, float thresh, float& sn, float& tau) {
   // approximate reciprocals / square roots: they only perturb the angle and scale the row pair by 1 + O(eps s^2);
   // eigenvalues are Rayleigh quotients taken afterwards and eigenvectors are the normalised rows, so neither matters.
   sn = 0.f; tau = 0.f;
   if (c * c > thresh * thresh * a * b) {
-    const float th = __fdividef(b - a, 2.f * c);
+    const float th = (b - a) * rcp_approx(2.f * c);
     const float h2 = 1.f + th * th;
-    const float t = __fdividef(th >= 0.f ? 1.f : -1.f, fabsf(th) + h2 * rsqrtf(h2));
-    const float cs = rsqrtf(1.f + t * t);
-    sn = t * cs; tau = __fdividef(sn, 1.f + cs);
+    const float t = copysignf(rcp_approx(fabsf(th) + h2 * rsqrt_approx(h2)), th);
+    const float cs = rsqrt_approx(1.f + t * t);
+    sn = t * cs; tau = sn * rcp_approx(1.f + cs);
   }
 }
 __device__ __forceinline__ void sweep_angle(double a, double b, double c, double thresh, double& sn, double& tau) {
