@@ -381,6 +381,19 @@ __global__ void __launch_bounds__(psd_small_max_threads(MAXI)) k_psd_fwd_small(P
       const int i = t / ldv, a = t - i * ldv;
       ws.Vt[t] = (i < p && a < p) ? Up[i * p + a] : ((i == a) ? (T)1 : (T)0);
     }
+    __syncthreads();
+    // One Newton-Schulz step U <- (3/2) U - (1/2) U (U'U) first: the basis is a product of hundreds of fp32 rotations
+    // per iterate and is carried from iterate to iterate, so its orthogonality error would grow with k (measured on
+    // cfg2: iterate error 8.6e-5 after 50 steps without this step, 1e-5 with it); the step squares that error.
+    smem_gemm<T>(pe, ws.Vt, ldv, 1, ws.Vt, 1, ldv, Tm, pe);    // Tm(i,j) = <u_i, u_j>
+    __syncthreads();
+    smem_gemm<T>(pe, Tm, pe, 1, ws.Vt, ldv, 1, Sd, pe);        // Sd(i,a) = sum_j Tm(i,j) U(a,j)
+    __syncthreads();
+    for (int t = threadIdx.x; t < pe * pe; t += blockDim.x) {
+      const int i = t / pe, a = t - i * pe;
+      ws.Vt[i * ldv + a] = (T)1.5 * ws.Vt[i * ldv + a] - (T)0.5 * Sd[i * pe + a];
+    }
+    __syncthreads();
     load_smat<T>(p, pe, pe, Sd, w, 0.0, nullptr);
     __syncthreads();
     smem_gemm<T>(pe, Sd, pe, 1, ws.Vt, 1, ldv, Tm, pe);        // Tm(a,i) = sum_b S(a,b) U(b,i)

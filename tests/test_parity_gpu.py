@@ -77,6 +77,31 @@ def test_runs_are_deterministic():
     assert np.array_equal(a["g_rho"], b["g_rho"]) and all(np.array_equal(u, v) for u, v in zip(a["xK"], b["xK"]))
 
 
+def test_repeated_calls_on_one_handle_are_bitwise_identical():
+    """The PSD kernels warm-start every eigendecomposition from the previous iterate's eigenbasis; each unroll (and
+    each LEAN backward) restarts cold, so a handle's results must not depend on what it computed before.
+    Small blocks (shared-memory Jacobi) and a block of the large path, FULL and LEAN checkpoints."""
+    import torch
+    import paper_2606_13825_b200 as cdu
+    for kw, opts in ((dict(batch=3, p=14, K=8), {}), (dict(batch=2, p=40, K=6), dict(psd_small_max=8))):
+        wl = W.make_config(2, **kw)
+        pk = W.pack_batch(wl.problems, wl.dtype)
+        for ckpt in (0, 1):
+            h = cdu.cdu_create(pk, K_max=wl.K, ckpt_mode=ckpt, **opts)
+            T = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float32, device="cuda")
+            rng = np.random.default_rng(5)
+            cot = [T(rng.standard_normal(int(pk[k][-1]))) for k in ("var_off", "row_off", "row_off")]
+            outs = []
+            for _ in range(2):
+                z = cdu.cdu_forward(h, wl.K, T(wl.rho), T(wl.alpha), wl.sigma, None, None, None)
+                g = cdu.cdu_backward(h, *cot)
+                torch.cuda.synchronize()
+                outs.append([t.clone() for t in z] + [g[k].clone() for k in ("g_rho", "g_alpha", "g_sigma", "g_x0", "g_s0", "g_y0")])
+            for a, b in zip(*outs):
+                assert torch.equal(a, b)
+            cdu.cdu_destroy(h)
+
+
 # ---- thread-block-cluster teams (several CTAs per problem) against the oracle ---------------------------------
 @pytest.mark.parametrize("dtype,team,ckpt", [("f64", 2, 0), ("f64", 4, 1), ("f32", 8, 0), ("f32", 16, 1)])
 def test_cluster_teams_all_cone_types(dtype, team, ckpt):
