@@ -668,47 +668,65 @@ cdu_status HandleT<T, IT>::init(const cdu_problem* pr, const cdu_options* op, cu
     D.P_smem = (C == 1 && p_dense && D.vec_smem && pd_bytes + vec_bytes <= budget) ? 1 : 0;
     lin_smem = (D.vec_smem ? vec_bytes : 0) + (D.P_smem ? pd_bytes : 0);
     team_C = C;
-    // ---- warp row batches (lin.cuh batch_rows): single-CTA teams with shared-memory vectors -------------------------
-    D.batched = 0; D.rp_smem = 0; D.nmax = nmax; D.mmax = mmax;
+    // ---- sliced-ELL chunk format (lin.cuh sell_rows): single-CTA teams with shared-memory vectors -------------------
+    D.batched = 0; D.nmax = nmax; D.mmax = mmax; D.sell_slots = 0;
     if (C == 1 && D.vec_smem && o.no_batch == 0) {
-      const size_t rp_bytes = ((((size_t)mmax + 1 + 3) & ~(size_t)3) + 2 * (((size_t)nmax + 1 + 3) & ~(size_t)3)) * sizeof(int);
-      const size_t fixed = (size_t)(lin_threads / 32) * BATCH_ELEMS * sizeof(double) + rp_bytes + vec_bytes;
-      if (fixed <= budget) {
-        D.batched = 1; D.rp_smem = 1;
-        D.P_smem = (p_dense && fixed + pd_bytes <= budget) ? 1 : 0;
-        lin_smem = fixed + (D.P_smem ? pd_bytes : 0);
-      }
-    }
-    if (D.batched) {
-      auto build = [&](const std::vector<int>& rp, const int64_t* off, std::vector<int2>& bt, std::vector<int>& bo) {
-        bo.assign(B + 1, 0);
+      struct SellHost {
+        std::vector<int> sl_base, slab_off, crow, mr_base; std::vector<int4> mrow; std::vector<T> val; std::vector<IT> idx; int max_slots = 0;
+      };
+      // rows [off[b], off[b+1]) of problem b; rp global row pointers; ci / v the element arrays
+      auto build = [&](const std::vector<int>& rp, const int64_t* off, const IT* ci, const T* v, SellHost& S) {
+        struct Chunk { int len, row, start, slot; };
+        S.sl_base.assign(B + 1, 0); S.mr_base.assign(B + 1, 0); S.slab_off.assign(1, 0);
+        std::vector<Chunk> ch;
+        int col = 0;
         for (int b = 0; b < B; ++b) {
-          const long long r0 = off[b], r1 = off[b + 1];
-          long long row = r0;
-          while (row < r1) {
-            const int len = rp[row + 1] - rp[row];
-            if (len >= LONG_ROW) { bt.push_back(make_int2((int)(row - r0), -1)); ++row; continue; }
-            const long long first = row;
-            int tot = 0;
-            while (row < r1 && row - first < 128) {
-              const int l = rp[row + 1] - rp[row];
-              if (l >= LONG_ROW || tot + l > BATCH_ELEMS) break;
-              tot += l; ++row;
-            }
-            bt.push_back(make_int2((int)(first - r0), (int)(row - first)));
+          ch.clear();
+          int slots = 0;
+          for (long long r = off[b]; r < off[b + 1]; ++r) {
+            const int len = rp[r + 1] - rp[r], nch = std::max(1, (len + 31) / 32);
+            if (nch > 1) S.mrow.push_back(make_int4((int)(r - off[b]), slots, nch, 0));
+            for (int c = 0; c < nch; ++c)
+              ch.push_back(Chunk{std::min(32, len - 32 * c), (int)(r - off[b]), rp[r] + 32 * c, nch > 1 ? slots++ : -1});
           }
-          bo[b + 1] = (int)bt.size();
+          S.max_slots = std::max(S.max_slots, slots);
+          std::stable_sort(ch.begin(), ch.end(), [](const Chunk& x, const Chunk& y) { return x.len > y.len; });
+          for (size_t i = 0; i < ch.size(); i += 32) {
+            const int L = ch[i].len;
+            const size_t base = S.val.size();
+            S.val.resize(base + (size_t)L * 32, (T)0); S.idx.resize(base + (size_t)L * 32, (IT)0);
+            for (int lane = 0; lane < 32; ++lane) {
+              if (i + lane >= ch.size()) { S.crow.push_back(SELL_NONE); continue; }
+              const Chunk& q = ch[i + lane];
+              S.crow.push_back(q.slot < 0 ? q.row : -(q.slot + 1));
+              for (int k = 0; k < q.len; ++k) { S.val[base + (size_t)k * 32 + lane] = v[q.start + k]; S.idx[base + (size_t)k * 32 + lane] = ci[q.start + k]; }
+            }
+            col += L;
+            S.slab_off.push_back(col);
+          }
+          S.sl_base[b + 1] = (int)S.slab_off.size() - 1;
+          S.mr_base[b + 1] = (int)S.mrow.size();
         }
       };
-      std::vector<int2> bta, btt, btp;
-      std::vector<int> boa, bot, bop;
-      build(A_rp, pr->row_off, bta, boa);
-      build(AT_rp, pr->var_off, btt, bot);
-      if (!p_dense) build(P_rp, pr->var_off, btp, bop); else bop.assign(B + 1, 0);
-      D.A_bt = pool.upload(bta, st); D.AT_bt = pool.upload(btt, st); D.P_bt = pool.upload(btp, st);
-      D.A_bo = pool.upload(boa, st); D.AT_bo = pool.upload(bot, st); D.P_bo = pool.upload(bop, st);
-      if (pool.last != cudaSuccess) { err = std::string("cdu_create (batches): ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
-      CU_OK(cudaStreamSynchronize(st));   // the staging vectors go out of scope
+      auto upload = [&](SellHost& S, Sell<T, IT>& dS) {
+        dS.sl_base = pool.upload(S.sl_base, st); dS.slab_off = pool.upload(S.slab_off, st); dS.crow = pool.upload(S.crow, st);
+        dS.mr_base = pool.upload(S.mr_base, st); dS.mrow = pool.upload(S.mrow, st); dS.val = pool.upload(S.val, st); dS.idx = pool.upload(S.idx, st);
+      };
+      SellHost hA, hAT, hP;
+      build(A_rp, pr->row_off, A_ci.data(), Av, hA);
+      build(AT_rp, pr->var_off, AT_ci.data(), AT_v.data(), hAT);
+      if (!p_dense) build(P_rp, pr->var_off, P_ci.data(), Pv, hP);     // rows without entries still emit a zero
+      else { hP.sl_base.assign(B + 1, 0); hP.mr_base.assign(B + 1, 0); hP.slab_off.assign(1, 0); }
+      const int slots = std::max(hA.max_slots, std::max(hAT.max_slots, hP.max_slots));
+      const size_t fixed = (((size_t)slots + 1) & ~(size_t)1) * sizeof(double) + vec_bytes;
+      if (fixed <= budget) {
+        D.batched = 1; D.sell_slots = slots;
+        D.P_smem = (p_dense && fixed + pd_bytes <= budget) ? 1 : 0;
+        lin_smem = fixed + (D.P_smem ? pd_bytes : 0);
+        upload(hA, D.SA); upload(hAT, D.SAT); upload(hP, D.SP);
+        if (pool.last != cudaSuccess) { err = std::string("cdu_create (sliced ELL): ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
+        CU_OK(cudaStreamSynchronize(st));   // the staging vectors go out of scope
+      }
     }
     const void* fns[4] = {(const void*)k_fwd<T, IT, false>, (const void*)k_bwd<T, IT, false>, (const void*)k_fwd<T, IT, true>,
                           (const void*)k_bwd<T, IT, true>};

@@ -35,12 +35,17 @@ __device__ __forceinline__ void block_sum(double (&v)[NV], double* sh) {
     for (int i = 0; i < NV; ++i) sh[i * 32 + wid] = v[i];
   }
   __syncthreads();
+  if (wid == 0) {   // one warp folds the per-warp partials (fixed shuffle tree: deterministic) and publishes the totals
 #pragma unroll
-  for (int i = 0; i < NV; ++i) {
-    double t = 0.0;
-    for (int w = 0; w < nw; ++w) t += sh[i * 32 + w];
-    v[i] = t;
+    for (int i = 0; i < NV; ++i) {
+      double t = lane < nw ? sh[i * 32 + lane] : 0.0;
+      t = warp_sum(t);
+      if (lane == 0) sh[i * 32] = t;
+    }
   }
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < NV; ++i) v[i] = sh[i * 32];
   __syncthreads();
 }
 

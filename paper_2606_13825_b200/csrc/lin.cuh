@@ -19,6 +19,23 @@
 namespace cdu {
 namespace cg = cooperative_groups;
 
+// Sliced ELL with row chunks: every row is cut into chunks of at most 32 elements; the chunks of a problem are sorted
+// by length and packed 32 to a slab, one per lane, stored lane-interleaved (element k of the 32 chunks is contiguous),
+// so a warp walks a slab with one coalesced value load, one index load, one gather and one FMA per element and
+// lane. A row of one chunk is finished in its lane (crow >= 0); the chunks of a longer row leave partial sums in
+// consecutive scratch slots (crow = -(slot + 1)) that are summed in chunk order afterwards (mrow). Padding is
+// value 0 / column 0. Fixed summation order: bit-reproducible.
+constexpr int SELL_NONE = -2147483647 - 1;
+template <typename TV, typename IT>
+struct Sell {
+  const int* sl_base;    // [B+1] first slab of each problem
+  const int* slab_off;   // [nslab+1] first element column of each slab (a column = 32 elements)
+  const TV* val; const IT* idx;
+  const int* crow;       // [nslab*32]
+  const int* mr_base;    // [B+1] first multi-chunk row of each problem
+  const int4* mrow;      // (row, first slot, number of slots, -)
+};
+
 template <typename T, typename IT>
 struct BatchDev {
   int B;
@@ -28,11 +45,9 @@ struct BatchDev {
   const int *P_rp;  const IT* P_ci;  const T* P_v;  int P_G;   // P   : full symmetric storage (CSR), or
   int P_dense; const long long* P_off;                 //       dense row-major n_b x n_b blocks at P_v + P_off[b]
   int P_smem, vec_smem;                                // dense P / CG vectors live in dynamic shared memory
-  // row batches (single-CTA teams): warp-sized work items built by cdu_create. bt = (first row, number of rows);
-  // rows shorter than LONG_ROW are packed into batches of at most BATCH_ELEMS elements, a longer row is a batch of
-  // its own (count -1). bo = per-problem offsets [B+1]. rp_smem: local row pointers are copied to shared memory.
-  int batched, rp_smem, nmax, mmax;
-  const int2 *A_bt, *AT_bt, *P_bt; const int *A_bo, *AT_bo, *P_bo;
+  // sliced-ELL chunk format (single-CTA teams), built by cdu_create - see Sell below.
+  int batched, nmax, mmax, sell_slots;
+  Sell<T, IT> SA, SAT, SP;
   const T *q, *b, *diagP, *colsq;
   const uint8_t* rowkind;                              // per row: cone kind
   const int *soc_off, *soc_start, *soc_dim;            // per problem SOC list (start = local row)
@@ -156,58 +171,40 @@ __device__ __forceinline__ void dense_rows(int lo, int hi, int n, const TV* __re
   }
 }
 
-// ---- batched rows: one warp per work item, every load of an item in flight at once ---------------------------
-constexpr int BATCH_ELEMS = 128;   // elements of a packed batch (4 loads per lane); scratch = 128 doubles per warp
-constexpr int LONG_ROW = 64;       // rows at least this long are taken by a whole warp
-
-// rows of one pass given as batches bt[0..nb): warps take batches round-robin. rp = local row pointers (shared or
-// global), v / ci = the problem's value / index arrays (element 0 = first element of local row 0).
-// emit(row, dot) runs on one lane per row (any lane).
+// ---- sliced-ELL rows: one warp per slab ---------------------------------------------------------------------
+// emit(row, dot) runs exactly once per row (any thread). Contains CTA barriers: every thread of the CTA must call.
 template <typename TACC, typename TV, typename IT, typename TX, typename F>
-__device__ __forceinline__ void batch_rows(const int2* __restrict__ bt, int nb, const int* rp, const TV* __restrict__ v,
-                                           const IT* __restrict__ ci, const TX* x, TACC* scratch, F emit) {
+__device__ __forceinline__ void sell_rows(const Sell<TV, IT>& S, int b, const TX* x, TACC* scratch, F emit) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
-  for (int i = warp; i < nb; i += nw) {
-    const int2 d = __ldg(bt + i);
-    if (d.y < 0) {   // one long row: strided by the warp, 8 loads per lane in flight
-      const int e0 = rp[d.x], e1 = rp[d.x + 1];
-      TACC acc = (TACC)0;
-      for (int base = e0 + lane; base < e1; base += 256) {
-        TV vv[8]; int cc[8];
+  const int s0 = __ldg(S.sl_base + b), s1 = __ldg(S.sl_base + b + 1);
+  for (int sl = s0 + warp; sl < s1; sl += nw) {
+    const int e0 = __ldg(S.slab_off + sl), len = __ldg(S.slab_off + sl + 1) - e0;
+    const TV* __restrict__ v = S.val + (size_t)e0 * 32 + lane;
+    const IT* __restrict__ ci = S.idx + (size_t)e0 * 32 + lane;
+    TACC a0 = (TACC)0, a1 = (TACC)0;
+    int k = 0;
+    for (; k + 8 <= len; k += 8) {
+      TV vv[8]; int cc[8];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const int e = base + 32 * j;
-          vv[j] = (TV)0; cc[j] = 0;
-          if (e < e1) { vv[j] = __ldg(v + e); cc[j] = (int)__ldg(ci + e); }
-        }
+      for (int j = 0; j < 8; ++j) { vv[j] = __ldg(v + (k + j) * 32); cc[j] = (int)__ldg(ci + (k + j) * 32); }
 #pragma unroll
-        for (int j = 0; j < 8; ++j) acc += (TACC)vv[j] * (TACC)x[cc[j]];
-      }
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-      if (lane == 0) emit(d.x, acc);
-    } else {         // d.y short rows, at most BATCH_ELEMS elements in total
-      const int e0 = rp[d.x], e1 = rp[d.x + d.y];
-      TV vv[4]; int cc[4];
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        const int e = e0 + lane + 32 * j;
-        vv[j] = (TV)0; cc[j] = 0;
-        if (e < e1) { vv[j] = __ldg(v + e); cc[j] = (int)__ldg(ci + e); }
-      }
-#pragma unroll
-      for (int j = 0; j < 4; ++j)
-        if (e0 + lane + 32 * j < e1) scratch[lane + 32 * j] = (TACC)vv[j] * (TACC)x[cc[j]];
-      __syncwarp();
-      for (int r = lane; r < d.y; r += 32) {
-        const int s0 = rp[d.x + r] - e0, s1 = rp[d.x + r + 1] - e0;
-        TACC acc = (TACC)0;
-        for (int t = s0; t < s1; ++t) acc += scratch[t];
-        emit(d.x + r, acc);
-      }
-      __syncwarp();
+      for (int j = 0; j < 8; j += 2) { a0 += (TACC)vv[j] * (TACC)x[cc[j]]; a1 += (TACC)vv[j + 1] * (TACC)x[cc[j + 1]]; }
     }
+    for (; k < len; ++k) a0 += (TACC)__ldg(v + k * 32) * (TACC)x[(int)__ldg(ci + k * 32)];
+    a0 += a1;
+    const int cr = __ldg(S.crow + (size_t)sl * 32 + lane);
+    if (cr >= 0) emit(cr, a0);
+    else if (cr != SELL_NONE) scratch[-cr - 1] = a0;
   }
+  __syncthreads();
+  const int m0 = __ldg(S.mr_base + b), m1 = __ldg(S.mr_base + b + 1);
+  for (int j = m0 + threadIdx.x; j < m1; j += blockDim.x) {
+    const int4 d = __ldg(S.mrow + j);
+    TACC a = (TACC)0;
+    for (int q = 0; q < d.z; ++q) a += scratch[d.y + q];
+    emit(d.x, a);
+  }
+  __syncthreads();
 }
 
 template <typename T, typename IT, bool MULTI>
@@ -221,9 +218,7 @@ struct Prob {  // one problem's view of the batch, as seen by one CTA of its tea
   T *r, *p, *Ap, *d, *dinv, *tA;
   double rho, alpha, sigma;
   Team<MULTI>* team;
-  const int *rpA, *rpAT, *rpP;        // local row pointers (shared memory when D.rp_smem)
-  const T *Av, *ATv, *Pv; const IT *Aci, *ATci, *Pci;   // the problem's arrays, element 0 = first element of row 0
-  double* scratch;                    // this warp's product staging (BATCH_ELEMS doubles)
+  double* scratch;                    // partial sums of multi-chunk rows (sell_rows), D.sell_slots doubles
   __device__ Prob(const BatchDev<T, IT>& D, int b_, Team<MULTI>* tm_, unsigned char* dsm) : b(b_), team(tm_) {
     const int v0 = D.var_off[b], r0 = D.row_off[b];
     n = D.var_off[b + 1] - v0; m = D.row_off[b + 1] - r0;
@@ -232,19 +227,10 @@ struct Prob {  // one problem's view of the batch, as seen by one CTA of its tea
     q = D.q + v0; bv = D.b + r0; diagP = D.diagP + v0; colsq = D.colsq + v0;
     xi = D.xi + v0; rd = D.rd + v0; lam = D.lam + v0; tm = D.tm + r0; W = D.W + r0; GW = D.GW + r0;
     Pd = D.P_dense ? D.P_v + D.P_off[b] : nullptr;
-    rpA = A_rp; rpAT = AT_rp; rpP = P_rp; scratch = nullptr;
+    scratch = nullptr;
     if (D.batched) {
-      const int a0 = A_rp[0], t0 = AT_rp[0], p0 = P_rp[0];
-      Av = D.A_v + a0; Aci = D.A_ci + a0; ATv = D.AT_v + t0; ATci = D.AT_ci + t0; Pv = D.P_v + p0; Pci = D.P_dense ? nullptr : D.P_ci + p0;
-      scratch = reinterpret_cast<double*>(dsm) + (threadIdx.x >> 5) * BATCH_ELEMS;
-      dsm += (size_t)(blockDim.x >> 5) * BATCH_ELEMS * sizeof(double);
-      int* rpa = reinterpret_cast<int*>(dsm); dsm += (((size_t)D.mmax + 1 + 3) & ~(size_t)3) * sizeof(int);
-      int* rpat = reinterpret_cast<int*>(dsm); dsm += (((size_t)D.nmax + 1 + 3) & ~(size_t)3) * sizeof(int);
-      int* rpp = reinterpret_cast<int*>(dsm); dsm += (((size_t)D.nmax + 1 + 3) & ~(size_t)3) * sizeof(int);
-      __syncthreads();   // the previous problem's readers are done
-      for (int i = threadIdx.x; i <= m; i += blockDim.x) rpa[i] = A_rp[i] - a0;
-      for (int i = threadIdx.x; i <= n; i += blockDim.x) { rpat[i] = AT_rp[i] - t0; rpp[i] = P_rp[i] - p0; }
-      rpA = rpa; rpAT = rpat; rpP = rpp;
+      scratch = reinterpret_cast<double*>(dsm);
+      dsm += (((size_t)D.sell_slots + 1) & ~(size_t)1) * sizeof(double);
     }
     T* sv = reinterpret_cast<T*>(dsm);
     if (D.P_smem) {   // cache the dense P of this problem (single-CTA teams only)
@@ -266,18 +252,18 @@ struct Prob {  // one problem's view of the batch, as seen by one CTA of its tea
 // One pass over the rows of A, A^T or P owned by this CTA: warp batches (single-CTA teams) or lane groups per row.
 template <typename TACC, typename T, typename IT, bool MULTI, typename TX, typename F>
 __device__ __forceinline__ void rows_A(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const TX* x, F emit) {
-  if (D.batched) batch_rows<TACC>(D.A_bt + D.A_bo[c.b], D.A_bo[c.b + 1] - D.A_bo[c.b], c.rpA, c.Av, c.Aci, x, reinterpret_cast<TACC*>(c.scratch), emit);
+  if (D.batched) sell_rows<TACC>(D.SA, c.b, x, reinterpret_cast<TACC*>(c.scratch), emit);
   else spmv_rows<TACC, MULTI>(c.mlo, c.mhi, c.A_rp, D.A_ci, D.A_v, x, D.A_G, emit);
 }
 template <typename TACC, typename T, typename IT, bool MULTI, typename TX, typename F>
 __device__ __forceinline__ void rows_AT(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const TX* x, F emit) {
-  if (D.batched) batch_rows<TACC>(D.AT_bt + D.AT_bo[c.b], D.AT_bo[c.b + 1] - D.AT_bo[c.b], c.rpAT, c.ATv, c.ATci, x, reinterpret_cast<TACC*>(c.scratch), emit);
+  if (D.batched) sell_rows<TACC>(D.SAT, c.b, x, reinterpret_cast<TACC*>(c.scratch), emit);
   else spmv_rows<TACC, MULTI>(c.nlo, c.nhi, c.AT_rp, D.AT_ci, D.AT_v, x, D.AT_G, emit);
 }
 template <typename TACC, typename T, typename IT, bool MULTI, typename TX, typename F>
 __device__ __forceinline__ void rows_P(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const TX* x, F emit) {
   if (c.Pd) dense_rows<TACC, MULTI>(c.nlo, c.nhi, c.n, c.Pd, x, emit);
-  else if (D.batched) batch_rows<TACC>(D.P_bt + D.P_bo[c.b], D.P_bo[c.b + 1] - D.P_bo[c.b], c.rpP, c.Pv, c.Pci, x, reinterpret_cast<TACC*>(c.scratch), emit);
+  else if (D.batched) sell_rows<TACC>(D.SP, c.b, x, reinterpret_cast<TACC*>(c.scratch), emit);
   else spmv_rows<TACC, MULTI>(c.nlo, c.nhi, c.P_rp, D.P_ci, D.P_v, x, D.P_G, emit);
 }
 
