@@ -692,14 +692,17 @@ cdu_status HandleT<T, IT>::init(const cdu_problem* pr, const cdu_options* op, cu
           S.max_slots = std::max(S.max_slots, slots);
           std::stable_sort(ch.begin(), ch.end(), [](const Chunk& x, const Chunk& y) { return x.len > y.len; });
           for (size_t i = 0; i < ch.size(); i += 32) {
-            const int L = ch[i].len;
+            const int L = (ch[i].len + 1) / 2;      // element pairs per lane
             const size_t base = S.val.size();
-            S.val.resize(base + (size_t)L * 32, (T)0); S.idx.resize(base + (size_t)L * 32, (IT)0);
+            S.val.resize(base + (size_t)L * 64, (T)0); S.idx.resize(base + (size_t)L * 64, (IT)0);
             for (int lane = 0; lane < 32; ++lane) {
               if (i + lane >= ch.size()) { S.crow.push_back(SELL_NONE); continue; }
               const Chunk& q = ch[i + lane];
               S.crow.push_back(q.slot < 0 ? q.row : -(q.slot + 1));
-              for (int k = 0; k < q.len; ++k) { S.val[base + (size_t)k * 32 + lane] = v[q.start + k]; S.idx[base + (size_t)k * 32 + lane] = ci[q.start + k]; }
+              for (int k = 0; k < q.len; ++k) {
+                const size_t o = base + ((size_t)(k >> 1) * 32 + lane) * 2 + (k & 1);
+                S.val[o] = v[q.start + k]; S.idx[o] = ci[q.start + k];
+              }
             }
             col += L;
             S.slab_off.push_back(col);

@@ -20,16 +20,16 @@ namespace cdu {
 namespace cg = cooperative_groups;
 
 // Sliced ELL with row chunks: every row is cut into chunks of at most 32 elements; the chunks of a problem are sorted
-// by length and packed 32 to a slab, one per lane, stored lane-interleaved (element k of the 32 chunks is contiguous),
-// so a warp walks a slab with one coalesced value load, one index load, one gather and one FMA per element and
-// lane. A row of one chunk is finished in its lane (crow >= 0); the chunks of a longer row leave partial sums in
+// by length and packed 32 to a slab, one per lane, stored lane-interleaved in element PAIRS (pair k of the 32 chunks
+// is contiguous: 32 x (v0, v1) and 32 x (c0, c1)), so a warp walks a slab with one coalesced 8-byte value load and one
+// index load per two elements, 16 elements of every lane in flight at a time, plus one gather and one FMA per element. A row of one chunk is finished in its lane (crow >= 0); the chunks of a longer row leave partial sums in
 // consecutive scratch slots (crow = -(slot + 1)) that are summed in chunk order afterwards (mrow). Padding is
 // value 0 / column 0. Fixed summation order: bit-reproducible.
 constexpr int SELL_NONE = -2147483647 - 1;
 template <typename TV, typename IT>
 struct Sell {
   const int* sl_base;    // [B+1] first slab of each problem
-  const int* slab_off;   // [nslab+1] first element column of each slab (a column = 32 elements)
+  const int* slab_off;   // [nslab+1] first pair column of each slab (a column = 32 lanes x 2 elements)
   const TV* val; const IT* idx;
   const int* crow;       // [nslab*32]
   const int* mr_base;    // [B+1] first multi-chunk row of each problem
@@ -171,6 +171,14 @@ __device__ __forceinline__ void dense_rows(int lo, int hi, int n, const TV* __re
   }
 }
 
+// two consecutive elements of a lane's chunk in one load (read-only path)
+__device__ __forceinline__ void ld_pair(const float* p, float& a, float& b) { const float2 t = __ldg(reinterpret_cast<const float2*>(p)); a = t.x; b = t.y; }
+__device__ __forceinline__ void ld_pair(const double* p, double& a, double& b) { const double2 t = __ldg(reinterpret_cast<const double2*>(p)); a = t.x; b = t.y; }
+__device__ __forceinline__ void ld_pair(const int* p, int& a, int& b) { const int2 t = __ldg(reinterpret_cast<const int2*>(p)); a = t.x; b = t.y; }
+__device__ __forceinline__ void ld_pair(const uint16_t* p, int& a, int& b) {
+  const unsigned t = __ldg(reinterpret_cast<const unsigned*>(p)); a = (int)(t & 0xffffu); b = (int)(t >> 16);
+}
+
 // ---- sliced-ELL rows: one warp per slab ---------------------------------------------------------------------
 // emit(row, dot) runs exactly once per row (any thread). Contains CTA barriers: every thread of the CTA must call.
 template <typename TACC, typename TV, typename IT, typename TX, typename F>
@@ -178,19 +186,23 @@ __device__ __forceinline__ void sell_rows(const Sell<TV, IT>& S, int b, const TX
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
   const int s0 = __ldg(S.sl_base + b), s1 = __ldg(S.sl_base + b + 1);
   for (int sl = s0 + warp; sl < s1; sl += nw) {
-    const int e0 = __ldg(S.slab_off + sl), len = __ldg(S.slab_off + sl + 1) - e0;
-    const TV* __restrict__ v = S.val + (size_t)e0 * 32 + lane;
-    const IT* __restrict__ ci = S.idx + (size_t)e0 * 32 + lane;
+    const int e0 = __ldg(S.slab_off + sl), lp = __ldg(S.slab_off + sl + 1) - e0;     // element PAIRS per lane
+    const TV* __restrict__ v = S.val + ((size_t)e0 * 32 + lane) * 2;
+    const IT* __restrict__ ci = S.idx + ((size_t)e0 * 32 + lane) * 2;
     TACC a0 = (TACC)0, a1 = (TACC)0;
     int k = 0;
-    for (; k + 8 <= len; k += 8) {
-      TV vv[8]; int cc[8];
+    for (; k + 8 <= lp; k += 8) {            // 16 elements of the chunk in flight per lane
+      TV v0[8], v1[8]; int c0[8], c1[8];
 #pragma unroll
-      for (int j = 0; j < 8; ++j) { vv[j] = __ldg(v + (k + j) * 32); cc[j] = (int)__ldg(ci + (k + j) * 32); }
+      for (int j = 0; j < 8; ++j) { ld_pair(v + (size_t)(k + j) * 64, v0[j], v1[j]); ld_pair(ci + (size_t)(k + j) * 64, c0[j], c1[j]); }
 #pragma unroll
-      for (int j = 0; j < 8; j += 2) { a0 += (TACC)vv[j] * (TACC)x[cc[j]]; a1 += (TACC)vv[j + 1] * (TACC)x[cc[j + 1]]; }
+      for (int j = 0; j < 8; ++j) { a0 += (TACC)v0[j] * (TACC)x[c0[j]]; a1 += (TACC)v1[j] * (TACC)x[c1[j]]; }
     }
-    for (; k < len; ++k) a0 += (TACC)__ldg(v + k * 32) * (TACC)x[(int)__ldg(ci + k * 32)];
+    for (; k < lp; ++k) {
+      TV v0, v1; int c0, c1;
+      ld_pair(v + (size_t)k * 64, v0, v1); ld_pair(ci + (size_t)k * 64, c0, c1);
+      a0 += (TACC)v0 * (TACC)x[c0]; a1 += (TACC)v1 * (TACC)x[c1];
+    }
     a0 += a1;
     const int cr = __ldg(S.crow + (size_t)sl * 32 + lane);
     if (cr >= 0) emit(cr, a0);
