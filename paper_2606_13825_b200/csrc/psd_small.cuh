@@ -304,19 +304,34 @@ __device__ int jacobi_planes(int pe, const JacobiWs<T>& w, double* shred, int ma
   return sweep;
 }
 
-// C(i,j) = sum_k A(i,k) B(k,j), all pe x pe in shared memory with generic strides; 2x2 register tiles.
+// C(i,j) = sum_k A(i,k) B(k,j), all pe x pe in shared memory with generic strides; 2x2 register tiles, consecutive
+// threads along j. When B is read transposed (sbk == 1: the rows of B' are k-contiguous with an even stride) the
+// threads of a warp would hit the same few banks at every k; they then walk k skewed by their tile column, which
+// makes the B loads and the (no longer broadcast) A loads conflict free.
 template <typename T>
 __device__ __forceinline__ void smem_gemm(int pe, const T* A, int sai, int sak, const T* B, int sbk, int sbj, T* C,
                                           int ldc) {
   const int h = pe >> 1;
+  const bool skewed = (sbk == 1 && sbj != 1 && sak == 1);
   for (int t = threadIdx.x; t < h * h; t += blockDim.x) {
-    const int i = (t / h) * 2, j = (t % h) * 2;
+    const int jt = t % h;
+    const int i = (t / h) * 2, j = jt * 2;
     T c00 = 0, c01 = 0, c10 = 0, c11 = 0;
     const T *a0 = A + i * sai, *a1 = a0 + sai, *b0 = B + j * sbj, *b1 = b0 + sbj;
+    if (skewed) {
+      int k = jt;                       // pe = 2 h > jt
 #pragma unroll 4
-    for (int k = 0; k < pe; ++k) {
-      const T x0 = a0[k * sak], x1 = a1[k * sak], y0 = b0[k * sbk], y1 = b1[k * sbk];
-      c00 += x0 * y0; c01 += x0 * y1; c10 += x1 * y0; c11 += x1 * y1;
+      for (int s = 0; s < pe; ++s) {
+        const T x0 = a0[k], x1 = a1[k], y0 = b0[k], y1 = b1[k];
+        c00 += x0 * y0; c01 += x0 * y1; c10 += x1 * y0; c11 += x1 * y1;
+        if (++k == pe) k = 0;
+      }
+    } else {
+#pragma unroll 4
+      for (int k = 0; k < pe; ++k) {
+        const T x0 = a0[k * sak], x1 = a1[k * sak], y0 = b0[k * sbk], y1 = b1[k * sbk];
+        c00 += x0 * y0; c01 += x0 * y1; c10 += x1 * y0; c11 += x1 * y1;
+      }
     }
     C[i * ldc + j] = c00; C[i * ldc + j + 1] = c01; C[(i + 1) * ldc + j] = c10; C[(i + 1) * ldc + j + 1] = c11;
   }
