@@ -229,9 +229,10 @@ def test_full_size_configs_sampled(cfg):
     assert st["flags_or"] == 0
 
 
-def test_full_size_cfg5_sampled():
+@pytest.mark.parametrize("ckpt", [0, 1])
+def test_full_size_cfg5_sampled(ckpt):
     wl = W.make_config(5)
-    e, st = PU.check(wl, problems=FULL[5], per_problem=True)
+    e, st = PU.check(wl, problems=FULL[5], per_problem=True, ckpt_mode=ckpt)
     print(wl.name, e, st)
     PU.assert_within(e, wl.dtype)
 
