@@ -895,6 +895,7 @@ cdu_status HandleT<T, IT>::backward(const void* gx, const void* gs, const void* 
     Q.Gin = GZ[(k + 1) & 1]; Q.Gout = GZ[k & 1];
     Q.g_rho_pb = g_rho_pb; Q.g_alpha_pb = g_alpha_pb; Q.g_sigma_pb = g_sigma_pb; Q.part_pre = part_pre;
     Q.recompute = full ? 0 : 1;
+    Q.warm_adjoint = k < K - 1 ? 1 : 0;
     if (!has_psd) {
       prof.begin(PC_LIN_BWD, st);
       cudaError_t le = launch_lin(k_bwd<T, IT, false>, k_bwd<T, IT, true>, st, Db, H, Q, k, 0);

@@ -508,6 +508,7 @@ struct BwdPtrs {
   double* g_sigma_pb;
   double* part_pre;    // [B][2] partials handed from the pre to the post phase
   int recompute;       // LEAN: re-solve for xt, st
+  int warm_adjoint;    // not the first reverse step: D.lam holds the previous step's adjoint solution
 };
 
 // Phase 1 of the reverse step: (LEAN: re-solve), w, and B1/B2/B4 for zero, nonneg and SOC rows.
@@ -598,7 +599,11 @@ __device__ void bwd_post(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const 
   rows_AT<double>(D, c, c.GW, [&](int row, double a) { c.xi[row] = al * (gx1[row] - a); });
   __syncthreads();
   // B7: adjoint solve M lam = g_xt (Eq. 5), zero start
-  *iters += solve_M(D, c, c.xi, (const double*)nullptr, c.lam, flag);
+  // Start: 0 (reading A5) or, when the forward solves of this problem needed many CG iterations, the lam of the previous
+  // reverse step: the start costs one extra fp64 operator application, which only pays for long solves. Same solution to
+  // the same tolerance either way; the choice depends on this unroll's forward only (results stay history independent).
+  const bool warm = Q.warm_adjoint && D.cg_max[b] >= 12;
+  *iters += solve_M(D, c, c.xi, warm ? (const double*)c.lam : (const double*)nullptr, c.lam, flag);
   // u = A lam; B7+B9 combined: g_rho += <u, st - s> (cancellation-free form of Eq. 6 + RHS term)
   double acc[3] = {0.0, 0.0, 0.0};   // rho, alpha, sigma
   rows_A<double>(D, c, c.lam, [&](int row, double u) {
