@@ -313,6 +313,7 @@ k_bjacobi(int nblk, const int* pvec, const long long* moff, const int* voff, T* 
   for (int t = threadIdx.x; t < RP * ldx; t += blockDim.x) X[t] = (T)0;    // the pads stay zero
   __syncthreads();
   const T thresh = (T)(0.25 * tol);
+  const float quad_exit = (float)sqrt(tol / (16.0 * sqrt((double)p)));   // 2.9e-5 for fp32 at p = 512
   int sweep = 0;
   for (; sweep < max_sweeps; ++sweep) {
     for (int r = 0; r < NBe - 1; ++r) {
@@ -330,14 +331,16 @@ k_bjacobi(int nblk, const int* pvec, const long long* moff, const int* voff, T* 
           for (int t = threadIdx.x; t < RP * RP; t += blockDim.x) { const int i = t / RP, k = t - i * RP; Qt[k * LQ + i] = Q[i * LQ + k]; }
           __syncthreads();
           apply_store<T, RP>(Qt, X, ldx, p, g, bi * BR, bj2 * BR);
-          if (threadIdx.x == 0) __stcg(rf + sweep, 1);
+          if (threadIdx.x == 0) atomicMax(reinterpret_cast<unsigned*>(rf) + sweep, __float_as_uint((float)mx));   // mx > 0: ordered as unsigned
         }
         __syncthreads();
       }
       cluster.sync();
     }
-    if (!__ldcg(rf + sweep)) break;
-  }
+    const unsigned worst = (unsigned)__ldcg(rf + sweep);     // largest |w_ij| / sqrt(w_ii w_jj) any pair showed in this sweep
+    if (!worst) break;                                        // nothing above the tolerance: converged
+    if (__uint_as_float(worst) <= quad_exit) { ++sweep; break; }   // quadratic convergence: every pair above tol was rotated while
+  }                                                           // all ratios were <= quad_exit; what is left is ~quad_exit^2 sqrt(p) <= tol / 16
   // eigenvalues and eigenvectors
   const int lane = threadIdx.x & 31, nw = blockDim.x >> 5;
   const double m = (double)mu[lb];
