@@ -173,7 +173,7 @@ __device__ int jacobi_planes(int pe, const JacobiWs<T>& w, double* shred, int ma
   const double normF2 = acc[0];
   *cur_out = 0;
   if (!(normF2 > 0.0)) { if (normF2 != normF2) *flag |= FLAG_NONFINITE; return 0; }
-  const double tol2 = 16.0 * (double)Eps<T>::v() * (double)Eps<T>::v() * normF2;
+  const double tol2 = 256.0 * (double)Eps<T>::v() * (double)Eps<T>::v() * normF2;   // off-diagonal norm <= 16 eps ||S||_F
   const T skip = (T)(0.01 * sqrt(tol2) / pe);
 
   // per-thread constants (registers): blocks, eigenvector slices, or the pivot an angle thread prepares
