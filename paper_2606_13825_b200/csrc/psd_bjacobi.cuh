@@ -193,13 +193,25 @@ __device__ __forceinline__ void sweep_angle(double a, double b, double c, double
 // row pair q; every lane derives the rotation of pair (lane mod RP/2) from the current buffer itself, the warp's own
 // rotation comes by shuffle; lanes < RP/2 update the 2 x 2 block (pair q rows, pair lane columns), all lanes the Q rows.
 template <typename T, int RP>
-__device__ __forceinline__ T* inner_sweep(T* W0, T* W1, T* Q, T thresh, const int* pairs) {
+__device__ __forceinline__ T* inner_sweep(T* W0, T* W1, T* Q, T thresh, const int* pairs, unsigned* mask) {
   constexpr int H = RP / 2, LW = RP + 1, LQ = RP + 4;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   for (int t = tid; t < RP * RP; t += blockDim.x) { const int i = t / RP, j = t - i * RP; Q[i * LQ + j] = (i == j) ? (T)1 : (T)0; }
+  if (tid == 0) *mask = 0u;
   __syncthreads();
+  // rounds that hold at least one pair above the convergence tolerance: the others are skipped (late sweeps of a warm-started
+  // matrix leave a handful of pairs to rotate; what a rotation adds to other entries is second order and is met by the
+  // next sweep of the blocks)
+  for (int t = tid; t < (RP - 1) * H; t += blockDim.x) {
+    const int pr = pairs[t], i = pr & 0xffff, j = pr >> 16;
+    const T c = W0[i * LW + j];
+    if (c * c > (T)16 * thresh * thresh * W0[i * LW + i] * W0[j * LW + j]) atomicOr(mask, 1u << (t / H));   // 4 thresh = tol
+  }
+  __syncthreads();
+  const unsigned active = *mask;
   T* Wc = W0; T* Wn = W1;
   for (int r = 0; r < RP - 1; ++r) {
+    if (!((active >> r) & 1u)) continue;
     if (warp < H) {
       const int q2 = lane % H;
       const int pr = pairs[r * H + q2], i2 = pr & 0xffff, j2 = pr >> 16;
@@ -326,7 +338,7 @@ k_bjacobi(int nblk, const int* pvec, const long long* moff, const int* voff, T* 
         __syncthreads();
         const double mx = gram_reduce<T, RP>(part, W, red);
         if (mx > tol) {
-          const T* Wf = inner_sweep<T, RP>(W, W1, Q, thresh, pairs);
+          const T* Wf = inner_sweep<T, RP>(W, W1, Q, thresh, pairs, reinterpret_cast<unsigned*>(red + 40));
           (void)Wf;
           for (int t = threadIdx.x; t < RP * RP; t += blockDim.x) { const int i = t / RP, k = t - i * RP; Qt[k * LQ + i] = Q[i * LQ + k]; }
           __syncthreads();
