@@ -207,6 +207,7 @@ def main():
     ap.add_argument("--cg-refine", type=int, default=-2, help="-2: workload default (handle default: one refinement pass for fp32)")
     ap.add_argument("--cg-refine-tol", type=float, default=0.0)
     ap.add_argument("--tensor-cores", type=int, default=-1)
+    ap.add_argument("--team-size", type=int, default=0, help="CTAs per problem in the linear step (0: automatic) (debug)")
     ap.add_argument("--no-batch", type=int, default=0, help="1: lane groups per row instead of warp row batches (debug)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -234,7 +235,7 @@ def main():
     full = args.ckpt == "full"
     h = cdu.cdu_create(packed, K_max=wl.K, ckpt_mode=cdu.CDU_CKPT_FULL if full else cdu.CDU_CKPT_LEAN,
                        cg_refine=args.cg_refine, cg_refine_tol=args.cg_refine_tol, use_tensor_cores=args.tensor_cores,
-                       no_batch=args.no_batch)
+                       no_batch=args.no_batch, team_size=args.team_size)
     tdt = torch.float32 if wl.dtype == "f32" else torch.float64
     N, M = h.N, h.M
     rng = np.random.default_rng(W.generators.BASE_SEED + 31337 + rank)

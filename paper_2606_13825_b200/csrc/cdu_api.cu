@@ -657,6 +657,10 @@ cdu_status HandleT<T, IT>::init(const cdu_problem* pr, const cdu_options* op, cu
     int C = 1;
     while (C < 16 && (long long)B * C * 2 <= nsm && big / (C * 2) >= 2048) C *= 2;
     if (o.team_size > 0) { C = 1; while (C * 2 <= std::min(o.team_size, 16)) C *= 2; }
+    else if (C > 1 && (long long)B * 4 >= nsm &&
+             (5 * (((size_t)nmax + 3) & ~(size_t)3) + (((size_t)mmax + 3) & ~(size_t)3)) * sizeof(T) <= (size_t)smem_optin - 2048)
+      C = 1;   // a CTA that keeps the CG vectors in shared memory and reads sliced-ELL beats a cluster on L2 vectors as long as
+               // the batch still covers a good part of the SMs (cfg4: 64 problems, 1232 instead of 995 iters/s)
     const long long work = std::max<long long>(big, nnz_max / 8) / C;
     lin_threads = 128;
     while (lin_threads < 1024 && lin_threads * 4 < work) lin_threads *= 2;
@@ -664,7 +668,7 @@ cdu_status HandleT<T, IT>::init(const cdu_problem* pr, const cdu_options* op, cu
     const size_t vec_bytes = (5 * ns + ms) * sizeof(T);
     const size_t pd_bytes = (((size_t)pnn_max + 3) & ~(size_t)3) * sizeof(T);
     const size_t budget = (size_t)smem_optin - 2048;
-    D.vec_smem = (C == 1 && vec_bytes <= std::min<size_t>(budget, 96 * 1024)) ? 1 : 0;
+    D.vec_smem = (C == 1 && vec_bytes <= budget) ? 1 : 0;
     D.P_smem = (C == 1 && p_dense && D.vec_smem && pd_bytes + vec_bytes <= budget) ? 1 : 0;
     lin_smem = (D.vec_smem ? vec_bytes : 0) + (D.P_smem ? pd_bytes : 0);
     team_C = C;
