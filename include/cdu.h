@@ -95,7 +95,9 @@ cdu_status cdu_create(const cdu_problem* prob, const cdu_options* opts, void* cu
  * stream-ordered work, and the call returns without synchronising. If io_on_host != 0 they are HOST pointers
  * (pinned memory recommended); the library stages them through its own device buffers and returns after the
  * results have landed (stream synchronised).
- * Errors: CDU_EINVAL (K < 1, K > K_max, sigma <= 0, NULL rho/alpha; host-side rho <= 0 or alpha outside (0,2)). */
+ * Errors: CDU_EINVAL (K < 1, K > K_max, sigma <= 0, NULL rho/alpha; host-side rho <= 0 or alpha outside (0,2)).
+ * Device-resident rho / alpha cannot be read without a host sync: they are checked by a kernel that raises flag 16 on
+ * the problems they apply to; cdu_get_stats then returns CDU_ENUMERIC. */
 cdu_status cdu_forward(cdu_handle h, int32_t K, const void* rho, int32_t rho_mode, double sigma, const void* alpha,
                        const void* x0, const void* s0, const void* y0,
                        void* xK, void* sK, void* yK, int32_t io_on_host, void* cuda_stream);
@@ -113,14 +115,19 @@ typedef struct {
   int32_t cg_iters_max;      /* largest single-solve count                                                  */
   int32_t eig_sweeps_max;    /* largest Jacobi sweep count of a PSD block                                   */
   int32_t n_flagged;         /* problems with a flag set (CG cap hit, non-positive curvature, sweep cap, NaN) */
-  int32_t flags_or;          /* OR of all per-problem flag words: 1 CG cap, 2 pAp<=0, 4 eig sweep cap, 8 non-finite */
+  int32_t flags_or;          /* OR of all per-problem flag words: 1 CG cap, 2 pAp<=0, 4 eig sweep cap, 8 non-finite,
+                                16 rho <= 0 or alpha outside (0,2) (device-side check of device-resident hyper-parameters) */
   int64_t device_bytes;      /* bytes of device memory owned by the handle                                  */
   int64_t ckpt_bytes;        /* of which checkpoint store                                                   */
   int64_t launches;          /* kernel launches issued by the handle since creation                         */
   int64_t eig_sweeps_sum;    /* Jacobi sweeps summed over PSD blocks and iterations of the last forward     */
+  int64_t cg_iters_fwd_pass0; /* of cg_iters_fwd: iterations of the first pass (to cg_tol), i.e. without refinement */
+  int64_t cg_iters_bwd_pass0; /* same for cg_iters_bwd                                                       */
 } cdu_stats;
 
-/* Synchronises the stream of the last call and reads back the per-problem counters. */
+/* Synchronises the stream of the last call and reads back the per-problem counters. `out` is always filled; the return
+ * value is CDU_ENUMERIC when any per-problem flag is set (CG cap, non-positive curvature, eigen-sweep cap, non-finite
+ * value, rho <= 0 or alpha outside (0,2) detected on the device), CDU_OK otherwise. */
 cdu_status cdu_get_stats(cdu_handle h, cdu_stats* out);
 
 /* Copies iterate z^k (0 <= k <= K of the last forward) into caller buffers (device or host per io_on_host). */
@@ -148,6 +155,15 @@ cdu_status cdu_psd_project(int32_t dtype, int32_t count, int32_t p, const void* 
                            int32_t path, int32_t use_tensor_cores, void* cuda_stream);
 cdu_status cdu_psd_vjp(int32_t dtype, int32_t count, int32_t p, const void* U, const void* lam, const void* Gbar,
                        void* Sbar, int32_t path, int32_t use_tensor_cores, void* cuda_stream);
+
+/* ---- roofline denominators measured in-tree (bench.py) ---------------------------------------
+ * Runs a micro-benchmark on the current device and stream and returns its best-of-5 rate in *value:
+ *   CDU_PEAK_FP32_FMA / CDU_PEAK_FP64_FMA : dependent-chain-free FMA loops on the plain ALUs, TFLOP/s;
+ *   CDU_PEAK_TF32_TENSOR : back-to-back tcgen05.mma kind::tf32 (M128 N256 K8) from shared-memory operands, dense
+ *                          TFLOP/s of the tensor pipe (1 x TF32; the 3xTF32 products execute three of these per flop);
+ *   CDU_PEAK_HBM_COPY    : device-to-device copy of 1 GiB, GB/s (read + write). */
+typedef enum { CDU_PEAK_FP32_FMA = 0, CDU_PEAK_FP64_FMA = 1, CDU_PEAK_TF32_TENSOR = 2, CDU_PEAK_HBM_COPY = 3 } cdu_peak_kind;
+cdu_status cdu_measure_peak(int32_t kind, double* value, void* cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -27,7 +27,8 @@ CDU_CKPT_FULL, CDU_CKPT_LEAN = 0, 1
 _STATUS = {0: "CDU_OK", 1: "CDU_EINVAL", 2: "CDU_ENOMEM", 3: "CDU_ECUDA", 4: "CDU_ESTATE", 5: "CDU_ENUMERIC"}
 
 EXPORTED_SYMBOLS = ("cdu_create", "cdu_forward", "cdu_backward", "cdu_get_stats", "cdu_get_iterate", "cdu_last_error",
-                    "cdu_destroy", "cdu_version", "cdu_psd_project", "cdu_psd_vjp", "cdu_profile", "cdu_get_profile")
+                    "cdu_destroy", "cdu_version", "cdu_psd_project", "cdu_psd_vjp", "cdu_profile", "cdu_get_profile",
+                    "cdu_measure_peak")
 
 
 class CduError(RuntimeError):
@@ -58,7 +59,7 @@ class _Stats(C.Structure):
     _fields_ = [("cg_iters_fwd", C.c_int64), ("cg_iters_bwd", C.c_int64), ("cg_iters_max", C.c_int32),
                 ("eig_sweeps_max", C.c_int32), ("n_flagged", C.c_int32), ("flags_or", C.c_int32),
                 ("device_bytes", C.c_int64), ("ckpt_bytes", C.c_int64), ("launches", C.c_int64),
-                ("eig_sweeps_sum", C.c_int64)]
+                ("eig_sweeps_sum", C.c_int64), ("cg_iters_fwd_pass0", C.c_int64), ("cg_iters_bwd_pass0", C.c_int64)]
 
 
 _lib = None
@@ -98,6 +99,8 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.cdu_psd_project.argtypes = [i32, i32, i32, vp, vp, vp, vp, i32, i32, vp]
     lib.cdu_psd_vjp.restype = i32
     lib.cdu_psd_vjp.argtypes = [i32, i32, i32, vp, vp, vp, vp, i32, i32, vp]
+    lib.cdu_measure_peak.restype = i32
+    lib.cdu_measure_peak.argtypes = [i32, C.POINTER(C.c_double), vp]
     if path is None:
         _lib = lib
     return lib
@@ -199,9 +202,14 @@ class Handle:
         return out
 
     def stats(self) -> dict:
+        """cdu_get_stats. `status` is CDU_OK or CDU_ENUMERIC (some problem raised a flag: see `flags_or`)."""
         s = _Stats()
-        self._check(self.lib.cdu_get_stats(self.h, C.byref(s)))
-        return {k: getattr(s, k) for k, _ in _Stats._fields_}
+        st = self.lib.cdu_get_stats(self.h, C.byref(s))
+        if st not in (CDU_OK, CDU_ENUMERIC):
+            self._check(st)
+        d = {k: getattr(s, k) for k, _ in _Stats._fields_}
+        d["status"] = st
+        return d
 
     PROFILE_CLASSES = ("lin_fwd", "psd_fwd_small", "eig_large", "gemm_large", "lin_bwd", "psd_bwd_small", "large_misc", "misc")
 
@@ -245,6 +253,21 @@ def cdu_get_stats(h: Handle) -> dict:
 
 def cdu_destroy(h: Handle) -> None:
     h.close()
+
+
+CDU_PEAK_FP32_FMA, CDU_PEAK_FP64_FMA, CDU_PEAK_TF32_TENSOR, CDU_PEAK_HBM_COPY = range(4)
+
+
+def cdu_measure_peak(kind: int) -> float:
+    """In-tree micro-benchmark of a roofline denominator (TFLOP/s, or GB/s for the copy); see include/cdu.h."""
+    if not _torch().cuda.is_available():
+        raise CduError(CDU_ECUDA, "no CUDA device (there is no CPU fallback)")
+    lib = load_library()
+    v = C.c_double(0.0)
+    st = lib.cdu_measure_peak(kind, C.byref(v), _stream())
+    if st != CDU_OK:
+        raise CduError(st, "cdu_measure_peak failed")
+    return float(v.value)
 
 
 def cdu_psd_project(S, path: int = 0, use_tensor_cores: int = 0, want_eig: bool = True):

@@ -5,7 +5,7 @@
 
 namespace cdu {
 
-enum : int { FLAG_CG_CAP = 1, FLAG_CG_CURV = 2, FLAG_EIG_CAP = 4, FLAG_NONFINITE = 8 };
+enum : int { FLAG_CG_CAP = 1, FLAG_CG_CURV = 2, FLAG_EIG_CAP = 4, FLAG_NONFINITE = 8, FLAG_BAD_HYPER = 16 };
 enum : int { KIND_ZERO = 0, KIND_NONNEG = 1, KIND_SOC = 2, KIND_PSD = 3 };
 
 template <typename T> struct Eps;

@@ -112,7 +112,7 @@ __device__ __forceinline__ float gamma_relu_f(float li, float lj) {   // same ru
 
 // C[lb] (p x p, row-major) = A[lb] Bt[lb]'  (+ Hadamard with Gamma(lam) when lam != NULL). mapA / mapB: 3-D tensor maps
 // {p, p, nblk} of the fp32 operands, box {BK, TILE, 1}, 128-byte swizzle.
-__global__ void __launch_bounds__(THREADS, 1)
+static __global__ void __launch_bounds__(THREADS, 1)
 k_gemm_tc(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, float* __restrict__ C, int p,
           const float* __restrict__ lam) {
   extern __shared__ unsigned char smem_dyn[];
@@ -257,7 +257,7 @@ k_gemm_tc(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUte
 
 // Vt (rows = eigenvectors) -> V = Vt' and Vs = V diag(lam) (lam = the rebuild's scale vector): the K-major operands
 // of the rebuild Vs V' and of the products that contract over the eigenvector index. 32 x 32 tiles through shared memory.
-__global__ void __launch_bounds__(256) k_tc_transpose(int p, const float* __restrict__ Vt, const float* __restrict__ lam,
+static __global__ void __launch_bounds__(256) k_tc_transpose(int p, const float* __restrict__ Vt, const float* __restrict__ lam,
                                                       float* __restrict__ V, float* __restrict__ Vs) {
   __shared__ float tl[32][33];
   const size_t off = (size_t)blockIdx.z * p * p;

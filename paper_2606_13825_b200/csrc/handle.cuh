@@ -1,0 +1,1084 @@
+// handle.cuh - host driver behind include/cdu.h: handle, re-packing, the K-loop, the checkpoint store, BPTT.
+// Everything on the hot path runs in the kernels of lin.cuh / psd_small.cuh / psd_large.cuh / psd_bjacobi.cuh /
+// gemm_tc.cuh; this file only validates, allocates and launches. No CPU fallback exists. Included by the inst_*.cu
+// translation units, one per (value type, index type).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "cdu.h"
+#include "handle_base.h"
+#include "lin.cuh"
+#include "psd_large.cuh"
+#include "psd_bjacobi.cuh"
+#include "psd_small.cuh"
+#include "gemm_tc.cuh"
+
+namespace cdu {
+namespace impl {
+
+struct DevPool {  // owns device allocations
+  std::vector<void*> ptrs;
+  size_t bytes = 0;
+  cudaError_t last = cudaSuccess;
+  template <class U> U* alloc(size_t n) {
+    if (n == 0) n = 1;
+    void* p = nullptr;
+    last = cudaMalloc(&p, n * sizeof(U));
+    if (last != cudaSuccess) return nullptr;
+    ptrs.push_back(p);
+    bytes += n * sizeof(U);
+    return reinterpret_cast<U*>(p);
+  }
+  template <class U> U* upload(const std::vector<U>& h, cudaStream_t st) {
+    U* d = alloc<U>(h.size());
+    if (d && !h.empty()) last = cudaMemcpyAsync(d, h.data(), h.size() * sizeof(U), cudaMemcpyHostToDevice, st);
+    return d;
+  }
+  template <class U> U* zeros(size_t n, cudaStream_t st) {
+    U* d = alloc<U>(n);
+    if (d) last = cudaMemsetAsync(d, 0, std::max<size_t>(n, 1) * sizeof(U), st);
+    return d;
+  }
+  void release() {
+    for (void* p : ptrs) cudaFree(p);
+    ptrs.clear();
+    bytes = 0;
+  }
+  ~DevPool() { release(); }
+};
+
+// Optional per-kernel-class timing with CUDA events on the launching stream (bench.py's roofline leg).
+enum ProfClass { PC_LIN_FWD = 0, PC_PSD_FWD_SMALL, PC_EIG_LARGE, PC_GEMM_LARGE, PC_LIN_BWD, PC_PSD_BWD_SMALL, PC_LARGE_MISC, PC_MISC, PC_COUNT };
+static_assert(PC_COUNT == PROFILE_CLASSES, "profile classes of cdu.h");
+struct Prof {
+  bool on = false;
+  std::vector<cudaEvent_t> pool;
+  std::vector<int> cls;
+  size_t used = 0;
+  void begin(int c, cudaStream_t st) {
+    if (!on) return;
+    if (used + 2 > pool.size()) { cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b); pool.push_back(a); pool.push_back(b); }
+    cls.push_back(c);
+    cudaEventRecord(pool[used], st);
+  }
+  void end(cudaStream_t st) {
+    if (!on) return;
+    cudaEventRecord(pool[used + 1], st);
+    used += 2;
+  }
+  void collect(double* ms, long long* cnt) {
+    for (int i = 0; i < PC_COUNT; ++i) { ms[i] = 0; cnt[i] = 0; }
+    for (size_t i = 0; i < cls.size(); ++i) {
+      float t = 0.f;
+      cudaEventSynchronize(pool[2 * i + 1]);
+      cudaEventElapsedTime(&t, pool[2 * i], pool[2 * i + 1]);
+      ms[cls[i]] += t; cnt[cls[i]] += 1;
+    }
+    cls.clear(); used = 0;
+  }
+  ~Prof() { for (auto e : pool) cudaEventDestroy(e); }
+};
+
+inline int pow2_group(double avg) {
+  int g = 1;
+  while (g < 32 && g < avg * 0.5) g <<= 1;
+  return g;
+}
+
+#define CU_OK(call)                                                                       \
+  do {                                                                                    \
+    cudaError_t e_ = (call);                                                              \
+    if (e_ != cudaSuccess) {                                                              \
+      err = std::string(#call) + ": " + cudaGetErrorString(e_);                           \
+      return CDU_ECUDA;                                                                   \
+    }                                                                                     \
+  } while (0)
+
+// ---------------------------------------------------------------------------------------------------------
+// PSD engine: shared by the handle and the stand-alone operator entry points
+// ---------------------------------------------------------------------------------------------------------
+template <typename T>
+struct PsdEngine {
+  std::string err;
+  PsdTab tab{};
+  int nblk = 0, n_small = 0, n_large = 0, pmax_small = 0, pmax_large = 0;
+  int* d_small_list = nullptr;
+  LargeTab lt{};
+  int* lprob = nullptr;          // owning problem of each large block
+  T *G = nullptr, *Vt = nullptr, *Tm = nullptr, *T2 = nullptr, *mu = nullptr, *lamL = nullptr, *scaleL = nullptr;
+  double* chunk_scr = nullptr; unsigned* chunk_tick = nullptr;   // partials / tickets of the chunked glue kernels
+  T* lmaxL = nullptr;            // max |lambda| per large block, from the last eigendecomposition
+  double* wprev = nullptr;       // svec of the last matrix each large block decomposed
+  int eig_impl = 1;              // 1: blocked one-sided Jacobi (orders <= 512), 0: k_hestenes everywhere
+  bool warm = false;             // Vt holds the eigenvectors of the previous call (warm start of the next one)
+  int warm_enable = 1;
+  float* tc_split = nullptr;   // hi/lo operand staging of the tcgen05 path
+  int* rotflags = nullptr;
+  int* sweeps_max = nullptr;
+  unsigned long long* sweeps_sum = nullptr;
+  PsdSmallCfg scfg{1, 96};
+  int use_tc = 0;
+  long long launches = 0;
+  Prof* prof = nullptr;
+  void pb(int c, cudaStream_t st) { if (prof) prof->begin(c, st); }
+  void pe(cudaStream_t st) { if (prof) prof->end(st); }
+  std::vector<int> h_large_p;
+  size_t sum_p2 = 0, sum_p = 0;
+
+  cdu_status build(DevPool& pool, const std::vector<int>& prob, const std::vector<int>& row0, const std::vector<int>& p,
+                   int small_max, int want_tc, cudaStream_t st) {
+    nblk = (int)p.size();
+    std::vector<long long> uoff(nblk);
+    std::vector<int> loff(nblk), small_list, gblk, voff, lp;
+    std::vector<long long> moff;
+    long long mo = 0;
+    int vo = 0;
+    for (int i = 0; i < nblk; ++i) {
+      uoff[i] = (long long)sum_p2; loff[i] = (int)sum_p;
+      sum_p2 += (size_t)p[i] * p[i]; sum_p += p[i];
+      if (p[i] <= small_max) { small_list.push_back(i); pmax_small = std::max(pmax_small, p[i]); }
+      else { gblk.push_back(i); moff.push_back(mo); voff.push_back(vo); lp.push_back(p[i]); mo += (long long)p[i] * p[i]; vo += p[i]; pmax_large = std::max(pmax_large, p[i]); }
+    }
+    n_small = (int)small_list.size(); n_large = (int)gblk.size();
+    h_large_p = lp;
+    tab.nblk = nblk;
+    tab.prob = pool.upload(prob, st); tab.row0 = pool.upload(row0, st); tab.p = pool.upload(p, st);
+    tab.uoff = pool.upload(uoff, st); tab.loff = pool.upload(loff, st);
+    d_small_list = pool.upload(small_list, st);
+    sweeps_max = pool.zeros<int>(1, st);
+    sweeps_sum = pool.zeros<unsigned long long>(1, st);
+    if (n_large) {
+      lt.nblk = n_large; lt.pmax = pmax_large;
+      std::vector<long long> soff; long long so = 0;
+      for (int q : lp) { soff.push_back(so); so += (long long)q * (q + 1) / 2; }
+      lt.soff = pool.upload(soff, st); wprev = pool.zeros<double>((size_t)so, st);
+      { std::vector<int> lpv; for (int gb : gblk) lpv.push_back(prob[gb]); lprob = pool.upload(lpv, st); }
+      lt.gblk = pool.upload(gblk, st); lt.moff = pool.upload(moff, st); lt.voff = pool.upload(voff, st); lt.pvec = pool.upload(lp, st);
+      G = pool.alloc<T>(mo); Vt = pool.alloc<T>(mo); Tm = pool.alloc<T>(mo); T2 = pool.alloc<T>(mo);
+      mu = pool.alloc<T>(n_large); lamL = pool.alloc<T>(vo); scaleL = pool.alloc<T>(vo); lmaxL = pool.zeros<T>(n_large, st);
+      chunk_scr = pool.zeros<double>((size_t)n_large * LARGE_NCH * 2, st); chunk_tick = pool.zeros<unsigned>(n_large, st);
+      rotflags = pool.zeros<int>((size_t)n_large * HESTENES_MAXSW, st);
+      use_tc = (want_tc != 0) && std::is_same<T, float>::value && gemm_tc_supported(pmax_large) ? (want_tc < 0 ? 3 : want_tc) : 0;   // bit 0: rebuild, bit 1: DK products
+      for (int q : lp) if (q != pmax_large) use_tc = 0;      // the tensor maps assume one block order
+      if (use_tc) { tc_split = pool.alloc<float>((size_t)mo * 2); tcmaps.nblk = n_large; tcmaps.p = pmax_large; }
+      if (!G || !Vt || !Tm || !T2 || !mu || !lamL || !rotflags) { err = "cudaMalloc (PSD large scratch)"; return CDU_ENOMEM; }
+    }
+    if (pool.last != cudaSuccess) { err = std::string("PSD tables: ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
+    if (n_small) {
+      const size_t sb = psd_small_smem_bytes(pmax_small, sizeof(T));
+      scfg = psd_small_cfg(pmax_small, sizeof(T));
+      if (sb > 227 * 1024 || scfg.maxi > PSD_SMALL_MAXI) { err = "psd_small_max too large for shared memory"; return CDU_EINVAL; }
+      const void* fn[8] = {(const void*)k_psd_fwd_small<T, 1>, (const void*)k_psd_fwd_small<T, 2>, (const void*)k_psd_fwd_small<T, 3>,
+                           (const void*)k_psd_fwd_small<T, 4>, (const void*)k_psd_bwd_small<T, 1>, (const void*)k_psd_bwd_small<T, 2>,
+                           (const void*)k_psd_bwd_small<T, 3>, (const void*)k_psd_bwd_small<T, 4>};
+      for (const void* f : fn) CU_OK(cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb));
+    }
+    return CDU_OK;
+  }
+  void launch_small_fwd(const Hyper<T>& H, int k, const PsdFwdArgs& A, cudaStream_t st) {
+    const size_t sm = psd_small_smem_bytes(pmax_small, sizeof(T));
+    if (scfg.maxi == 1) k_psd_fwd_small<T, 1><<<n_small, scfg.threads, sm, st>>>(tab, H, k, A, d_small_list);
+    else if (scfg.maxi == 2) k_psd_fwd_small<T, 2><<<n_small, scfg.threads, sm, st>>>(tab, H, k, A, d_small_list);
+    else if (scfg.maxi == 3) k_psd_fwd_small<T, 3><<<n_small, scfg.threads, sm, st>>>(tab, H, k, A, d_small_list);
+    else k_psd_fwd_small<T, 4><<<n_small, scfg.threads, sm, st>>>(tab, H, k, A, d_small_list);
+  }
+  void launch_small_bwd(const Hyper<T>& H, int k, const PsdBwdArgs& A, cudaStream_t st) {
+    const size_t sm = psd_small_smem_bytes(pmax_small, sizeof(T));
+    if (scfg.maxi == 1) k_psd_bwd_small<T, 1><<<n_small, scfg.threads, sm, st>>>(tab, H, k, A, d_small_list);
+    else if (scfg.maxi == 2) k_psd_bwd_small<T, 2><<<n_small, scfg.threads, sm, st>>>(tab, H, k, A, d_small_list);
+    else if (scfg.maxi == 3) k_psd_bwd_small<T, 3><<<n_small, scfg.threads, sm, st>>>(tab, H, k, A, d_small_list);
+    else k_psd_bwd_small<T, 4><<<n_small, scfg.threads, sm, st>>>(tab, H, k, A, d_small_list);
+  }
+
+  cdu_status gemm(const T* A, int ta, const T* Bm, int tb, T* C, const T* kscale, int relu, cudaStream_t st) {
+    pb(PC_GEMM_LARGE, st);
+    cdu_status s = gemm_(A, ta, Bm, tb, C, kscale, relu, st);
+    pe(st);
+    return s;
+  }
+  cdu_status gemm_(const T* A, int ta, const T* Bm, int tb, T* C, const T* kscale, int relu, cudaStream_t st) {
+    const int tiles = (pmax_large + 63) / 64;
+    k_gemm_fma<T><<<dim3(tiles, tiles, n_large), 256, 0, st>>>(n_large, lt.pvec, lt.moff, lt.voff, A, ta, Bm, tb, C, kscale, relu);
+    ++launches;
+    CU_OK(cudaGetLastError());
+    return CDU_OK;
+  }
+
+  // tcgen05 path (fp32 handles, uniform block order, multiple of 128): C = A Bt' per block, see gemm_tc.cuh
+  tc::Maps tcmaps;
+  cdu_status gemm_nt(const T* A, const T* Bt, T* C, const T* lam, cudaStream_t st) {
+    pb(PC_GEMM_LARGE, st);
+    cdu_status s = tc::gemm_nt(tcmaps, (const float*)A, (const float*)Bt, (float*)C, (const float*)lam, st, err);
+    pe(st);
+    ++launches;
+    return s;
+  }
+  cdu_status tc_transpose(const T* lam, cudaStream_t st) {   // tc_split[0] = V = Vt', tc_split[1] = V diag(lam+)
+    const int p = pmax_large;
+    pb(PC_LARGE_MISC, st);
+    tc::k_tc_transpose<<<dim3(p / 32, p / 32, n_large), 256, 0, st>>>(p, (const float*)Vt, (const float*)lam, tc_split,
+                                                                     lam ? tc_split + (size_t)n_large * p * p : nullptr);
+    pe(st);
+    ++launches;
+    CU_OK(cudaGetLastError());
+    return CDU_OK;
+  }
+
+  // blocked one-sided Jacobi (psd_bjacobi.cuh): one pair of row blocks per CTA and round, cluster size chosen from what the
+  // device can co-schedule. fp32: tensor-core variant (32 rows per pair); fp64: FMA variant (16 rows per pair).
+  cdu_status eig_blocked(cudaStream_t st, int* flags) {
+    constexpr bool F32 = std::is_same<T, float>::value;
+    constexpr int RP = F32 ? 32 : 16;
+    const int BR = RP / 2, NB = (pmax_large + BR - 1) / BR, NP = ((NB + 1) & ~1) / 2;
+    const size_t smem = F32 ? bj::tcv::smem_bytes(pmax_large) : bj::smem_bytes<T, RP>(pmax_large);
+    const void* kern;
+    if constexpr (F32) kern = (const void*)bj::tcv::k_bjacobi_tc; else kern = (const void*)bj::k_bjacobi<T, 16>;
+    if (bj_C == 0) {
+      CU_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      CU_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+      long long best = -1;
+      for (int C = 16; C >= 1; C >>= 1) {
+        if (C > 1 && C / 2 >= NP) continue;                // smaller cluster already covers all pairs
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(n_large * C); cfg.blockDim = dim3(bj::THREADS); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int active = 0;
+        if (cudaOccupancyMaxActiveClusters(&active, kern, &cfg) != cudaSuccess || active < 1) { cudaGetLastError(); continue; }
+        const long long cost = (long long)((n_large + active - 1) / active) * ((NP + C - 1) / C);
+        if (best < 0 || cost < best) { best = cost; bj_C = C; }
+      }
+      if (bj_C == 0) { err = "k_bjacobi: no launchable cluster size"; return CDU_ECUDA; }
+    }
+    CU_OK(cudaMemsetAsync(rotflags, 0, (size_t)n_large * bj::MAXSW * sizeof(int), st));
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(n_large * bj_C); cfg.blockDim = dim3(bj::THREADS); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = bj_C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    double tol = F32 ? 3e-7 : 1e-15;
+    int nl = n_large, maxsw = bj::MAXSW - 1;
+    const int* pv = lt.pvec; const long long* mo = lt.moff; const int* vo = lt.voff; const int* lp = lprob;
+    T *g = G, *v = Vt, *l = lamL; const T* m = mu; int* rf = rotflags; int* sw = sweeps_max; unsigned long long* ss = sweeps_sum;
+    void* args[] = {&nl, &pv, &mo, &vo, &g, &v, &m, &l, &rf, &sw, &ss, &maxsw, &tol, &lp, &flags};
+    pb(PC_EIG_LARGE, st);
+    cudaError_t e = cudaLaunchKernelExC(&cfg, kern, args);
+    pe(st);
+    ++launches;
+    CU_OK(e);
+    return CDU_OK;
+  }
+  int bj_C = 0;
+
+  cdu_status eig_large(cudaStream_t st, int* flags) {   // G = Vt (S + mu I), Vt orthonormal (I on a cold start)  ->  Vt, lamL
+    if (eig_impl == 1 && pmax_large <= 512) return eig_blocked(st, flags);
+    CU_OK(cudaMemsetAsync(rotflags, 0, (size_t)n_large * HESTENES_MAXSW * sizeof(int), st));
+    const int C = 8;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(n_large * C); cfg.blockDim = dim3(512); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    const double tol = std::is_same<T, float>::value ? 3e-7 : 1e-15;
+    const int maxsw = HESTENES_MAXSW - 1;
+    int nl = n_large;
+    const int* pv = lt.pvec; const long long* mo = lt.moff; const int* vo = lt.voff;
+    T *g = G, *v = Vt, *l = lamL; const T* m = mu; int* rf = rotflags; int* sw = sweeps_max; unsigned long long* ss = sweeps_sum;
+    const int* lp = lprob;
+    cudaError_t e;
+    pb(PC_EIG_LARGE, st);
+    if (pmax_large <= 128) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 4>, nl, pv, mo, vo, g, v, m, l, rf, sw, ss, maxsw, tol, lp, flags);
+    else if (pmax_large <= 256) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 8>, nl, pv, mo, vo, g, v, m, l, rf, sw, ss, maxsw, tol, lp, flags);
+    else if (pmax_large <= 512) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 16>, nl, pv, mo, vo, g, v, m, l, rf, sw, ss, maxsw, tol, lp, flags);
+    else if (pmax_large <= 1024) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 32>, nl, pv, mo, vo, g, v, m, l, rf, sw, ss, maxsw, tol, lp, flags);
+    else { err = "PSD block order > 1024 not supported"; return CDU_EINVAL; }
+    pe(st);
+    ++launches;
+    CU_OK(e);
+    return CDU_OK;
+  }
+
+  // Eigendecomposition of smat(w) for every large block. Cold: G = S + mu I, Vt = I. Warm (Vt = eigenvectors left by
+  // the previous call, nearby because consecutive ADMM iterates are): Tm = S + mu I, G = Vt Tm, so the Jacobi sweeps
+  // start from an almost orthogonal G.
+  cdu_status eig_of_w(const Hyper<T>& H, int k, const double* Wv, int* flags, cudaStream_t st) {
+    const bool w = warm && warm_enable;
+    pb(PC_LARGE_MISC, st);
+    const bool rq = eig_impl == 1 && pmax_large <= 512;   // blocked Jacobi: eigenvalues by Rayleigh quotient afterwards
+    if (w) k_large_smat<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, Wv, nullptr, H, k, 0, 2, Tm, nullptr, mu, wprev, lmaxL, rq ? T2 : nullptr, chunk_scr, chunk_tick, flags);
+    else k_large_smat<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, Wv, nullptr, H, k, 0, 1, G, Vt, mu, wprev, lmaxL, rq ? T2 : nullptr, chunk_scr, chunk_tick, flags);
+    pe(st);
+    ++launches;
+    CU_OK(cudaGetLastError());
+    cdu_status s;
+    if (w) {
+      if (use_tc) s = gemm_nt(Vt, Tm, G, nullptr, st);       // Tm is symmetric: Vt Tm = Vt Tm'
+      else s = gemm(Vt, 0, Tm, 0, G, nullptr, 0, st);
+      if (s != CDU_OK) return s;
+    }
+    s = eig_large(st, flags);
+    if (s != CDU_OK) return s;
+    if (rq) {
+      if (use_tc) s = gemm_nt(Vt, T2, G, nullptr, st);       // R = Vt S (S symmetric)
+      else s = gemm(Vt, 0, T2, 0, G, nullptr, 0, st);
+      if (s != CDU_OK) return s;
+      pb(PC_LARGE_MISC, st);
+      k_large_rayleigh<T><<<dim3(16, n_large), 256, 0, st>>>(lt.pvec, lt.moff, lt.voff, G, Vt, lamL);
+      pe(st);
+      ++launches;
+    }
+    pb(PC_LARGE_MISC, st);
+    k_large_post<T><<<n_large, 256, 0, st>>>(lt.pvec, lt.voff, lamL, scaleL, lmaxL);
+    pe(st);
+    ++launches;
+    CU_OK(cudaGetLastError());
+    warm = true;
+    return CDU_OK;
+  }
+
+  cdu_status forward(const Hyper<T>& H, int k, const PsdFwdArgs& A, cudaStream_t st) {
+    if (n_small) {
+      pb(PC_PSD_FWD_SMALL, st);
+      launch_small_fwd(H, k, A, st);
+      pe(st);
+      ++launches;
+      CU_OK(cudaGetLastError());
+    }
+    if (n_large) {
+      cdu_status s = eig_of_w(H, k, A.W, A.flags, st);
+      if (s != CDU_OK) return s;
+      if (use_tc & 1) {
+        if ((s = tc_transpose(scaleL, st)) != CDU_OK) return s;
+        s = gemm_nt((const T*)(tc_split + (size_t)n_large * pmax_large * pmax_large), (const T*)tc_split, Tm, nullptr, st);   // Tm = (V diag(lam+)) V'
+      } else {
+        s = gemm(Vt, 1, Vt, 0, Tm, scaleL, 0, st);        // Tm = Vt' diag(scale) Vt
+      }
+      if (s != CDU_OK) return s;
+      pb(PC_LARGE_MISC, st);
+      k_large_finish_fwd<T><<<dim3(64, n_large), 256, 0, st>>>(tab, lt, H, k, Tm, Vt, lamL, A);
+      pe(st);
+      ++launches;
+      CU_OK(cudaGetLastError());
+    }
+    return CDU_OK;
+  }
+
+  cdu_status backward(const Hyper<T>& H, int k, const PsdBwdArgs& A, cudaStream_t st) {
+    if (n_small) {
+      pb(PC_PSD_BWD_SMALL, st);
+      launch_small_bwd(H, k, A, st);
+      pe(st);
+      ++launches;
+      CU_OK(cudaGetLastError());
+    }
+    if (n_large) {
+      if (A.recompute) {
+        cdu_status s = eig_of_w(H, k, A.W, A.flags, st);
+        if (s != CDU_OK) return s;
+      } else {
+        pb(PC_LARGE_MISC, st);
+      k_large_fetch<T><<<dim3(64, n_large), 256, 0, st>>>(tab, lt, (const T*)A.Ustore, (const T*)A.Lstore, Vt, lamL);
+      pe(st);
+        ++launches;
+        CU_OK(cudaGetLastError());
+      }
+      pb(PC_LARGE_MISC, st);
+      k_large_smat<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, A.Gs, A.Gy, H, k, 1, 0, G, nullptr, nullptr, nullptr, nullptr, nullptr, chunk_scr, chunk_tick, nullptr);   // G = smat(g_s + rho g_y)
+      pe(st);
+      ++launches;
+      CU_OK(cudaGetLastError());
+      cdu_status s;
+      if (use_tc & 2) {   // every product as A Bt' with both operands row-major: G and C o Gamma are symmetric, V = Vt'
+        const T* V = (const T*)tc_split;
+        if ((s = tc_transpose(nullptr, st)) != CDU_OK) return s;
+        if ((s = gemm_nt(Vt, G, Tm, nullptr, st)) != CDU_OK) return s;         // Tm = Vt G
+        if ((s = gemm_nt(Tm, Vt, G, lamL, st)) != CDU_OK) return s;            // C  = (Tm Vt') o Gamma   (Hadamard in the epilogue)
+        if ((s = gemm_nt(V, G, Tm, nullptr, st)) != CDU_OK) return s;          // Tm = Vt' C
+        if ((s = gemm_nt(Tm, V, G, nullptr, st)) != CDU_OK) return s;          // out = Tm Vt
+        pb(PC_LARGE_MISC, st);
+        k_large_finish_bwd<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, H, k, G, A, chunk_scr, chunk_tick);
+        pe(st);
+        ++launches;
+        CU_OK(cudaGetLastError());
+        return CDU_OK;
+      }
+      if ((s = gemm(Vt, 0, G, 0, Tm, nullptr, 0, st)) != CDU_OK) return s;     // Tm = Vt G
+      if ((s = gemm(Tm, 0, Vt, 1, G, nullptr, 0, st)) != CDU_OK) return s;     // C  = Tm Vt'
+      pb(PC_LARGE_MISC, st);
+      k_large_hadamard<T><<<dim3(64, n_large), 256, 0, st>>>(n_large, lt.pvec, lt.moff, lt.voff, G, lamL);
+      pe(st);
+      ++launches;
+      CU_OK(cudaGetLastError());
+      if ((s = gemm(Vt, 1, G, 0, Tm, nullptr, 0, st)) != CDU_OK) return s;     // Tm = Vt' C
+      if ((s = gemm(Tm, 0, Vt, 0, G, nullptr, 0, st)) != CDU_OK) return s;     // out = Tm Vt
+      pb(PC_LARGE_MISC, st);
+      k_large_finish_bwd<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, H, k, G, A, chunk_scr, chunk_tick);
+      pe(st);
+      ++launches;
+      CU_OK(cudaGetLastError());
+    }
+    return CDU_OK;
+  }
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// handle
+// ---------------------------------------------------------------------------------------------------------
+template <typename T, typename IT>
+struct HandleT : cdu_handle_s {
+  DevPool pool;
+  BatchDev<T, IT> D{};
+  int team_C = 1, lin_grid = 1;      // CTAs per team (cluster size), persistent grid size
+  size_t lin_smem = 0;               // dynamic shared memory of the linear-step kernels
+  PsdEngine<T> psd;
+  int B = 0, K_max = 0, ckpt_mode = 0, lin_threads = 256;
+  long long N = 0, Mtot = 0;
+  size_t zstride = 0;
+  double* Z = nullptr;       // [(K_max+1)][N + 2 Mtot]
+  double* XT = nullptr;      // FULL: [K_max][N], LEAN: [N]
+  double* ST = nullptr;      // FULL: [K_max][Mtot], LEAN: [Mtot]
+  T* Ustore = nullptr;       // FULL: [K_max][sum p^2], LEAN: one slot
+  T* Lstore = nullptr;
+  double* GZ[2] = {nullptr, nullptr};
+  double *g_rho_pb = nullptr, *g_alpha_pb = nullptr, *g_sigma_pb = nullptr, *part_pre = nullptr;
+  T *d_rho = nullptr, *d_alpha = nullptr;
+  T* stage = nullptr;        // host-I/O staging, N + 2 Mtot (+ gradient outputs)
+  T* stage_g = nullptr;      // 2 K_max B + B
+  int *cg_f = nullptr, *cg_b = nullptr, *cg_f0 = nullptr, *cg_b0 = nullptr, *cg_max = nullptr, *flags = nullptr;
+  int K_last = 0, mode_last = 0;
+  double sigma_last = 0;
+  size_t ckpt_bytes = 0;
+  long long launches = 0;
+  cudaStream_t last_stream = nullptr;
+  bool has_psd = false;
+  Prof prof;
+
+  double* z_at(int k) { return Z + (size_t)k * zstride; }
+
+  // One launch of a linear-step kernel over the whole batch: persistent CTAs (team_C == 1) or clusters of team_C CTAs.
+  template <typename... Args>
+  cudaError_t launch_lin(void (*single)(Args...), void (*multi)(Args...), cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(lin_grid); cfg.blockDim = dim3(lin_threads); cfg.dynamicSmemBytes = lin_smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    if (team_C > 1) {
+      at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = team_C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      return cudaLaunchKernelEx(&cfg, multi, args...);
+    }
+    return cudaLaunchKernelEx(&cfg, single, args...);
+  }
+
+  cdu_status init(const cdu_problem* pr, const cdu_options* op, cudaStream_t st);
+  Hyper<T> hyper() const {
+    Hyper<T> H;
+    H.rho = d_rho; H.alpha = d_alpha; H.sigma = sigma_last;
+    H.kstride = mode_last == CDU_RHO_PER_ITER ? 1 : B; H.pstride = mode_last == CDU_RHO_PER_ITER ? 0 : 1;
+    return H;
+  }
+  cdu_status forward(int K, const void* rho, int mode, double sigma, const void* alpha, const void* x0, const void* s0,
+                     const void* y0, void* xK, void* sK, void* yK, int host, cudaStream_t st) override;
+  cdu_status backward(const void* gx, const void* gs, const void* gy, void* g_rho, void* g_sigma, void* g_alpha,
+                      void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st) override;
+  cdu_status stats(cdu_stats* out) override;
+  cdu_status iterate(int k, void* x, void* s, void* y, int host, cudaStream_t st) override;
+  void profile_enable(int on) override { prof.on = on != 0; }
+  void profile_collect(double* ms, long long* cnt) override { prof.collect(ms, cnt); }
+  cudaStream_t stream_of_last_call() const override { return last_stream; }
+  cdu_status export_state(const double* z, void* x, void* s, void* y, int host, cudaStream_t st);
+  cdu_status import_state(double* z, const void* x, const void* s, const void* y, int host, cudaStream_t st);
+};
+
+template <typename T, typename IT>
+cdu_status HandleT<T, IT>::init(const cdu_problem* pr, const cdu_options* op, cudaStream_t st) {
+  B = pr->batch;
+  if (B < 1 || !pr->var_off || !pr->row_off || !pr->A_rowptr || !pr->P_rowptr || !pr->cone_off || !pr->cones || !pr->q || !pr->b) {
+    err = "cdu_create: NULL array or batch < 1"; return CDU_EINVAL;
+  }
+  if (pr->var_off[0] != 0 || pr->row_off[0] != 0 || pr->cone_off[0] != 0) { err = "cdu_create: offsets must start at 0"; return CDU_EINVAL; }
+  for (int b = 0; b < B; ++b)
+    if (pr->var_off[b + 1] <= pr->var_off[b] || pr->row_off[b + 1] < pr->row_off[b] || pr->cone_off[b + 1] < pr->cone_off[b]) {
+      err = "cdu_create: offsets must be increasing (n_b >= 1)"; return CDU_EINVAL;
+    }
+  N = pr->var_off[B]; Mtot = pr->row_off[B];
+  const long long nnzA = pr->A_rowptr[Mtot], nnzP = pr->P_rowptr[N];
+  if (N >= (1LL << 31) || Mtot >= (1LL << 31) || nnzA >= (1LL << 31) || nnzP >= (1LL << 31) || nnzA < 0 || nnzP < 0) {
+    err = "cdu_create: sizes exceed int32 range"; return CDU_EINVAL;
+  }
+  if ((nnzA && (!pr->A_colidx || !pr->A_val)) || (nnzP && (!pr->P_colidx || !pr->P_val))) { err = "cdu_create: NULL CSR arrays"; return CDU_EINVAL; }
+  cdu_options o{};
+  if (op) o = *op;
+  else { o.cg_refine = -1; o.use_tensor_cores = -1; o.team_size = 0; o.no_batch = 0; }
+  if (o.K_max < 1) { err = "cdu_create: options.K_max must be >= 1"; return CDU_EINVAL; }
+  const bool f32 = std::is_same<T, float>::value;
+  K_max = o.K_max; ckpt_mode = o.ckpt_mode == CDU_CKPT_LEAN ? CDU_CKPT_LEAN : CDU_CKPT_FULL;
+  const int small_max = o.psd_small_max > 0 ? o.psd_small_max : (f32 ? 128 : 88);
+
+  // ---- cones ------------------------------------------------------------------------------------------
+  std::vector<uint8_t> rowkind((size_t)Mtot);
+  std::vector<int> soc_off(B + 1, 0), soc_start, soc_dim, psdblk_off(B + 1, 0), psd_prob, psd_row0, psd_p;
+  int nmax = 0, mmax = 0;
+  for (int b = 0; b < B; ++b) {
+    const long long r0 = pr->row_off[b], m = pr->row_off[b + 1] - r0;
+    nmax = std::max<long long>(nmax, pr->var_off[b + 1] - pr->var_off[b]); mmax = std::max<long long>(mmax, m);
+    long long r = 0;
+    for (long long c = pr->cone_off[b]; c < pr->cone_off[b + 1]; ++c) {
+      const int kind = pr->cones[c].kind, dim = pr->cones[c].dim;
+      if (dim < 1 || kind < 0 || kind > 3) { err = "cdu_create: bad cone"; return CDU_EINVAL; }
+      const long long rows = kind == CDU_PSD ? (long long)dim * (dim + 1) / 2 : dim;
+      if (r + rows > m) { err = "cdu_create: cones exceed the rows of a problem"; return CDU_EINVAL; }
+      if (kind == CDU_SOC) { soc_start.push_back((int)r); soc_dim.push_back(dim); }
+      if (kind == CDU_PSD) { psd_prob.push_back(b); psd_row0.push_back((int)(r0 + r)); psd_p.push_back(dim); }
+      std::fill(rowkind.begin() + r0 + r, rowkind.begin() + r0 + r + rows, (uint8_t)kind);
+      r += rows;
+    }
+    if (r != m) { err = "cdu_create: cones do not tile the rows of a problem"; return CDU_EINVAL; }
+    soc_off[b + 1] = (int)soc_start.size(); psdblk_off[b + 1] = (int)psd_p.size();
+  }
+  has_psd = !psd_p.empty();
+
+  // ---- CSR re-packing: int32 rowptr, transposed copy, diag(P), column square sums ----------------------------
+  const T* Av = reinterpret_cast<const T*>(pr->A_val);
+  const T* Pv = reinterpret_cast<const T*>(pr->P_val);
+  std::vector<int> A_rp((size_t)Mtot + 1), P_rp((size_t)N + 1), AT_rp((size_t)N + 1, 0);
+  std::vector<IT> A_ci((size_t)nnzA), AT_ci((size_t)nnzA), P_ci;
+  std::vector<T> AT_v((size_t)nnzA), diagP((size_t)N, (T)0), colsq((size_t)N, (T)0);
+  std::vector<long long> P_off(B, 0);
+  for (long long i = 0; i <= Mtot; ++i) A_rp[i] = (int)pr->A_rowptr[i];
+  for (long long i = 0; i <= N; ++i) P_rp[i] = (int)pr->P_rowptr[i];
+  for (long long i = 0; i < Mtot; ++i) if (A_rp[i + 1] < A_rp[i]) { err = "cdu_create: A_rowptr not monotone"; return CDU_EINVAL; }
+  for (long long i = 0; i < N; ++i) if (P_rp[i + 1] < P_rp[i]) { err = "cdu_create: P_rowptr not monotone"; return CDU_EINVAL; }
+  bool p_dense = nnzP > 0;      // every P_b stored as all n_b^2 entries with sorted columns -> no index array needed
+  long long nnz_max = 0, pnn_max = 0;
+  {
+    std::vector<double> csq((size_t)N, 0.0);
+    for (int b = 0; b < B; ++b) {
+      const long long v0 = pr->var_off[b], n = pr->var_off[b + 1] - v0, r0 = pr->row_off[b], r1 = pr->row_off[b + 1];
+      nnz_max = std::max<long long>(nnz_max, A_rp[r1] - A_rp[r0]);
+      for (long long e = A_rp[r0]; e < A_rp[r1]; ++e) {
+        const int c = pr->A_colidx[e];
+        if (c < 0 || c >= n) { err = "cdu_create: A column index out of range"; return CDU_EINVAL; }
+        A_ci[e] = (IT)c;
+        ++AT_rp[v0 + c + 1];
+      }
+    }
+    for (long long i = 0; i < N; ++i) AT_rp[i + 1] += AT_rp[i];
+    std::vector<int> fill(AT_rp.begin(), AT_rp.end() - 1);
+    for (int b = 0; b < B; ++b) {
+      const long long v0 = pr->var_off[b], r0 = pr->row_off[b], r1 = pr->row_off[b + 1];
+      for (long long r = r0; r < r1; ++r)
+        for (long long e = A_rp[r]; e < A_rp[r + 1]; ++e) {
+          const long long col = v0 + pr->A_colidx[e];
+          const int dst = fill[col]++;
+          AT_ci[dst] = (IT)(r - r0);
+          AT_v[dst] = Av[e];
+          csq[col] += (double)Av[e] * (double)Av[e];
+        }
+      const long long n = pr->var_off[b + 1] - v0;
+      P_off[b] = P_rp[v0];
+      pnn_max = std::max<long long>(pnn_max, P_rp[v0 + n] - P_rp[v0]);
+      if (P_rp[v0 + n] - P_rp[v0] != n * n) p_dense = false;
+      for (long long i = 0; i < n; ++i) {
+        if (P_rp[v0 + i + 1] - P_rp[v0 + i] != n) p_dense = false;
+        for (long long e = P_rp[v0 + i]; e < P_rp[v0 + i + 1]; ++e) {
+          const int c = pr->P_colidx[e];
+          if (c < 0 || c >= n) { err = "cdu_create: P column index out of range"; return CDU_EINVAL; }
+          if (c != e - P_rp[v0 + i]) p_dense = false;
+          if (c == i) diagP[v0 + i] += Pv[e];
+        }
+      }
+    }
+    for (long long i = 0; i < N; ++i) colsq[i] = (T)csq[i];
+  }
+  if (!p_dense) { P_ci.resize((size_t)nnzP); for (long long e = 0; e < nnzP; ++e) P_ci[e] = (IT)pr->P_colidx[e]; }
+  std::vector<int> var_off32(B + 1), row_off32(B + 1);
+  for (int b = 0; b <= B; ++b) { var_off32[b] = (int)pr->var_off[b]; row_off32[b] = (int)pr->row_off[b]; }
+
+  // ---- upload -------------------------------------------------------------------------------------------
+  D.B = B; D.N = N; D.Mtot = Mtot;
+  D.var_off = pool.upload(var_off32, st); D.row_off = pool.upload(row_off32, st);
+  D.A_rp = pool.upload(A_rp, st); D.P_rp = pool.upload(P_rp, st); D.AT_rp = pool.upload(AT_rp, st);
+  {
+    T* v = pool.alloc<T>(nnzA); T* pv = pool.alloc<T>(nnzP);
+    T* q = pool.alloc<T>(N); T* bb = pool.alloc<T>(Mtot);
+    if (!v || !pv || !q || !bb) { err = "cudaMalloc (problem data)"; return CDU_ENOMEM; }
+    if (nnzA) CU_OK(cudaMemcpyAsync(v, Av, nnzA * sizeof(T), cudaMemcpyHostToDevice, st));
+    if (nnzP) CU_OK(cudaMemcpyAsync(pv, Pv, nnzP * sizeof(T), cudaMemcpyHostToDevice, st));
+    CU_OK(cudaMemcpyAsync(q, pr->q, N * sizeof(T), cudaMemcpyHostToDevice, st));
+    if (Mtot) CU_OK(cudaMemcpyAsync(bb, pr->b, Mtot * sizeof(T), cudaMemcpyHostToDevice, st));
+    D.A_v = v; D.P_v = pv; D.q = q; D.b = bb;
+  }
+  D.A_ci = pool.upload(A_ci, st); D.P_ci = pool.upload(P_ci, st);
+  D.AT_ci = pool.upload(AT_ci, st); D.AT_v = pool.upload(AT_v, st);
+  D.P_dense = p_dense ? 1 : 0; D.P_off = pool.upload(P_off, st);
+  D.diagP = pool.upload(diagP, st); D.colsq = pool.upload(colsq, st);
+  D.rowkind = pool.upload(rowkind, st);
+  D.soc_off = pool.upload(soc_off, st); D.soc_start = pool.upload(soc_start, st); D.soc_dim = pool.upload(soc_dim, st);
+  D.psdblk_off = pool.upload(psdblk_off, st);
+  D.A_G = pow2_group((double)nnzA / std::max<long long>(Mtot, 1));
+  D.AT_G = pow2_group((double)nnzA / (double)N);
+  D.P_G = pow2_group((double)nnzP / (double)N);
+  // scratch
+  D.xi = pool.alloc<double>(N); D.rd = pool.alloc<double>(N); D.lam = pool.alloc<double>(N);
+  D.tm = pool.alloc<double>(Mtot); D.W = pool.alloc<double>(Mtot); D.GW = pool.alloc<double>(Mtot);
+  D.r = pool.alloc<T>(N); D.p = pool.alloc<T>(N); D.Ap = pool.alloc<T>(N); D.d = pool.alloc<T>(N); D.dinv = pool.alloc<T>(N);
+  D.tA = pool.alloc<T>(Mtot);
+  D.tol = o.cg_tol > 0 ? o.cg_tol : (f32 ? 1e-6 : 1e-10);
+  D.tol_ref = o.cg_refine_tol > 0 ? o.cg_refine_tol : 1e-4;
+  D.refine = o.cg_refine >= 0 ? o.cg_refine : (f32 ? 1 : 0);
+  D.maxit = o.cg_max_iter > 0 ? o.cg_max_iter : 2 * nmax + 50;
+  cg_f = pool.zeros<int>(B, st); cg_b = pool.zeros<int>(B, st); cg_f0 = pool.zeros<int>(B, st); cg_b0 = pool.zeros<int>(B, st); cg_max = pool.zeros<int>(B, st); flags = pool.zeros<int>(B, st);
+  D.cg_iters = cg_f; D.cg_iters0 = cg_f0; D.cg_max = cg_max; D.flags = flags;
+  if (pool.last != cudaSuccess) { err = std::string("cdu_create: ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
+
+  // ---- team shape (lin.cuh): cluster size, CTA size, shared-memory residency, persistent grid -----------------
+  {
+    int dev = 0, nsm = 148, smem_optin = 227 * 1024;
+    CU_OK(cudaGetDevice(&dev));
+    CU_OK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    CU_OK(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    const long long big = std::max(nmax, mmax);
+    int C = 1;
+    while (C < 16 && (long long)B * C * 2 <= nsm && big / (C * 2) >= 2048) C *= 2;
+    if (o.team_size > 0) { C = 1; while (C * 2 <= std::min(o.team_size, 16)) C *= 2; }
+    else if (C > 1 && (long long)B * 4 >= nsm &&
+             (5 * (((size_t)nmax + 3) & ~(size_t)3) + (((size_t)mmax + 3) & ~(size_t)3)) * sizeof(T) <= (size_t)smem_optin - 2048)
+      C = 1;   // a CTA that keeps the CG vectors in shared memory and reads sliced-ELL beats a cluster on L2 vectors as long as
+               // the batch still covers a good part of the SMs (cfg4: 64 problems, 1232 instead of 995 iters/s)
+    const long long work = std::max<long long>(big, nnz_max / 8) / C;
+    lin_threads = 128;
+    while (lin_threads < 1024 && lin_threads * 4 < work) lin_threads *= 2;
+    const size_t ns = ((size_t)nmax + 3) & ~(size_t)3, ms = ((size_t)mmax + 3) & ~(size_t)3;
+    const size_t vec_bytes = (5 * ns + ms) * sizeof(T);
+    const size_t pd_bytes = (((size_t)pnn_max + 3) & ~(size_t)3) * sizeof(T);
+    const size_t budget = (size_t)smem_optin - 2048;
+    D.vec_smem = (C == 1 && vec_bytes <= budget) ? 1 : 0;
+    D.P_smem = (C == 1 && p_dense && D.vec_smem && pd_bytes + vec_bytes <= budget) ? 1 : 0;
+    lin_smem = (D.vec_smem ? vec_bytes : 0) + (D.P_smem ? pd_bytes : 0);
+    team_C = C;
+    // ---- sliced-ELL chunk format (lin.cuh sell_rows): single-CTA teams with shared-memory vectors -------------------
+    D.batched = 0; D.nmax = nmax; D.mmax = mmax; D.sell_slots = 0;
+    if (C == 1 && D.vec_smem && o.no_batch == 0) {
+      struct SellHost {
+        std::vector<int> sl_base, slab_off, crow, mr_base; std::vector<int4> mrow; std::vector<T> val; std::vector<IT> idx; int max_slots = 0;
+      };
+      // rows [off[b], off[b+1]) of problem b; rp global row pointers; ci / v the element arrays
+      auto build = [&](const std::vector<int>& rp, const int64_t* off, const IT* ci, const T* v, SellHost& S) {
+        struct Chunk { int len, row, start, slot; };
+        S.sl_base.assign(B + 1, 0); S.mr_base.assign(B + 1, 0); S.slab_off.assign(1, 0);
+        std::vector<Chunk> ch;
+        int col = 0;
+        for (int b = 0; b < B; ++b) {
+          ch.clear();
+          int slots = 0;
+          for (long long r = off[b]; r < off[b + 1]; ++r) {
+            const int len = rp[r + 1] - rp[r], nch = std::max(1, (len + 31) / 32);
+            if (nch > 1) S.mrow.push_back(make_int4((int)(r - off[b]), slots, nch, 0));
+            for (int c = 0; c < nch; ++c)
+              ch.push_back(Chunk{std::min(32, len - 32 * c), (int)(r - off[b]), rp[r] + 32 * c, nch > 1 ? slots++ : -1});
+          }
+          S.max_slots = std::max(S.max_slots, slots);
+          std::stable_sort(ch.begin(), ch.end(), [](const Chunk& x, const Chunk& y) { return x.len > y.len; });
+          for (size_t i = 0; i < ch.size(); i += 32) {
+            const int L = (ch[i].len + 1) / 2;      // element pairs per lane
+            const size_t base = S.val.size();
+            S.val.resize(base + (size_t)L * 64, (T)0); S.idx.resize(base + (size_t)L * 64, (IT)0);
+            for (int lane = 0; lane < 32; ++lane) {
+              if (i + lane >= ch.size()) { S.crow.push_back(SELL_NONE); continue; }
+              const Chunk& q = ch[i + lane];
+              S.crow.push_back(q.slot < 0 ? q.row : -(q.slot + 1));
+              for (int k = 0; k < q.len; ++k) {
+                const size_t o = base + ((size_t)(k >> 1) * 32 + lane) * 2 + (k & 1);
+                S.val[o] = v[q.start + k]; S.idx[o] = ci[q.start + k];
+              }
+            }
+            col += L;
+            S.slab_off.push_back(col);
+          }
+          S.sl_base[b + 1] = (int)S.slab_off.size() - 1;
+          S.mr_base[b + 1] = (int)S.mrow.size();
+        }
+      };
+      auto upload = [&](SellHost& S, Sell<T, IT>& dS) {
+        dS.sl_base = pool.upload(S.sl_base, st); dS.slab_off = pool.upload(S.slab_off, st); dS.crow = pool.upload(S.crow, st);
+        dS.mr_base = pool.upload(S.mr_base, st); dS.mrow = pool.upload(S.mrow, st); dS.val = pool.upload(S.val, st); dS.idx = pool.upload(S.idx, st);
+      };
+      SellHost hA, hAT, hP;
+      build(A_rp, pr->row_off, A_ci.data(), Av, hA);
+      build(AT_rp, pr->var_off, AT_ci.data(), AT_v.data(), hAT);
+      if (!p_dense) build(P_rp, pr->var_off, P_ci.data(), Pv, hP);     // rows without entries still emit a zero
+      else { hP.sl_base.assign(B + 1, 0); hP.mr_base.assign(B + 1, 0); hP.slab_off.assign(1, 0); }
+      const int slots = std::max(hA.max_slots, std::max(hAT.max_slots, hP.max_slots));
+      const size_t fixed = (((size_t)slots + 1) & ~(size_t)1) * sizeof(double) + vec_bytes;
+      if (fixed <= budget) {
+        D.batched = 1; D.sell_slots = slots;
+        D.P_smem = (p_dense && fixed + pd_bytes <= budget) ? 1 : 0;
+        lin_smem = fixed + (D.P_smem ? pd_bytes : 0);
+        upload(hA, D.SA); upload(hAT, D.SAT); upload(hP, D.SP);
+        if (pool.last != cudaSuccess) { err = std::string("cdu_create (sliced ELL): ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
+        CU_OK(cudaStreamSynchronize(st));   // the staging vectors go out of scope
+      }
+    }
+    const void* fns[4] = {(const void*)k_fwd<T, IT, false>, (const void*)k_bwd<T, IT, false>, (const void*)k_fwd<T, IT, true>,
+                          (const void*)k_bwd<T, IT, true>};
+    for (int i = 0; i < 4; ++i) {
+      CU_OK(cudaFuncSetAttribute(fns[i], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(lin_smem, 1024)));
+      if (i >= 2 && C > 8) CU_OK(cudaFuncSetAttribute(fns[i], cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    }
+    if (C == 1) {
+      int occ = 1;
+      CU_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bwd<T, IT, false>, lin_threads, lin_smem));
+      occ = std::max(occ, 1);
+      // keep the matrices of the problems in flight inside L2 (126 MB): they are re-read every CG iteration
+      const double ws = ((double)nnzA * 2.0 * (sizeof(T) + sizeof(IT)) + (D.P_smem ? 0.0 : (double)nnzP * (sizeof(T) + (p_dense ? 0 : sizeof(IT))))) / B;
+      const long long conc = (long long)(96.0 * 1024 * 1024 / std::max(ws, 1.0));
+      lin_grid = (int)std::min<long long>(B, std::min<long long>((long long)nsm * occ, std::max<long long>(conc, nsm)));
+    } else {
+      cudaLaunchConfig_t cfg{};
+      cfg.gridDim = dim3(B * C); cfg.blockDim = dim3(lin_threads); cfg.dynamicSmemBytes = lin_smem;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      int ncl = 0;
+      cudaError_t e = cudaOccupancyMaxActiveClusters(&ncl, k_bwd<T, IT, true>, &cfg);
+      if (e != cudaSuccess || ncl < 1) { (void)cudaGetLastError(); err = "cdu_create: cluster launch not possible for the linear-step kernels"; return CDU_ECUDA; }
+      lin_grid = std::min(B, ncl) * C;
+    }
+  }
+
+  // ---- PSD engine -----------------------------------------------------------------------------------------
+  {
+    psd.prof = &prof;
+    cdu_status s = psd.build(pool, psd_prob, psd_row0, psd_p, small_max, o.use_tensor_cores, st);
+    if (s != CDU_OK) { err = psd.err; return s; }
+  }
+  D.psd_part = pool.zeros<double>(2 * (size_t)std::max(psd.nblk, 1), st);
+
+  // ---- checkpoint store -------------------------------------------------------------------------------------
+  const size_t before = pool.bytes;
+  zstride = (size_t)N + 2 * (size_t)Mtot;
+  Z = pool.alloc<double>((size_t)(K_max + 1) * zstride);
+  const size_t slots = ckpt_mode == CDU_CKPT_FULL ? (size_t)K_max : 1;
+  XT = pool.alloc<double>(slots * N); ST = pool.alloc<double>(slots * Mtot);
+  Ustore = pool.alloc<T>(slots * psd.sum_p2); Lstore = pool.alloc<T>(slots * psd.sum_p);
+  if (!Z || !XT || !ST || !Ustore || !Lstore) { err = "cudaMalloc (checkpoint store)"; return CDU_ENOMEM; }
+  ckpt_bytes = pool.bytes - before;
+  GZ[0] = pool.alloc<double>(zstride); GZ[1] = pool.alloc<double>(zstride);
+  g_rho_pb = pool.zeros<double>((size_t)K_max * B, st); g_alpha_pb = pool.zeros<double>((size_t)K_max * B, st);
+  g_sigma_pb = pool.zeros<double>((size_t)K_max * B, st); part_pre = pool.zeros<double>(2 * (size_t)B, st);
+  d_rho = pool.alloc<T>((size_t)K_max * B); d_alpha = pool.alloc<T>((size_t)K_max * B);
+  stage = pool.alloc<T>(zstride); stage_g = pool.alloc<T>(2 * (size_t)K_max * B + B);
+  if (pool.last != cudaSuccess || !GZ[0] || !GZ[1] || !stage || !stage_g) { err = std::string("cdu_create: ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
+  CU_OK(cudaStreamSynchronize(st));   // host vectors above go out of scope
+  return CDU_OK;
+}
+
+template <typename T, typename IT>
+cdu_status HandleT<T, IT>::import_state(double* z, const void* x, const void* s, const void* y, int host, cudaStream_t st) {
+  const void* src[3] = {x, s, y};
+  const long long len[3] = {N, Mtot, Mtot};
+  double* dst[3] = {z, z + N, z + N + Mtot};
+  T* stg = stage;
+  for (int i = 0; i < 3; ++i) {
+    const T* dsrc = reinterpret_cast<const T*>(src[i]);
+    if (src[i] && host) {
+      CU_OK(cudaMemcpyAsync(stg, src[i], len[i] * sizeof(T), cudaMemcpyHostToDevice, st));
+      dsrc = stg; stg += len[i];
+    }
+    if (len[i] == 0) continue;
+    if (!src[i]) { CU_OK(cudaMemsetAsync(dst[i], 0, len[i] * sizeof(double), st)); }
+    else { k_load_vec<T><<<(int)std::min<long long>((len[i] + 255) / 256, 2048), 256, 0, st>>>(dst[i], dsrc, len[i]); ++launches; CU_OK(cudaGetLastError()); }
+  }
+  return CDU_OK;
+}
+
+template <typename T, typename IT>
+cdu_status HandleT<T, IT>::export_state(const double* z, void* x, void* s, void* y, int host, cudaStream_t st) {
+  void* dstp[3] = {x, s, y};
+  const long long len[3] = {N, Mtot, Mtot};
+  const double* src[3] = {z, z + N, z + N + Mtot};
+  T* stg = stage;
+  for (int i = 0; i < 3; ++i) {
+    if (!dstp[i] || len[i] == 0) continue;
+    T* ddst = host ? stg : reinterpret_cast<T*>(dstp[i]);
+    k_store_vec<T><<<(int)std::min<long long>((len[i] + 255) / 256, 2048), 256, 0, st>>>(ddst, src[i], len[i]);
+    ++launches;
+    CU_OK(cudaGetLastError());
+    if (host) { CU_OK(cudaMemcpyAsync(dstp[i], stg, len[i] * sizeof(T), cudaMemcpyDeviceToHost, st)); stg += len[i]; }
+  }
+  return CDU_OK;
+}
+
+template <typename T, typename IT>
+cdu_status HandleT<T, IT>::forward(int K, const void* rho, int mode, double sigma, const void* alpha, const void* x0,
+                               const void* s0, const void* y0, void* xK, void* sK, void* yK, int host, cudaStream_t st) {
+  if (K < 1 || K > K_max) { err = "cdu_forward: K out of [1, K_max]"; return CDU_EINVAL; }
+  if (!rho || !alpha) { err = "cdu_forward: NULL rho/alpha"; return CDU_EINVAL; }
+  if (!(sigma > 0.0)) { err = "cdu_forward: sigma must be > 0"; return CDU_EINVAL; }
+  if (mode != CDU_RHO_PER_ITER && mode != CDU_RHO_PER_PROBLEM) { err = "cdu_forward: bad rho_mode"; return CDU_EINVAL; }
+  const size_t cnt = (size_t)K * (mode == CDU_RHO_PER_ITER ? 1 : B);
+  if (host) {
+    const T* r = reinterpret_cast<const T*>(rho); const T* a = reinterpret_cast<const T*>(alpha);
+    for (size_t i = 0; i < cnt; ++i)
+      if (!(r[i] > (T)0) || !(a[i] > (T)0) || !(a[i] < (T)2)) { err = "cdu_forward: rho must be > 0 and alpha in (0,2)"; return CDU_EINVAL; }
+  }
+  const cudaMemcpyKind kind = host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+  CU_OK(cudaMemcpyAsync(d_rho, rho, cnt * sizeof(T), kind, st));
+  CU_OK(cudaMemcpyAsync(d_alpha, alpha, cnt * sizeof(T), kind, st));
+  CU_OK(cudaMemsetAsync(flags, 0, B * sizeof(int), st));
+  if (!host) {   // device-resident hyper-parameters: checked by a kernel, reported through the per-problem flags
+    k_check_hyper<T><<<std::min<int>((int)((cnt + 255) / 256), 64), 256, 0, st>>>(d_rho, d_alpha, (long long)cnt, mode == CDU_RHO_PER_ITER ? 0 : B, B, flags);
+    ++launches;
+    CU_OK(cudaGetLastError());
+  }
+  K_last = 0; mode_last = mode; sigma_last = sigma; last_stream = st;
+  cdu_status s = import_state(z_at(0), x0, s0, y0, host, st);
+  if (s != CDU_OK) return s;
+  CU_OK(cudaMemsetAsync(cg_f, 0, B * sizeof(int), st));
+  CU_OK(cudaMemsetAsync(cg_f0, 0, B * sizeof(int), st));
+  CU_OK(cudaMemsetAsync(cg_max, 0, B * sizeof(int), st));
+  CU_OK(cudaMemsetAsync(psd.sweeps_max, 0, sizeof(int), st));
+  CU_OK(cudaMemsetAsync(psd.sweeps_sum, 0, sizeof(unsigned long long), st));
+  const Hyper<T> H = hyper();
+  BatchDev<T, IT> Df = D; Df.cg_iters = cg_f; Df.cg_iters0 = cg_f0;
+  const bool full = ckpt_mode == CDU_CKPT_FULL;
+  psd.warm = false;        // every unroll starts cold: results do not depend on the handle's history
+  for (int k = 0; k < K; ++k) {
+    IterPtrs I;
+    I.Zk = z_at(k); I.Zk1 = z_at(k + 1);
+    I.XT = XT + (full ? (size_t)k * N : 0); I.ST = ST + (full ? (size_t)k * Mtot : 0);
+    prof.begin(PC_LIN_FWD, st);
+    cudaError_t le = launch_lin(k_fwd<T, IT, false>, k_fwd<T, IT, true>, st, Df, H, I, k);
+    prof.end(st);
+    ++launches;
+    CU_OK(le);
+    if (has_psd) {
+      PsdFwdArgs A;
+      A.W = D.W; A.S1 = z_at(k + 1) + N; A.Y1 = z_at(k + 1) + N + Mtot;
+      A.Ustore = Ustore + (full ? (size_t)k * psd.sum_p2 : 0); A.Lstore = Lstore + (full ? (size_t)k * psd.sum_p : 0);
+      A.Uprev = (k > 0 && psd.warm_enable) ? (const void*)(Ustore + (full ? (size_t)(k - 1) * psd.sum_p2 : 0)) : nullptr;
+      A.sweeps_max = psd.sweeps_max; A.flags = flags; A.sweeps_sum = psd.sweeps_sum;
+      s = psd.forward(H, k, A, st);
+      if (s != CDU_OK) { err = psd.err; return s; }
+    }
+  }
+  K_last = K;
+  s = export_state(z_at(K), xK, sK, yK, host, st);
+  if (s != CDU_OK) return s;
+  if (host) CU_OK(cudaStreamSynchronize(st));
+  return CDU_OK;
+}
+
+template <typename T, typename IT>
+cdu_status HandleT<T, IT>::backward(const void* gx, const void* gs, const void* gy, void* g_rho, void* g_sigma, void* g_alpha,
+                                void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st) {
+  if (K_last < 1) { err = "cdu_backward: no forward pass on this handle"; return CDU_ESTATE; }
+  const int K = K_last;
+  last_stream = st;
+  cdu_status s = import_state(GZ[K & 1], gx, gs, gy, host, st);
+  if (s != CDU_OK) return s;
+  CU_OK(cudaMemsetAsync(cg_b, 0, B * sizeof(int), st));
+  CU_OK(cudaMemsetAsync(cg_b0, 0, B * sizeof(int), st));
+  const Hyper<T> H = hyper();
+  BatchDev<T, IT> Db = D; Db.cg_iters = cg_b; Db.cg_iters0 = cg_b0;
+  const bool full = ckpt_mode == CDU_CKPT_FULL;
+  psd.warm = false;
+  for (int k = K - 1; k >= 0; --k) {
+    BwdPtrs Q;
+    Q.Zk = z_at(k); Q.Zk1 = z_at(k + 1);
+    Q.XT = XT + (full ? (size_t)k * N : 0); Q.ST = ST + (full ? (size_t)k * Mtot : 0);
+    Q.Gin = GZ[(k + 1) & 1]; Q.Gout = GZ[k & 1];
+    Q.g_rho_pb = g_rho_pb; Q.g_alpha_pb = g_alpha_pb; Q.g_sigma_pb = g_sigma_pb; Q.part_pre = part_pre;
+    Q.recompute = full ? 0 : 1;
+    Q.warm_adjoint = k < K - 1 ? 1 : 0;
+    if (!has_psd) {
+      prof.begin(PC_LIN_BWD, st);
+      cudaError_t le = launch_lin(k_bwd<T, IT, false>, k_bwd<T, IT, true>, st, Db, H, Q, k, 0);
+      prof.end(st);
+      ++launches;
+      CU_OK(le);
+    } else {
+      prof.begin(PC_LIN_BWD, st);
+      cudaError_t le = launch_lin(k_bwd<T, IT, false>, k_bwd<T, IT, true>, st, Db, H, Q, k, 1);
+      prof.end(st);
+      ++launches;
+      CU_OK(le);
+      PsdBwdArgs A;
+      A.W = D.W; A.Yk = z_at(k) + N + Mtot; A.S1 = z_at(k + 1) + N;
+      A.Gs = Q.Gin + N; A.Gy = Q.Gin + N + Mtot; A.GW = D.GW; A.part = D.psd_part;
+      A.Ustore = Ustore + (full ? (size_t)k * psd.sum_p2 : 0); A.Lstore = Lstore + (full ? (size_t)k * psd.sum_p : 0);
+      A.recompute = full ? 0 : 1; A.flags = flags;
+      s = psd.backward(H, k, A, st);
+      if (s != CDU_OK) { err = psd.err; return s; }
+      prof.begin(PC_LIN_BWD, st);
+      le = launch_lin(k_bwd<T, IT, false>, k_bwd<T, IT, true>, st, Db, H, Q, k, 2);
+      prof.end(st);
+      ++launches;
+      CU_OK(le);
+    }
+  }
+  const int pp = mode_last == CDU_RHO_PER_PROBLEM;
+  const size_t cnt = (size_t)K * (pp ? B : 1), scnt = pp ? B : 1;
+  T* o_rho = host ? stage_g : reinterpret_cast<T*>(g_rho);
+  T* o_alpha = host ? stage_g + cnt : reinterpret_cast<T*>(g_alpha);
+  T* o_sigma = host ? stage_g + 2 * cnt : reinterpret_cast<T*>(g_sigma);
+  if (host) { if (!g_rho) o_rho = nullptr; if (!g_alpha) o_alpha = nullptr; if (!g_sigma) o_sigma = nullptr; }
+  k_reduce_grads<T><<<1, 256, 0, st>>>(g_rho_pb, g_alpha_pb, g_sigma_pb, K, B, pp, o_rho, o_alpha, o_sigma);
+  ++launches;
+  CU_OK(cudaGetLastError());
+  if (host) {
+    if (g_rho) CU_OK(cudaMemcpyAsync(g_rho, o_rho, cnt * sizeof(T), cudaMemcpyDeviceToHost, st));
+    if (g_alpha) CU_OK(cudaMemcpyAsync(g_alpha, o_alpha, cnt * sizeof(T), cudaMemcpyDeviceToHost, st));
+    if (g_sigma) CU_OK(cudaMemcpyAsync(g_sigma, o_sigma, scnt * sizeof(T), cudaMemcpyDeviceToHost, st));
+  }
+  s = export_state(GZ[0], g_x0, g_s0, g_y0, host, st);
+  if (s != CDU_OK) return s;
+  if (host) CU_OK(cudaStreamSynchronize(st));
+  return CDU_OK;
+}
+
+template <typename T, typename IT>
+cdu_status HandleT<T, IT>::iterate(int k, void* x, void* s, void* y, int host, cudaStream_t st) {
+  if (k < 0 || k > K_last) { err = "cdu_get_iterate: k out of range"; return CDU_EINVAL; }
+  cdu_status r = export_state(z_at(k), x, s, y, host, st);
+  if (r != CDU_OK) return r;
+  if (host) CU_OK(cudaStreamSynchronize(st));
+  return CDU_OK;
+}
+
+template <typename T, typename IT>
+cdu_status HandleT<T, IT>::stats(cdu_stats* out) {
+  if (!out) { err = "cdu_get_stats: NULL out"; return CDU_EINVAL; }
+  CU_OK(cudaStreamSynchronize(last_stream));
+  std::vector<int> f(B), bw(B), mx(B), fl(B), f0(B), b0(B);
+  int sw = 0;
+  CU_OK(cudaMemcpy(f.data(), cg_f, B * sizeof(int), cudaMemcpyDeviceToHost));
+  CU_OK(cudaMemcpy(bw.data(), cg_b, B * sizeof(int), cudaMemcpyDeviceToHost));
+  CU_OK(cudaMemcpy(mx.data(), cg_max, B * sizeof(int), cudaMemcpyDeviceToHost));
+  CU_OK(cudaMemcpy(f0.data(), cg_f0, B * sizeof(int), cudaMemcpyDeviceToHost));
+  CU_OK(cudaMemcpy(b0.data(), cg_b0, B * sizeof(int), cudaMemcpyDeviceToHost));
+  CU_OK(cudaMemcpy(fl.data(), flags, B * sizeof(int), cudaMemcpyDeviceToHost));
+  CU_OK(cudaMemcpy(&sw, psd.sweeps_max, sizeof(int), cudaMemcpyDeviceToHost));
+  unsigned long long ssum = 0;
+  CU_OK(cudaMemcpy(&ssum, psd.sweeps_sum, sizeof(ssum), cudaMemcpyDeviceToHost));
+  std::memset(out, 0, sizeof(*out));
+  for (int b = 0; b < B; ++b) {
+    out->cg_iters_fwd += f[b]; out->cg_iters_bwd += bw[b];
+    out->cg_iters_fwd_pass0 += f0[b]; out->cg_iters_bwd_pass0 += b0[b];
+    out->cg_iters_max = std::max(out->cg_iters_max, mx[b]);
+    if (fl[b]) { ++out->n_flagged; out->flags_or |= fl[b]; }
+  }
+  out->eig_sweeps_max = sw;
+  out->eig_sweeps_sum = (int64_t)ssum;
+  out->device_bytes = (int64_t)pool.bytes; out->ckpt_bytes = (int64_t)ckpt_bytes;
+  out->launches = launches + psd.launches;
+  if (out->n_flagged) { err = "cdu_get_stats: per-problem flags are set (flags_or = " + std::to_string(out->flags_or) + ")"; return CDU_ENUMERIC; }
+  return CDU_OK;
+}
+
+template <typename T, typename IT>
+cdu_status create_t(const cdu_problem* pr, const cdu_options* op, cudaStream_t st, cdu_handle* out) {
+  HandleT<T, IT>* h = new (std::nothrow) HandleT<T, IT>();
+  if (!h) { create_error() = "out of host memory"; return CDU_ENOMEM; }
+  cdu_status s;
+  try { s = h->init(pr, op, st); }
+  catch (const std::bad_alloc&) { h->err = "out of host memory"; s = CDU_ENOMEM; }
+  if (s != CDU_OK) { create_error() = h->err; delete h; return s; }
+  *out = h;
+  return CDU_OK;
+}
+
+// ---- stand-alone PSD operators ------------------------------------------------------------------------------
+template <typename T>
+__global__ void k_dense_to_svec(int p, const T* S, double* v) {   // one block per matrix
+  const long long off = (long long)blockIdx.x * p * p;
+  const int nsv = p * (p + 1) / 2;
+  for (long long t = threadIdx.x; t < (long long)p * p; t += blockDim.x) {
+    const int r = (int)(t / p), c = (int)(t - (long long)r * p);
+    if (r <= c) {
+      const double x = r == c ? (double)S[off + t] : 0.5 * ((double)S[off + t] + (double)S[off + (long long)c * p + r]) * 1.41421356237309504880;
+      v[(long long)blockIdx.x * nsv + svec_idx(r, c)] = x;
+    }
+  }
+}
+template <typename T>
+__global__ void k_svec_to_dense(int p, const double* v, T* S) {
+  const long long off = (long long)blockIdx.x * p * p;
+  const int nsv = p * (p + 1) / 2;
+  for (long long t = threadIdx.x; t < (long long)p * p; t += blockDim.x) {
+    const int r = (int)(t / p), c = (int)(t - (long long)r * p);
+    const double x = v[(long long)blockIdx.x * nsv + (r <= c ? svec_idx(r, c) : svec_idx(c, r))];
+    S[off + t] = (T)(r == c ? x : x * 0.70710678118654752440);
+  }
+}
+template <typename T>
+__global__ void k_transpose_batched(int p, const T* A, T* Bm) {
+  const long long off = (long long)blockIdx.x * p * p;
+  for (long long t = threadIdx.x; t < (long long)p * p; t += blockDim.x) {
+    const int r = (int)(t / p), c = (int)(t - (long long)r * p);
+    Bm[off + (long long)c * p + r] = A[off + t];
+  }
+}
+
+template <typename T>
+cdu_status psd_op_t(bool vjp, int count, int p, const void* in1, const void* in2, const void* in3, void* out1, void* out2,
+                    void* out3, int path, int use_tc, cudaStream_t st) {
+  std::string& err = create_error();
+  // projection: in1 = S           -> out1 = PiS, out2 = U, out3 = lam
+  // vjp       : in1 = U, in2 = lam, in3 = Gbar -> out1 = Sbar
+  if (count < 1 || p < 1 || !in1 || !out1 || (vjp && (!in2 || !in3))) { err = "cdu_psd_*: bad arguments"; return CDU_EINVAL; }
+  DevPool pool;
+  PsdEngine<T> eng;
+  const int nsv = p * (p + 1) / 2;
+  std::vector<int> prob(count), row0(count), pv(count, p);
+  for (int i = 0; i < count; ++i) { prob[i] = i; row0[i] = i * nsv; }
+  const bool f32 = std::is_same<T, float>::value;
+  int small_max = f32 ? 128 : 88;
+  if (path == 1) small_max = 1 << 30; else if (path == 2) small_max = 0;
+  cdu_status s = eng.build(pool, prob, row0, pv, small_max, use_tc, st);
+  if (s != CDU_OK) { err = eng.err; return s; }
+  const size_t tot = (size_t)count * nsv;
+  double* W = pool.zeros<double>(tot, st); double* S1 = pool.zeros<double>(tot, st); double* Y1 = pool.zeros<double>(tot, st);
+  double* GW = pool.zeros<double>(tot, st); double* part = pool.zeros<double>(2 * (size_t)count, st);
+  double* Gs = pool.zeros<double>(tot, st);
+  T* Us = pool.alloc<T>((size_t)count * p * p); T* Ls = pool.alloc<T>((size_t)count * p);
+  int* flags = pool.zeros<int>(count, st);
+  std::vector<T> one(1, (T)1);
+  T* d_one = pool.upload(one, st);
+  if (pool.last != cudaSuccess || !W || !S1 || !Y1 || !GW || !part || !Gs || !Us || !Ls || !flags || !d_one) { err = "cudaMalloc (psd op)"; return CDU_ENOMEM; }
+  Hyper<T> H; H.rho = d_one; H.alpha = d_one; H.kstride = 0; H.pstride = 0; H.sigma = 1.0;
+  if (!vjp) {
+    k_dense_to_svec<T><<<count, 256, 0, st>>>(p, (const T*)in1, W);
+    PsdFwdArgs A; A.W = W; A.S1 = S1; A.Y1 = Y1; A.Ustore = Us; A.Lstore = Ls; A.Uprev = nullptr; A.sweeps_max = eng.sweeps_max; A.flags = flags; A.sweeps_sum = eng.sweeps_sum;
+    s = eng.forward(H, 0, A, st);
+    if (s != CDU_OK) { err = eng.err; return s; }
+    k_svec_to_dense<T><<<count, 256, 0, st>>>(p, S1, (T*)out1);
+    if (out2) k_transpose_batched<T><<<count, 256, 0, st>>>(p, Us, (T*)out2);   // both paths store eigenvectors as rows
+    if (out3) CU_OK(cudaMemcpyAsync(out3, Ls, (size_t)count * p * sizeof(T), cudaMemcpyDeviceToDevice, st));
+  } else {
+    k_transpose_batched<T><<<count, 256, 0, st>>>(p, (const T*)in1, Us);
+    CU_OK(cudaMemcpyAsync(Ls, in2, (size_t)count * p * sizeof(T), cudaMemcpyDeviceToDevice, st));
+    k_dense_to_svec<T><<<count, 256, 0, st>>>(p, (const T*)in3, Gs);
+    PsdBwdArgs A; A.W = W; A.Yk = Y1; A.S1 = S1; A.Gs = Gs; A.Gy = W /* zeros */; A.GW = GW; A.part = part;
+    A.Ustore = Us; A.Lstore = Ls; A.recompute = 0; A.flags = flags;
+    s = eng.backward(H, 0, A, st);
+    if (s != CDU_OK) { err = eng.err; return s; }
+    k_svec_to_dense<T><<<count, 256, 0, st>>>(p, GW, (T*)out1);
+  }
+  CU_OK(cudaGetLastError());
+  CU_OK(cudaStreamSynchronize(st));
+  return CDU_OK;
+}
+
+
+}  // namespace impl
+}  // namespace cdu

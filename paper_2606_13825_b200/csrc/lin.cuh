@@ -56,7 +56,7 @@ struct BatchDev {
   T *r, *p, *Ap, *d, *dinv, *tA;                       // CG vectors (global copies; unused parts when vec_smem)
   double tol, tol_ref;
   int maxit, refine;
-  int *cg_iters, *cg_max, *flags;                      // [B] statistics
+  int *cg_iters, *cg_iters0, *cg_max, *flags;          // [B] statistics (cg_iters0: iterations of pass 0 only, i.e. without refinement)
   double* psd_part;                                    // [nblk][2] partial dots written by the PSD backward
   long long N, Mtot;
 };
@@ -347,7 +347,7 @@ __device__ int pcg(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, double
 // rhs: owner rows valid. out: every row valid team-wide on return (after a team sync).
 template <typename T, typename IT, bool MULTI>
 __device__ int solve_M(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const double* rhs, const double* xbase,
-                       double* out, int* flag) {
+                       double* out, int* flag, int* it0) {
   const int tid = threadIdx.x, nt = blockDim.x;
   double acc[1] = {0.0};
   for (int i = c.nlo + tid; i < c.nhi; i += nt) {
@@ -393,6 +393,7 @@ __device__ int solve_M(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, co
     }
     const int it = pcg(D, c, thresh, rr0, flag);
     total += it;
+    if (pass == 0) *it0 += it;
     if (it == 0 && pass == 0 && D.refine == 0) break;
     for (int i = c.nlo + tid; i < c.nhi; i += nt) out[i] += (double)c.d[i];
     c.team->sync();
@@ -404,13 +405,13 @@ __device__ int solve_M(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, co
 // xi and x-tilde of one step from z^k = (x, s, y): S1 + S2. Writes xt; st is produced by the caller's A pass.
 template <typename T, typename IT, bool MULTI>
 __device__ int lin_solve_step(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const double* x, const double* s,
-                              const double* y, double* xt, int* flag) {
+                              const double* y, double* xt, int* flag, int* it0) {
   const int tid = threadIdx.x, nt = blockDim.x;
   for (int i = c.mlo + tid; i < c.mhi; i += nt) c.tm[i] = c.rho * ((double)c.bv[i] - s[i]) - y[i];
   c.team->sync();
   rows_AT<double>(D, c, c.tm, [&](int row, double a) { c.xi[row] = c.sigma * x[row] - (double)c.q[row] + a; });
   c.team->sync();   // tm is reused by solve_M's residual pass
-  return solve_M(D, c, c.xi, x, xt, flag);
+  return solve_M(D, c, c.xi, x, xt, flag, it0);
 }
 
 __device__ __forceinline__ int soc_branch(double t, double nu) { return (nu <= t) ? 0 : ((nu <= -t) ? 1 : 2); }
@@ -442,8 +443,8 @@ __global__ void __launch_bounds__(1024) k_fwd(BatchDev<T, IT> D, Hyper<T> H, Ite
     const double *x = I.Zk + v0, *s = I.Zk + D.N + r0, *y = I.Zk + D.N + D.Mtot + r0;
     double *x1 = I.Zk1 + v0, *s1 = I.Zk1 + D.N + r0, *y1 = I.Zk1 + D.N + D.Mtot + r0;
     double *xt = I.XT + v0, *st = I.ST + r0;
-    int flag = 0;
-    const int iters = lin_solve_step(D, c, x, s, y, xt, &flag);
+    int flag = 0, it0 = 0;
+    const int iters = lin_solve_step(D, c, x, s, y, xt, &flag, &it0);
     const double al = c.alpha, rho = c.rho;
     const uint8_t* kind = D.rowkind + r0;
     rows_A<double>(D, c, xt, [&](int row, double a) {
@@ -485,6 +486,7 @@ __global__ void __launch_bounds__(1024) k_fwd(BatchDev<T, IT> D, Hyper<T> H, Ite
     }
     if (tid == 0 && team.rank == 0) {
       D.cg_iters[b] += iters;
+      D.cg_iters0[b] += it0;
       if (iters > D.cg_max[b]) D.cg_max[b] = iters;
       if (flag) D.flags[b] |= flag;
     }
@@ -514,7 +516,7 @@ struct BwdPtrs {
 // Phase 1 of the reverse step: (LEAN: re-solve), w, and B1/B2/B4 for zero, nonneg and SOC rows.
 template <typename T, typename IT, bool MULTI>
 __device__ void bwd_pre(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const BwdPtrs& Q, double* out_part, int* flag,
-                        int* iters) {
+                        int* iters, int* it0) {
   const int b = c.b, tid = threadIdx.x, nt = blockDim.x;
   const long long v0 = D.var_off[b], r0 = D.row_off[b];
   const double *x = Q.Zk + v0, *s = Q.Zk + D.N + r0, *y = Q.Zk + D.N + D.Mtot + r0;
@@ -523,7 +525,7 @@ __device__ void bwd_pre(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const B
   double *xt = Q.XT + v0, *st = Q.ST + r0;
   const double al = c.alpha, rho = c.rho;
   if (Q.recompute) {
-    *iters += lin_solve_step(D, c, x, s, y, xt, flag);
+    *iters += lin_solve_step(D, c, x, s, y, xt, flag, it0);
     rows_A<double>(D, c, xt, [&](int row, double a) { st[row] = (double)c.bv[row] - a; });
     __syncthreads();
   }
@@ -585,7 +587,7 @@ __device__ void bwd_pre(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const B
 // Phase 2: B5-B9 with the adjoint solve; needs GW complete on every row (PSD rows written by the PSD kernels).
 template <typename T, typename IT, bool MULTI>
 __device__ void bwd_post(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const BwdPtrs& Q, const double* part, int k,
-                         int* flag, int* iters) {
+                         int* flag, int* iters, int* it0) {
   const int b = c.b, tid = threadIdx.x, nt = blockDim.x;
   const long long v0 = D.var_off[b], r0 = D.row_off[b];
   const double *x = Q.Zk + v0, *s = Q.Zk + D.N + r0;
@@ -603,7 +605,7 @@ __device__ void bwd_post(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const 
   // reverse step: the start costs one extra fp64 operator application, which only pays for long solves. Same solution to
   // the same tolerance either way; the choice depends on this unroll's forward only (results stay history independent).
   const bool warm = Q.warm_adjoint && D.cg_max[b] >= 12;
-  *iters += solve_M(D, c, c.xi, warm ? (const double*)c.lam : (const double*)nullptr, c.lam, flag);
+  *iters += solve_M(D, c, c.xi, warm ? (const double*)c.lam : (const double*)nullptr, c.lam, flag, it0);
   // u = A lam; B7+B9 combined: g_rho += <u, st - s> (cancellation-free form of Eq. 6 + RHS term)
   double acc[3] = {0.0, 0.0, 0.0};   // rho, alpha, sigma
   rows_A<double>(D, c, c.lam, [&](int row, double u) {
@@ -636,17 +638,18 @@ __global__ void __launch_bounds__(1024) k_bwd(BatchDev<T, IT> D, Hyper<T> H, Bwd
   for (int b = team_id; b < D.B; b += nteams) {
     Prob<T, IT, MULTI> c(D, b, &team, dsm_);
     c.rho = H.rho_at(k, b); c.alpha = H.alpha_at(k, b); c.sigma = H.sigma;
-    int flag = 0, iters = 0;
+    int flag = 0, iters = 0, it0 = 0;
     double part[2];
     if (phase != 2) {
-      bwd_pre(D, c, Q, part, &flag, &iters);
+      bwd_pre(D, c, Q, part, &flag, &iters, &it0);
       if (phase == 1 && threadIdx.x == 0 && team.rank == 0) { Q.part_pre[2 * b] = part[0]; Q.part_pre[2 * b + 1] = part[1]; }
     } else {
       part[0] = Q.part_pre[2 * b]; part[1] = Q.part_pre[2 * b + 1];
     }
-    if (phase != 1) bwd_post(D, c, Q, part, k, &flag, &iters);
+    if (phase != 1) bwd_post(D, c, Q, part, k, &flag, &iters, &it0);
     if (threadIdx.x == 0 && team.rank == 0) {
       D.cg_iters[b] += iters;
+      D.cg_iters0[b] += it0;
       if (flag) D.flags[b] |= flag;
     }
     team.sync();
@@ -655,6 +658,18 @@ __global__ void __launch_bounds__(1024) k_bwd(BatchDev<T, IT> D, Hyper<T> H, Bwd
 }
 
 // ---- small utility kernels -------------------------------------------------------------------------------
+// Device-side validation of device-resident hyper-parameters (cdu.h): rho > 0, alpha in (0, 2). per_problem = B when the
+// arrays are [K][B] (the flag goes to that problem), 0 when they are [K] (shared: every problem is flagged).
+template <typename T>
+__global__ void k_check_hyper(const T* rho, const T* alpha, long long cnt, int per_problem, int B, int* flags) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < cnt; i += (long long)gridDim.x * blockDim.x) {
+    const T r = rho[i], a = alpha[i];
+    if (!(r > (T)0) || !(a > (T)0) || !(a < (T)2)) {
+      if (per_problem) atomicOr(flags + (int)(i % per_problem), FLAG_BAD_HYPER);
+      else for (int b = 0; b < B; ++b) atomicOr(flags + b, FLAG_BAD_HYPER);
+    }
+  }
+}
 template <typename T>
 __global__ void k_load_vec(double* dst, const T* src, long long n) {   // dst = src (NULL -> 0)
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)

@@ -300,7 +300,7 @@ __device__ __forceinline__ void apply_store(const T* Qt, const T* X, int ldx, in
 template <typename T, int RP>
 __global__ void __launch_bounds__(THREADS, 1)
 k_bjacobi(int nblk, const int* pvec, const long long* moff, const int* voff, T* G, T* Vt, const T* mu, T* lam, int* rotflags,
-          int* sweeps_out, unsigned long long* sweeps_sum, int max_sweeps, double tol) {
+          int* sweeps_out, unsigned long long* sweeps_sum, int max_sweeps, double tol, const int* prob_of, int* flags) {
   constexpr int BR = RP / 2, LQ = RP + 4;
   extern __shared__ __align__(16) unsigned char smem_bj[];
   cg::cluster_group cluster = cg::this_cluster();
@@ -327,6 +327,7 @@ k_bjacobi(int nblk, const int* pvec, const long long* moff, const int* voff, T* 
   const T thresh = (T)(0.25 * tol);
   const float quad_exit = (float)sqrt(tol / (16.0 * sqrt((double)p)));   // 2.9e-5 for fp32 at p = 512
   int sweep = 0;
+  bool capped = true;
   for (; sweep < max_sweeps; ++sweep) {
     for (int r = 0; r < NBe - 1; ++r) {
       for (int q = rank; q < NP; q += C) {
@@ -350,8 +351,8 @@ k_bjacobi(int nblk, const int* pvec, const long long* moff, const int* voff, T* 
       cluster.sync();
     }
     const unsigned worst = (unsigned)__ldcg(rf + sweep);     // largest |w_ij| / sqrt(w_ii w_jj) any pair showed in this sweep
-    if (!worst) break;                                        // nothing above the tolerance: converged
-    if (__uint_as_float(worst) <= quad_exit) { ++sweep; break; }   // quadratic convergence: every pair above tol was rotated while
+    if (!worst) { capped = false; break; }                    // nothing above the tolerance: converged
+    if (__uint_as_float(worst) <= quad_exit) { ++sweep; capped = false; break; }   // quadratic convergence: every pair above tol was rotated while
   }                                                           // all ratios were <= quad_exit; what is left is ~quad_exit^2 sqrt(p) <= tol / 16
   // eigenvalues and eigenvectors
   const int lane = threadIdx.x & 31, nw = blockDim.x >> 5;
@@ -366,10 +367,280 @@ k_bjacobi(int nblk, const int* pvec, const long long* moff, const int* voff, T* 
     const double inv = na > 0.0 ? 1.0 / na : 0.0;
     for (int c = lane; c < p; c += 32) vt[(size_t)i * p + c] = (T)((double)ld_cg(g + (size_t)i * p + c) * inv);
   }
-  if (rank == 0 && threadIdx.x == 0) { atomicMax(sweeps_out, sweep); if (sweeps_sum) atomicAdd(sweeps_sum, (unsigned long long)sweep); }
+  if (rank == 0 && threadIdx.x == 0) {
+    atomicMax(sweeps_out, sweep);
+    if (sweeps_sum) atomicAdd(sweeps_sum, (unsigned long long)sweep);
+    if (capped && flags) atomicOr(flags + prob_of[lb], FLAG_EIG_CAP);   // the sweep cap ended the iteration
+  }
 }
 
 template <typename T, int RP> inline size_t smem_bytes(int p) { return Plan<T, RP>(p).bytes; }
+
+// ---------------------------------------------------------------------------------------------------------
+// fp32 variant on the tensor cores (mma.sync m16n8k8, 3xTF32). Same algorithm and the same fixed point as k_bjacobi;
+// what changes is where the time of a block round goes (profiles/r01_bjacobi_cfg5.md: 20 % Gram + 12 % apply on FMA
+// units with the tensor pipe idle, half of it in the 31 dependent rounds of the inner sweep):
+//   * rows come in with cp.async (16-byte chunks, all in flight at once) instead of dependent L2 loads;
+//   * Gram W = X X' (32 x 32 x p): warp w contracts its own k slice of p/16 columns with 3xTF32 mma.sync into fresh
+//     accumulators (leading term a_hi b_hi apart from the two small terms, so the tensor core's truncating adder sees at
+//     most 4 additions per accumulator); the 16 partial matrices are summed in fp64 in a fixed order. Only the six
+//     16 x 8 tiles of the upper block triangle are formed. Shared-memory row stride = 4 mod 32 words: conflict free;
+//   * apply X' = Q X (32 x 32 x p): warp w owns p/16 columns, Q's fragments stay in registers, 3xTF32, results go
+//     from the accumulators straight to L2. The k slots of a fragment map to rows (2t, 2t+1) instead of (t, t+4) so that
+//     the transposed reads of X are conflict free with the same stride;
+//   * the pair table of the inner sweep meets the 256 CROSS pairs (one row of each block) in its first 16 rounds and
+//     the pairs inside a block in the last 15: rows of one block leave every block round mutually orthogonal, so once a
+//     matrix is past its first sweep the within-block rounds hold nothing above the tolerance and the round mask skips
+//     them - the dependent chain of a block round is 16 rotations long instead of 31.
+// Raises FLAG_EIG_CAP on the owning problem when the sweep cap ends the iteration (cdu.h, cdu_stats.flags_or).
+// ---------------------------------------------------------------------------------------------------------
+namespace tcv {
+constexpr int RP = 32, BR = 16, NWARP = 16, LW = RP + 1, LQ = RP + 4, LP = 40;   // LP: row stride of a Gram partial
+
+struct Plan {
+  int pk, ldx;
+  size_t off_part, off_w, off_w1, off_q, off_red, off_pairs, bytes;
+  __host__ __device__ explicit Plan(int p) {
+    pk = ((p + 127) / 128) * 128;            // every warp's k slice / column slice is a multiple of 8
+    ldx = pk + 4;
+    size_t o = (size_t)RP * ldx * sizeof(float);
+    off_part = o; o += (size_t)NWARP * RP * LP * sizeof(float);
+    off_w = o; o += (size_t)RP * LW * sizeof(float);
+    off_w1 = o; o += (size_t)RP * LW * sizeof(float);
+    off_q = (o + 15) & ~(size_t)15; o = off_q + (size_t)RP * LQ * sizeof(float);
+    off_red = (o + 15) & ~(size_t)15; o = off_red + 64 * sizeof(double);
+    off_pairs = o; o += (size_t)(RP - 1) * (RP / 2) * sizeof(int);
+    bytes = o;
+  }
+};
+
+__device__ __forceinline__ void split3(float a, uint32_t& hi, uint32_t& lo) {
+  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(hi) : "f"(a));
+  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(lo) : "f"(a - __uint_as_float(hi)));
+}
+__device__ __forceinline__ void mma_tf32(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+
+// rows of blocks bi, bj -> X[0..15], X[16..31]; pad columns [p, pk) keep their zeros, rows >= p are zero filled.
+__device__ __forceinline__ void load_pair(const float* __restrict__ g, int p, int bi, int bj, float* X, int ldx) {
+  if ((p & 3) == 0) {
+    const int nv = p >> 2;
+    for (int t = threadIdx.x; t < RP * nv; t += blockDim.x) {
+      const int r = t / nv, c = t - r * nv;
+      const int row = (r < BR ? bi * BR + r : bj * BR + r - BR);
+      float* dst = X + (size_t)r * ldx + 4 * c;
+      if (row < p) cp_async16(dst, g + (size_t)row * p + 4 * c);
+      else *reinterpret_cast<float4*>(dst) = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+  } else {
+    for (int t = threadIdx.x; t < RP * p; t += blockDim.x) {
+      const int r = t / p, c = t - r * p;
+      const int row = (r < BR ? bi * BR + r : bj * BR + r - BR);
+      X[(size_t)r * ldx + c] = row < p ? __ldcg(g + (size_t)row * p + c) : 0.f;
+    }
+  }
+}
+
+// part[warp] (32 x 32, stride LP; the block (rows 16-31, columns 0-15) is NOT written: read its mirror image).
+__device__ __forceinline__ void gram_mma(const float* X, int ldx, int ks, float* part) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  float accM[6][4], accS[6][4];
+#pragma unroll
+  for (int i = 0; i < 6; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { accM[i][j] = 0.f; accS[i][j] = 0.f; }
+  const float* xb = X + (size_t)g * ldx + warp * ks + t;
+  for (int kk = 0; kk < ks; kk += 8) {
+    uint32_t h[4][2], l[4][2];     // rows g + 8 a, columns t and t + 4 of this k step: A and B fragments share them
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+      split3(xb[(size_t)(8 * a) * ldx + kk], h[a][0], l[a][0]);
+      split3(xb[(size_t)(8 * a) * ldx + kk + 4], h[a][1], l[a][1]);
+    }
+    // tiles (m tile, n tile): (0,0) (0,1) (0,2) (0,3) (1,2) (1,3)
+#pragma unroll
+    for (int tl = 0; tl < 6; ++tl) {
+      const int mt = tl < 4 ? 0 : 1, nt = tl < 4 ? tl : tl - 2;
+      mma_tf32(accS[tl], l[2 * mt][0], l[2 * mt + 1][0], l[2 * mt][1], l[2 * mt + 1][1], h[nt][0], h[nt][1]);
+      mma_tf32(accS[tl], h[2 * mt][0], h[2 * mt + 1][0], h[2 * mt][1], h[2 * mt + 1][1], l[nt][0], l[nt][1]);
+      mma_tf32(accM[tl], h[2 * mt][0], h[2 * mt + 1][0], h[2 * mt][1], h[2 * mt + 1][1], h[nt][0], h[nt][1]);
+    }
+  }
+  float* pw = part + (size_t)warp * RP * LP;
+#pragma unroll
+  for (int tl = 0; tl < 6; ++tl) {
+    const int mt = tl < 4 ? 0 : 1, nt = tl < 4 ? tl : tl - 2;
+    const int r0 = 16 * mt + g, c0 = 8 * nt + 2 * t;
+    *reinterpret_cast<float2*>(pw + r0 * LP + c0) = make_float2(accM[tl][0] + accS[tl][0], accM[tl][1] + accS[tl][1]);
+    *reinterpret_cast<float2*>(pw + (r0 + 8) * LP + c0) = make_float2(accM[tl][2] + accS[tl][2], accM[tl][3] + accS[tl][3]);
+  }
+}
+
+// W = sum of the 16 partials (fp64, fixed order); returns max_{i<j} |w_ij| / sqrt(w_ii w_jj) to every thread.
+__device__ __forceinline__ double gram_reduce(const float* part, float* W, double* red) {
+  for (int e = threadIdx.x; e < RP * RP; e += blockDim.x) {
+    const int i = e >> 5, j = e & 31;
+    const int ri = (i >= 16 && j < 16) ? j : i, rj = (i >= 16 && j < 16) ? i : j;
+    double a = 0.0;
+#pragma unroll
+    for (int w = 0; w < NWARP; ++w) a += (double)part[(size_t)w * RP * LP + ri * LP + rj];
+    W[i * LW + j] = (float)a;
+  }
+  __syncthreads();
+  double mx = 0.0;
+  for (int e = threadIdx.x; e < RP * RP; e += blockDim.x) {
+    const int i = e >> 5, j = e & 31;
+    if (i < j) {
+      const double d = (double)W[i * LW + i] * (double)W[j * LW + j];
+      if (d > 0.0) mx = fmax(mx, fabs((double)W[i * LW + j]) * rsqrt(d));
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = mx;
+  __syncthreads();
+  mx = 0.0;
+#pragma unroll
+  for (int w = 0; w < NWARP; ++w) mx = fmax(mx, red[w]);
+  __syncthreads();
+  return mx;
+}
+
+// X' = Q X for this warp's column slice, written straight to the matrix (rows 0-15 -> block bi, 16-31 -> block bj).
+__device__ __forceinline__ void apply_mma(const float* Q, const float* X, int ldx, int ns, int p, float* __restrict__ gm, int rowA, int rowB) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  uint32_t qh[2][4][4], ql[2][4][4];      // [m tile][k step][fragment register]; k slot t <-> row 2t, slot t+4 <-> row 2t+1
+#pragma unroll
+  for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+    for (int ks = 0; ks < 4; ++ks) {
+      const float2 u = *reinterpret_cast<const float2*>(Q + (16 * mt + g) * LQ + 8 * ks + 2 * t);
+      const float2 v = *reinterpret_cast<const float2*>(Q + (16 * mt + g + 8) * LQ + 8 * ks + 2 * t);
+      split3(u.x, qh[mt][ks][0], ql[mt][ks][0]); split3(v.x, qh[mt][ks][1], ql[mt][ks][1]);
+      split3(u.y, qh[mt][ks][2], ql[mt][ks][2]); split3(v.y, qh[mt][ks][3], ql[mt][ks][3]);
+    }
+  for (int n0 = warp * ns; n0 < (warp + 1) * ns; n0 += 8) {
+    if (n0 >= p) break;
+    float accM[2][4], accS[2][4];
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+      for (int j = 0; j < 4; ++j) { accM[i][j] = 0.f; accS[i][j] = 0.f; }
+#pragma unroll
+    for (int ks = 0; ks < 4; ++ks) {
+      uint32_t bh0, bl0, bh1, bl1;
+      split3(X[(size_t)(8 * ks + 2 * t) * ldx + n0 + g], bh0, bl0);
+      split3(X[(size_t)(8 * ks + 2 * t + 1) * ldx + n0 + g], bh1, bl1);
+#pragma unroll
+      for (int mt = 0; mt < 2; ++mt) {
+        mma_tf32(accS[mt], ql[mt][ks][0], ql[mt][ks][1], ql[mt][ks][2], ql[mt][ks][3], bh0, bh1);
+        mma_tf32(accS[mt], qh[mt][ks][0], qh[mt][ks][1], qh[mt][ks][2], qh[mt][ks][3], bl0, bl1);
+        mma_tf32(accM[mt], qh[mt][ks][0], qh[mt][ks][1], qh[mt][ks][2], qh[mt][ks][3], bh0, bh1);
+      }
+    }
+    const int col = n0 + 2 * t;
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+      for (int hf = 0; hf < 2; ++hf) {
+        const int i = 16 * mt + g + 8 * hf;
+        const int grow = i < BR ? rowA + i : rowB + (i - BR);
+        if (grow < p) {
+          const float v0 = accM[mt][2 * hf] + accS[mt][2 * hf], v1 = accM[mt][2 * hf + 1] + accS[mt][2 * hf + 1];
+          float* dst = gm + (size_t)grow * p + col;
+          if (col + 1 < p && (p & 1) == 0) __stcg(reinterpret_cast<float2*>(dst), make_float2(v0, v1));
+          else { if (col < p) __stcg(dst, v0); if (col + 1 < p) __stcg(dst + 1, v1); }
+        }
+      }
+  }
+}
+
+static __global__ void __launch_bounds__(THREADS, 1)
+k_bjacobi_tc(int nblk, const int* pvec, const long long* moff, const int* voff, float* G, float* Vt, const float* mu, float* lam,
+             int* rotflags, int* sweeps_out, unsigned long long* sweeps_sum, int max_sweeps, double tol, const int* prob_of,
+             int* flags) {
+  extern __shared__ __align__(16) unsigned char smem_bj[];
+  cg::cluster_group cluster = cg::this_cluster();
+  const int C = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
+  const int lb = blockIdx.x / C;
+  const int p = pvec[lb];
+  const Plan pl(p);
+  float* X = reinterpret_cast<float*>(smem_bj);
+  float* part = reinterpret_cast<float*>(smem_bj + pl.off_part);
+  float* W = reinterpret_cast<float*>(smem_bj + pl.off_w);
+  float* W1 = reinterpret_cast<float*>(smem_bj + pl.off_w1);
+  float* Q = reinterpret_cast<float*>(smem_bj + pl.off_q);
+  double* red = reinterpret_cast<double*>(smem_bj + pl.off_red);
+  int* pairs = reinterpret_cast<int*>(smem_bj + pl.off_pairs);
+  float* g = G + moff[lb];
+  int* rf = rotflags + lb * MAXSW;
+  const int ldx = pl.ldx, ks = pl.pk / NWARP;
+  const int NB = (p + BR - 1) / BR, NBe = (NB + 1) & ~1, NP = NBe >> 1;
+  // inner pair table: rounds 0-15 cross pairs (q, 16 + (q + r) mod 16), rounds 16-30 the pairs inside each block
+  for (int t = threadIdx.x; t < (RP - 1) * BR; t += blockDim.x) {
+    const int r = t / BR, q = t - r * BR;
+    int i, j;
+    if (r < BR) { i = q; j = BR + ((q + r) & (BR - 1)); }
+    else { rr_pair(r - BR, q & 7, BR, i, j); if (q >= 8) { i += BR; j += BR; } }
+    pairs[t] = i | (j << 16);
+  }
+  for (int t = threadIdx.x; t < RP * ldx; t += blockDim.x) X[t] = 0.f;    // the pads stay zero
+  __syncthreads();
+  const float thresh = (float)(0.25 * tol);
+  const float quad_exit = (float)sqrt(tol / (16.0 * sqrt((double)p)));
+  int sweep = 0;
+  bool capped = true;
+  for (; sweep < max_sweeps; ++sweep) {
+    for (int r = 0; r < NBe - 1; ++r) {
+      for (int q = rank; q < NP; q += C) {
+        int bi, bj2; rr_pair(r, q, NBe, bi, bj2);
+        load_pair(g, p, bi, bj2, X, ldx);
+        __syncthreads();
+        gram_mma(X, ldx, ks, part);
+        __syncthreads();
+        const double mx = gram_reduce(part, W, red);
+        if (mx > tol) {
+          inner_sweep<float, RP>(W, W1, Q, thresh, pairs, reinterpret_cast<unsigned*>(red + 40));
+          apply_mma(Q, X, ldx, ks, p, g, bi * BR, bj2 * BR);
+          if (threadIdx.x == 0) atomicMax(reinterpret_cast<unsigned*>(rf) + sweep, __float_as_uint((float)mx));
+        }
+        __syncthreads();
+      }
+      cluster.sync();
+    }
+    const unsigned worst = (unsigned)__ldcg(rf + sweep);
+    if (!worst) { capped = false; break; }
+    if (__uint_as_float(worst) <= quad_exit) { ++sweep; capped = false; break; }
+  }
+  const int lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+  const double m = (double)mu[lb];
+  float* vt = Vt + moff[lb];
+  for (int i = rank * nw + (threadIdx.x >> 5); i < p; i += C * nw) {
+    double a = 0.0;
+    for (int c = lane; c < p; c += 32) { const double x = (double)__ldcg(g + (size_t)i * p + c); a += x * x; }
+    a = warp_sum(a);
+    const double na = sqrt(a);
+    if (lane == 0) lam[voff[lb] + i] = (float)(na - m);
+    const double inv = na > 0.0 ? 1.0 / na : 0.0;
+    for (int c = lane; c < p; c += 32) vt[(size_t)i * p + c] = (float)((double)__ldcg(g + (size_t)i * p + c) * inv);
+  }
+  if (rank == 0 && threadIdx.x == 0) {
+    atomicMax(sweeps_out, sweep);
+    if (sweeps_sum) atomicAdd(sweeps_sum, (unsigned long long)sweep);
+    if (capped && flags) atomicOr(flags + prob_of[lb], FLAG_EIG_CAP);
+  }
+}
+
+inline size_t smem_bytes(int p) { return Plan(p).bytes; }
+}  // namespace tcv
+
 
 }  // namespace bj
 }  // namespace cdu

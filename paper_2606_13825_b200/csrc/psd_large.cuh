@@ -41,7 +41,7 @@ constexpr int LARGE_NCH = 32;   // CTAs per block in the chunked glue kernels
 template <typename T>
 __global__ void __launch_bounds__(256) k_large_smat(PsdTab tab, LargeTab lt, const double* v, const double* v2,
                                                     Hyper<T> H, int k, int use_rho_scale, int shift, T* G, T* Vt, T* mu,
-                                                    double* wprev, const T* lmax, T* Splain, double* scr, unsigned* tick) {
+                                                    double* wprev, const T* lmax, T* Splain, double* scr, unsigned* tick, int* flags) {
   __shared__ double sh[64];
   __shared__ unsigned last;
   const int lb = blockIdx.y, blk = lt.gblk[lb], nch = gridDim.x, ch = blockIdx.x;
@@ -113,6 +113,7 @@ __global__ void __launch_bounds__(256) k_large_smat(PsdTab tab, LargeTab lt, con
   double n2 = 0.0, d2 = 0.0;
   for (int c = 0; c < nch; ++c) { n2 += __ldcg(scr + ((size_t)lb * LARGE_NCH + c) * 2); d2 += __ldcg(scr + ((size_t)lb * LARGE_NCH + c) * 2 + 1); }
   double m = sqrt(n2);
+  if (!(m <= 1.7e308) && flags && threadIdx.x == 0) atomicOr(flags + tab.prob[blk], FLAG_NONFINITE);   // NaN or Inf in w
   if (shift == 2) {
     const double weyl = 1.5 * (1.02 * (double)lmax[lb] + sqrt(d2)) + 1e-30;
     if (weyl < m) m = weyl;
@@ -125,30 +126,13 @@ __global__ void __launch_bounds__(256) k_large_smat(PsdTab tab, LargeTab lt, con
   }
 }
 
-// Dense-input variant for the stand-alone entry points: G = S + mu I, Vt = I.
-template <typename T>
-__global__ void __launch_bounds__(1024) k_large_dense_init(int p, const T* S, T* G, T* Vt, T* mu) {
-  __shared__ double sh[32];
-  const long long off = (long long)blockIdx.x * p * p;
-  double acc[1] = {0.0};
-  for (long long t = threadIdx.x; t < (long long)p * p; t += blockDim.x) { const double x = (double)S[off + t]; acc[0] += x * x; }
-  block_sum<1>(acc, sh);
-  const double m = sqrt(acc[0]);
-  if (threadIdx.x == 0) mu[blockIdx.x] = (T)m;
-  for (long long t = threadIdx.x; t < (long long)p * p; t += blockDim.x) {
-    const int r = (int)(t / p), c = (int)(t - (long long)r * p);
-    G[off + t] = S[off + t] + ((r == c) ? (T)m : (T)0);
-    Vt[off + t] = (r == c) ? (T)1 : (T)0;
-  }
-}
-
 constexpr int HESTENES_MAXSW = 64;
 
 // One cluster per matrix. G, Vt: p x p row-major with column i of the working matrix stored as row i.
 template <typename T, int NE>
 __global__ void __launch_bounds__(512) k_hestenes(int nblk, const int* pvec, const long long* moff, const int* voff, T* G, T* Vt,
                                                   const T* mu, T* lam, int* rotflags, int* sweeps_out, unsigned long long* sweeps_sum,
-                                                  int max_sweeps, double tol) {
+                                                  int max_sweeps, double tol, const int* prob_of, int* flags) {
   cg::cluster_group cluster = cg::this_cluster();
   const int C = cluster.num_blocks();
   const int lb = blockIdx.x / C, rank = cluster.block_rank();
@@ -198,6 +182,7 @@ __global__ void __launch_bounds__(512) k_hestenes(int nblk, const int* pvec, con
     const int rot = __ldcg(rf + sweep);
     if (!rot) break;
   }
+  if (sweep >= max_sweeps && flags && rank == 0 && threadIdx.x == 0) atomicOr(flags + prob_of[lb], FLAG_EIG_CAP);
   // eigenvalues
   for (int i = gw; i < p; i += wtot) {
     double a = 0.0;

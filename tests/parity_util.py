@@ -114,20 +114,49 @@ def compare(wl, ref, res, per_problem):
     return e
 
 
-def full_cotangent(wl, ref):
-    """Cotangent list for the whole batch: the oracle's for compared problems, zeros elsewhere."""
+def full_cotangent(wl, ref, fill_seed=None):
+    """Cotangent list for the whole batch: the oracle's for compared problems; elsewhere zeros, or (fill_seed given)
+    seeded N(0,1) scaled to the compared problems' cotangents, so that the backward of EVERY problem does real work."""
     cots = [(np.zeros(pr.n), np.zeros(pr.m), np.zeros(pr.m)) for pr in wl.problems]
+    if fill_seed is not None:
+        rng = np.random.default_rng(fill_seed)
+        sc = max([float(np.max(np.abs(c))) for cot in ref["cot"] for c in cot if c.size] + [1e-30])
+        cots = [tuple(round_to(sc * rng.standard_normal(k), wl.dtype) for k in (pr.n, pr.m, pr.m)) for pr in wl.problems]
     for j, b in enumerate(ref["idx"]):
         cots[b] = ref["cot"][j]
     return cots
 
 
-def check(wl, problems=None, per_problem=None, x_star=None, ckpt_mode=0, host=False, tol_scale=1.0, **opts):
-    """Oracle vs GPU on `problems` (default: all). Returns (errors, stats)."""
+def assert_batch_sane(wl, res, rel_tol):
+    """Every problem of the batch (not only the ones compared with the oracle): all outputs finite and s_K inside its
+    cone (oracle.cones.in_cone) up to rel_tol x the scale of the iterate."""
+    from oracle import cones as C
+    for k in ("xK", "sK", "yK", "g_x0", "g_s0", "g_y0"):
+        for b, v in enumerate(res[k]):
+            assert np.all(np.isfinite(v)), f"{k} of problem {b} is not finite"
+    for k in ("g_rho", "g_alpha", "g_sigma"):
+        assert np.all(np.isfinite(res[k])), k
+    for b, pr in enumerate(wl.problems):
+        s = res["sK"][b]
+        sc = max(float(np.max(np.abs(s), initial=0.0)), float(np.max(np.abs(res["xK"][b]), initial=0.0)), 1e-30)
+        r = 0
+        for kind, dim in pr.cones:
+            rows = W.cone_rows(kind, dim)
+            assert C.in_cone(kind, dim, s[r:r + rows], tol=rel_tol * sc), f"s_K of problem {b} leaves cone ({kind},{dim})"
+            r += rows
+
+
+def check(wl, problems=None, per_problem=None, x_star=None, ckpt_mode=0, host=False, tol_scale=1.0, fill_seed=None,
+          sane_tol=None, **opts):
+    """Oracle vs GPU on `problems` (default: all). Returns (errors, stats). fill_seed: random cotangents on the problems
+    that are not compared (needs per-problem hyper-parameters); sane_tol: also run assert_batch_sane on the whole batch."""
     ref = oracle_reference(wl, problems, x_star)
     if per_problem is None:
         per_problem = problems is not None and len(list(problems)) != wl.batch
-    res = gpu_run(wl, full_cotangent(wl, ref), ckpt_mode=ckpt_mode, per_problem=per_problem, host=host, **opts)
+    assert fill_seed is None or per_problem
+    res = gpu_run(wl, full_cotangent(wl, ref, fill_seed), ckpt_mode=ckpt_mode, per_problem=per_problem, host=host, **opts)
+    if sane_tol is not None:
+        assert_batch_sane(wl, res, sane_tol)
     e = compare(wl, ref, res, per_problem)
     return e, res["stats"]
 

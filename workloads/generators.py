@@ -263,15 +263,17 @@ def lovasz_dual_feasible_start(pr: Problem):
 
 
 def make_config(cfg: int, batch: Optional[int] = None, K: Optional[int] = None,
-                p: Optional[int] = None, seed_offset: int = 0) -> Workload:
+                p: Optional[int] = None, seed_offset: int = 0, dtype: Optional[str] = None) -> Workload:
     """BASELINE.json configs[cfg-1] with the recipes of SURVEY.md 8(d). `batch`, `K`, `p` (graph order /
     number of variables for cfg3) override the full sizes for down-scaled parity cases; `seed_offset` shifts the
-    instance seeds (hyper-parameters stay shared) so that every rank of a weak-scaling run draws its own batch."""
+    instance seeds (hyper-parameters stay shared) so that every rank of a weak-scaling run draws its own batch;
+    `dtype` overrides the config's precision (parity cases that push the fp64 kernels through the large-block path)."""
     full = {1: (4, 20, 10), 2: (256, 50, 50), 3: (1024, 100, 200), 4: (64, 100, 100), 5: (8, 200, 512)}[cfg]
     B = batch if batch is not None else full[0]
     Kk = K if K is not None else full[1]
     pp = p if p is not None else full[2]
-    dtype = "f64" if cfg == 1 else "f32"
+    dtype_cfg = "f64" if cfg == 1 else "f32"
+    dtype = dtype if dtype is not None else dtype_cfg
     hrng = np.random.default_rng(BASE_SEED + 1000 * cfg + 999)
     problems = []
     for b in range(B):
@@ -305,8 +307,8 @@ def make_config(cfg: int, batch: Optional[int] = None, K: Optional[int] = None,
         else:
             a, b_, c = np.zeros(pr.n), np.zeros(pr.m), np.zeros(pr.m)
         x0.append(_round_to(a, dtype)); s0.append(_round_to(b_, dtype)); y0.append(_round_to(c, dtype))
-    return Workload(name=CONFIG_NAMES[cfg] if (batch, K, p) == (None, None, None) else
-                    f"cfg{cfg}-p{pp}-b{B}-K{Kk}", dtype=dtype, problems=problems, K=Kk,
+    return Workload(name=CONFIG_NAMES[cfg] if (batch, K, p) == (None, None, None) and dtype == dtype_cfg else
+                    f"cfg{cfg}-p{pp}-b{B}-K{Kk}-{dtype}", dtype=dtype, problems=problems, K=Kk,
                     rho=_round_to(rho, dtype), alpha=_round_to(alpha, dtype), sigma=sigma, x0=x0, s0=s0, y0=y0)
 
 
