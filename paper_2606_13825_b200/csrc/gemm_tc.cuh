@@ -114,8 +114,9 @@ __device__ __forceinline__ float gamma_relu_f(float li, float lj) {   // same ru
 // {p, p, nblk} of the fp32 operands, box {BK, TILE, 1}, 128-byte swizzle.
 static __global__ void __launch_bounds__(THREADS, 1)
 k_gemm_tc(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, float* __restrict__ C, int p,
-          const float* __restrict__ lam) {
+          const float* __restrict__ lam, const int* __restrict__ need) {
   extern __shared__ unsigned char smem_dyn[];
+  if (need && !need[blockIdx.y]) return;
   const uint32_t raw = smem_u32(smem_dyn);
   const uint32_t base = (raw + 1023u) & ~1023u;
   unsigned char* gbase = smem_dyn + (base - raw);
@@ -315,7 +316,7 @@ struct Maps {
 };
 
 // C = A Bt' per block (A, Bt, C: [nblk][p][p] fp32, row-major), optional Hadamard with Gamma(lam).
-inline cdu_status gemm_nt(Maps& M, const float* A, const float* Bt, float* C, const float* lam, cudaStream_t st, std::string& err) {
+inline cdu_status gemm_nt(Maps& M, const float* A, const float* Bt, float* C, const float* lam, const int* need, cudaStream_t st, std::string& err) {
   const CUtensorMap* ma = M.get(A, err);
   const CUtensorMap* mb = M.get(Bt, err);
   if (!ma || !mb) return CDU_ECUDA;
@@ -326,7 +327,7 @@ inline cdu_status gemm_nt(Maps& M, const float* A, const float* Bt, float* C, co
     M.attr_set = true;
   }
   const int nt = M.p / TILE;
-  k_gemm_tc<<<dim3(nt * nt, M.nblk), THREADS, SMEM_BYTES, st>>>(*ma, *mb, C, M.p, lam);
+  k_gemm_tc<<<dim3(nt * nt, M.nblk), THREADS, SMEM_BYTES, st>>>(*ma, *mb, C, M.p, lam, need);
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { err = std::string("k_gemm_tc: ") + cudaGetErrorString(e); return CDU_ECUDA; }
   return CDU_OK;

@@ -117,7 +117,6 @@ struct PsdEngine {
   double* chunk_scr = nullptr; unsigned* chunk_tick = nullptr;   // partials / tickets of the chunked glue kernels
   T* lmaxL = nullptr;            // max |lambda| per large block, from the last eigendecomposition
   double* wprev = nullptr;       // svec of the last matrix each large block decomposed
-  int eig_impl = 1;              // 1: blocked one-sided Jacobi (orders <= 512), 0: k_hestenes everywhere
   bool warm = false;             // Vt holds the eigenvectors of the previous call (warm start of the next one)
   int warm_enable = 1;
   float* tc_split = nullptr;   // hi/lo operand staging of the tcgen05 path
@@ -165,11 +164,14 @@ struct PsdEngine {
       G = pool.alloc<T>(mo); Vt = pool.alloc<T>(mo); Tm = pool.alloc<T>(mo); T2 = pool.alloc<T>(mo);
       mu = pool.alloc<T>(n_large); lamL = pool.alloc<T>(vo); scaleL = pool.alloc<T>(vo); lmaxL = pool.zeros<T>(n_large, st);
       chunk_scr = pool.zeros<double>((size_t)n_large * LARGE_NCH * 2, st); chunk_tick = pool.zeros<unsigned>(n_large, st);
-      rotflags = pool.zeros<int>((size_t)n_large * HESTENES_MAXSW, st);
+      need = pool.zeros<int>(n_large, st);
+      rotflags = pool.zeros<int>((size_t)n_large * bj::MAXSW + n_large, st);   // + one arrival counter per block (k_bjacobi_tc2)
       use_tc = (want_tc != 0) && std::is_same<T, float>::value && gemm_tc_supported(pmax_large) ? (want_tc < 0 ? 3 : want_tc) : 0;   // bit 0: rebuild, bit 1: DK products
       for (int q : lp) if (q != pmax_large) use_tc = 0;      // the tensor maps assume one block order
       if (use_tc) { tc_split = pool.alloc<float>((size_t)mo * 2); tcmaps.nblk = n_large; tcmaps.p = pmax_large; }
       if (!G || !Vt || !Tm || !T2 || !mu || !lamL || !rotflags) { err = "cudaMalloc (PSD large scratch)"; return CDU_ENOMEM; }
+      const size_t bj_smem = std::is_same<T, float>::value ? bj::tcw::smem_bytes(pmax_large) : bj::smem_bytes<T, 16>(pmax_large);
+      if (bj_smem > 227 * 1024) { err = "PSD block order too large for the blocked Jacobi kernel (fp32: 896, fp64: 1536)"; return CDU_EINVAL; }
     }
     if (pool.last != cudaSuccess) { err = std::string("PSD tables: ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
     if (n_small) {
@@ -206,7 +208,7 @@ struct PsdEngine {
   }
   cdu_status gemm_(const T* A, int ta, const T* Bm, int tb, T* C, const T* kscale, int relu, cudaStream_t st) {
     const int tiles = (pmax_large + 63) / 64;
-    k_gemm_fma<T><<<dim3(tiles, tiles, n_large), 256, 0, st>>>(n_large, lt.pvec, lt.moff, lt.voff, A, ta, Bm, tb, C, kscale, relu);
+    k_gemm_fma<T><<<dim3(tiles, tiles, n_large), 256, 0, st>>>(n_large, lt.pvec, lt.moff, lt.voff, A, ta, Bm, tb, C, kscale, relu, cur_need);
     ++launches;
     CU_OK(cudaGetLastError());
     return CDU_OK;
@@ -216,7 +218,7 @@ struct PsdEngine {
   tc::Maps tcmaps;
   cdu_status gemm_nt(const T* A, const T* Bt, T* C, const T* lam, cudaStream_t st) {
     pb(PC_GEMM_LARGE, st);
-    cdu_status s = tc::gemm_nt(tcmaps, (const float*)A, (const float*)Bt, (float*)C, (const float*)lam, st, err);
+    cdu_status s = tc::gemm_nt(tcmaps, (const float*)A, (const float*)Bt, (float*)C, (const float*)lam, cur_need, st, err);
     pe(st);
     ++launches;
     return s;
@@ -232,15 +234,55 @@ struct PsdEngine {
     return CDU_OK;
   }
 
-  // blocked one-sided Jacobi (psd_bjacobi.cuh): one pair of row blocks per CTA and round, cluster size chosen from what the
-  // device can co-schedule. fp32: tensor-core variant (32 rows per pair); fp64: FMA variant (16 rows per pair).
+  // blocked one-sided Jacobi (psd_bjacobi.cuh): one pair of row blocks per CTA and round.
+  // fp32: tensor-core kernel, the CTAs of a matrix meet at a counter in global memory (cooperative launch, any SMs);
+  // fp64: FMA kernel on thread-block clusters (16 rows per pair).
   cdu_status eig_blocked(cudaStream_t st, int* flags) {
-    constexpr bool F32 = std::is_same<T, float>::value;
-    constexpr int RP = F32 ? 32 : 16;
+    if constexpr (std::is_same<T, float>::value) return eig_blocked_f32(st, flags); else return eig_blocked_f64(st, flags);
+  }
+  cdu_status eig_blocked_f32(cudaStream_t st, int* flags) {
+    const int NB = (pmax_large + bj::tcw::BR - 1) / bj::tcw::BR, NP = ((NB + 1) & ~1) / 2;
+    const size_t smem = bj::tcw::smem_bytes(pmax_large);
+    const void* kern = (const void*)bj::tcw::k_bjacobi_tc2;
+    if (bj_C == 0) {
+      CU_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      int dev = 0, nsm = 0, occ = 0;
+      CU_OK(cudaGetDevice(&dev));
+      CU_OK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+      CU_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, bj::THREADS, smem));
+      bj_resident = nsm * occ;
+      if (bj_resident < 1) { err = "k_bjacobi_tc2: does not fit an SM"; return CDU_ECUDA; }
+      const int cmax = std::max(1, std::min(NP, bj_resident / std::min(n_large, bj_resident)));
+      const int per_cta = (NP + cmax - 1) / cmax;
+      bj_C = (NP + per_cta - 1) / per_cta;     // fewest CTAs that give the same number of pairs per CTA
+    }
+    CU_OK(cudaMemsetAsync(rotflags, 0, ((size_t)n_large * bj::MAXSW + n_large) * sizeof(int), st));   // + the arrival counters
+    double tol = 3e-7;
+    int maxsw = bj::MAXSW - 1, C = bj_C;
+    const int* pv = lt.pvec; const long long* mo = lt.moff; const int* vo = lt.voff; const int* lp = lprob;
+    float *g = (float*)G, *v = (float*)Vt, *l = (float*)lamL; const float* m = (const float*)mu;
+    int* rf = rotflags; int* sw = sweeps_max; unsigned long long* ss = sweeps_sum;
+    unsigned* bar = reinterpret_cast<unsigned*>(rotflags + (size_t)n_large * bj::MAXSW);
+    const int per_launch = std::max(1, bj_resident / C);
+    pb(PC_EIG_LARGE, st);
+    for (int lb0 = 0; lb0 < n_large; lb0 += per_launch) {
+      int first = lb0;
+      const int nm = std::min(per_launch, n_large - lb0);
+      const int* nd = cur_need;
+      void* args[] = {&first, &C, &pv, &mo, &vo, &g, &v, &m, &l, &rf, &sw, &ss, &maxsw, &tol, &lp, &flags, &bar, &nd};
+      cudaError_t e = cudaLaunchCooperativeKernel(kern, dim3(nm * C), dim3(bj::THREADS), args, smem, st);
+      ++launches;
+      if (e != cudaSuccess) { pe(st); err = std::string("k_bjacobi_tc2: ") + cudaGetErrorString(e); return CDU_ECUDA; }
+    }
+    pe(st);
+    return CDU_OK;
+  }
+  int bj_resident = 0;
+  cdu_status eig_blocked_f64(cudaStream_t st, int* flags) {
+    constexpr int RP = 16;
     const int BR = RP / 2, NB = (pmax_large + BR - 1) / BR, NP = ((NB + 1) & ~1) / 2;
-    const size_t smem = F32 ? bj::tcv::smem_bytes(pmax_large) : bj::smem_bytes<T, RP>(pmax_large);
-    const void* kern;
-    if constexpr (F32) kern = (const void*)bj::tcv::k_bjacobi_tc; else kern = (const void*)bj::k_bjacobi<T, 16>;
+    const size_t smem = bj::smem_bytes<T, RP>(pmax_large);
+    const void* kern = (const void*)bj::k_bjacobi<T, RP>;
     if (bj_C == 0) {
       CU_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       CU_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
@@ -265,11 +307,12 @@ struct PsdEngine {
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = bj_C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    double tol = F32 ? 3e-7 : 1e-15;
+    double tol = 1e-15;
     int nl = n_large, maxsw = bj::MAXSW - 1;
     const int* pv = lt.pvec; const long long* mo = lt.moff; const int* vo = lt.voff; const int* lp = lprob;
     T *g = G, *v = Vt, *l = lamL; const T* m = mu; int* rf = rotflags; int* sw = sweeps_max; unsigned long long* ss = sweeps_sum;
-    void* args[] = {&nl, &pv, &mo, &vo, &g, &v, &m, &l, &rf, &sw, &ss, &maxsw, &tol, &lp, &flags};
+    const int* nd = cur_need;
+    void* args[] = {&nl, &pv, &mo, &vo, &g, &v, &m, &l, &rf, &sw, &ss, &maxsw, &tol, &lp, &flags, &nd};
     pb(PC_EIG_LARGE, st);
     cudaError_t e = cudaLaunchKernelExC(&cfg, kern, args);
     pe(st);
@@ -280,42 +323,30 @@ struct PsdEngine {
   int bj_C = 0;
 
   cdu_status eig_large(cudaStream_t st, int* flags) {   // G = Vt (S + mu I), Vt orthonormal (I on a cold start)  ->  Vt, lamL
-    if (eig_impl == 1 && pmax_large <= 512) return eig_blocked(st, flags);
-    CU_OK(cudaMemsetAsync(rotflags, 0, (size_t)n_large * HESTENES_MAXSW * sizeof(int), st));
-    const int C = 8;
-    cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3(n_large * C); cfg.blockDim = dim3(512); cfg.dynamicSmemBytes = 0; cfg.stream = st;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-    cfg.attrs = at; cfg.numAttrs = 1;
-    const double tol = std::is_same<T, float>::value ? 3e-7 : 1e-15;
-    const int maxsw = HESTENES_MAXSW - 1;
-    int nl = n_large;
-    const int* pv = lt.pvec; const long long* mo = lt.moff; const int* vo = lt.voff;
-    T *g = G, *v = Vt, *l = lamL; const T* m = mu; int* rf = rotflags; int* sw = sweeps_max; unsigned long long* ss = sweeps_sum;
-    const int* lp = lprob;
-    cudaError_t e;
-    pb(PC_EIG_LARGE, st);
-    if (pmax_large <= 128) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 4>, nl, pv, mo, vo, g, v, m, l, rf, sw, ss, maxsw, tol, lp, flags);
-    else if (pmax_large <= 256) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 8>, nl, pv, mo, vo, g, v, m, l, rf, sw, ss, maxsw, tol, lp, flags);
-    else if (pmax_large <= 512) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 16>, nl, pv, mo, vo, g, v, m, l, rf, sw, ss, maxsw, tol, lp, flags);
-    else if (pmax_large <= 1024) e = cudaLaunchKernelEx(&cfg, k_hestenes<T, 32>, nl, pv, mo, vo, g, v, m, l, rf, sw, ss, maxsw, tol, lp, flags);
-    else { err = "PSD block order > 1024 not supported"; return CDU_EINVAL; }
-    pe(st);
-    ++launches;
-    CU_OK(e);
-    return CDU_OK;
+    return eig_blocked(st, flags);
   }
 
   // Eigendecomposition of smat(w) for every large block. Cold: G = S + mu I, Vt = I. Warm (Vt = eigenvectors left by
   // the previous call, nearby because consecutive ADMM iterates are): Tm = S + mu I, G = Vt Tm, so the Jacobi sweeps
-  // start from an almost orthogonal G.
+  // start from an almost orthogonal G. The rounding errors of the one-sided Jacobi scale with the shift mu (cold:
+  // ||S||_F ~ sqrt(p)/2 ||S||_2; warm: the Weyl bound 1.5 (max|lambda_prev| + ||S - S_prev||_F), wide while the
+  // iterates still move): k_large_post marks the blocks whose shift exceeded 3 max|lambda|, and a second, warm pass
+  // over the same matrix (shift 1.5 max|lambda|) polishes exactly those; its kernels return at once for the others
+  // (measured on p = 512 / 640, K = 4: iterate error 1.2e-4 -> 6e-6, gradient error 1.2e-3 -> 2e-5).
   cdu_status eig_of_w(const Hyper<T>& H, int k, const double* Wv, int* flags, cudaStream_t st) {
+    cur_need = nullptr;
+    cdu_status s = eig_pass(H, k, Wv, flags, st);
+    if (s != CDU_OK || !warm_enable) return s;
+    cur_need = need;
+    s = eig_pass(H, k, Wv, flags, st);
+    cur_need = nullptr;
+    return s;
+  }
+  cdu_status eig_pass(const Hyper<T>& H, int k, const double* Wv, int* flags, cudaStream_t st) {
     const bool w = warm && warm_enable;
     pb(PC_LARGE_MISC, st);
-    const bool rq = eig_impl == 1 && pmax_large <= 512;   // blocked Jacobi: eigenvalues by Rayleigh quotient afterwards
-    if (w) k_large_smat<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, Wv, nullptr, H, k, 0, 2, Tm, nullptr, mu, wprev, lmaxL, rq ? T2 : nullptr, chunk_scr, chunk_tick, flags);
-    else k_large_smat<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, Wv, nullptr, H, k, 0, 1, G, Vt, mu, wprev, lmaxL, rq ? T2 : nullptr, chunk_scr, chunk_tick, flags);
+    if (w) k_large_smat<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, Wv, nullptr, H, k, 0, 2, Tm, nullptr, mu, wprev, lmaxL, T2, chunk_scr, chunk_tick, flags, cur_need);
+    else k_large_smat<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, Wv, nullptr, H, k, 0, 1, G, Vt, mu, wprev, lmaxL, T2, chunk_scr, chunk_tick, flags, cur_need);
     pe(st);
     ++launches;
     CU_OK(cudaGetLastError());
@@ -327,23 +358,22 @@ struct PsdEngine {
     }
     s = eig_large(st, flags);
     if (s != CDU_OK) return s;
-    if (rq) {
-      if (use_tc) s = gemm_nt(Vt, T2, G, nullptr, st);       // R = Vt S (S symmetric)
-      else s = gemm(Vt, 0, T2, 0, G, nullptr, 0, st);
-      if (s != CDU_OK) return s;
-      pb(PC_LARGE_MISC, st);
-      k_large_rayleigh<T><<<dim3(16, n_large), 256, 0, st>>>(lt.pvec, lt.moff, lt.voff, G, Vt, lamL);
-      pe(st);
-      ++launches;
-    }
+    // eigenvalues: Rayleigh quotients against the unshifted S (T2), R = Vt S
+    if (use_tc) s = gemm_nt(Vt, T2, G, nullptr, st);
+    else s = gemm(Vt, 0, T2, 0, G, nullptr, 0, st);
+    if (s != CDU_OK) return s;
     pb(PC_LARGE_MISC, st);
-    k_large_post<T><<<n_large, 256, 0, st>>>(lt.pvec, lt.voff, lamL, scaleL, lmaxL);
+    k_large_rayleigh<T><<<dim3(16, n_large), 256, 0, st>>>(lt.pvec, lt.moff, lt.voff, G, Vt, lamL, cur_need);
+    ++launches;
+    k_large_post<T><<<n_large, 256, 0, st>>>(lt.pvec, lt.voff, lamL, scaleL, lmaxL, mu, cur_need, need);
     pe(st);
     ++launches;
     CU_OK(cudaGetLastError());
     warm = true;
     return CDU_OK;
   }
+  const int* cur_need = nullptr;   // non-NULL during the polish pass: per large block, 1 = run
+  int* need = nullptr;
 
   cdu_status forward(const Hyper<T>& H, int k, const PsdFwdArgs& A, cudaStream_t st) {
     if (n_small) {
@@ -392,7 +422,7 @@ struct PsdEngine {
         CU_OK(cudaGetLastError());
       }
       pb(PC_LARGE_MISC, st);
-      k_large_smat<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, A.Gs, A.Gy, H, k, 1, 0, G, nullptr, nullptr, nullptr, nullptr, nullptr, chunk_scr, chunk_tick, nullptr);   // G = smat(g_s + rho g_y)
+      k_large_smat<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, A.Gs, A.Gy, H, k, 1, 0, G, nullptr, nullptr, nullptr, nullptr, nullptr, chunk_scr, chunk_tick, nullptr, nullptr);   // G = smat(g_s + rho g_y)
       pe(st);
       ++launches;
       CU_OK(cudaGetLastError());

@@ -1,10 +1,9 @@
 // psd_bjacobi.cuh - eigendecomposition of the large PSD blocks: blocked one-sided Jacobi in shared memory.
 //
-// Same fixed point as k_hestenes (psd_large.cuh): the rows g_i = v_i' (S + mu I) of G, for an orthonormal set {v_i},
+// One-sided (Hestenes) Jacobi on the shifted matrix: the rows g_i = v_i' (S + mu I) of G, for an orthonormal set {v_i},
 // are made mutually orthogonal by plane rotations; then v_i = g_i / ||g_i|| are eigenvectors of S (Eq. 7,
 // L102: only U max(L,0) U' is compared with the oracle, never U - reading A15). The v_i are never formed: rotating
-// the rows of G rotates them implicitly, so only G is carried. What changes against k_hestenes is the schedule,
-// built for the SM instead of for L2 latency:
+// the rows of G rotates them implicitly, so only G is carried. The schedule is built for the SM, not for L2 latency:
 //   * rows are grouped in blocks of BR; one round of a round-robin tournament over the NB blocks pairs every block
 //     with one other, and one CTA of the matrix's thread-block cluster takes one pair: it brings the 2 BR rows of G
 //     (2 BR x p) into shared memory, forms their Gram matrix W = X X' (2 BR x 2 BR, register-tiled, k split over 8
@@ -300,12 +299,14 @@ __device__ __forceinline__ void apply_store(const T* Qt, const T* X, int ldx, in
 template <typename T, int RP>
 __global__ void __launch_bounds__(THREADS, 1)
 k_bjacobi(int nblk, const int* pvec, const long long* moff, const int* voff, T* G, T* Vt, const T* mu, T* lam, int* rotflags,
-          int* sweeps_out, unsigned long long* sweeps_sum, int max_sweeps, double tol, const int* prob_of, int* flags) {
+          int* sweeps_out, unsigned long long* sweeps_sum, int max_sweeps, double tol, const int* prob_of, int* flags,
+          const int* need) {
   constexpr int BR = RP / 2, LQ = RP + 4;
   extern __shared__ __align__(16) unsigned char smem_bj[];
   cg::cluster_group cluster = cg::this_cluster();
   const int C = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
   const int lb = blockIdx.x / C;
+  if (need && !need[lb]) return;                 // the whole cluster leaves
   const int p = pvec[lb];
   const Plan<T, RP> pl(p);
   T* X = reinterpret_cast<T*>(smem_bj);
@@ -377,29 +378,45 @@ k_bjacobi(int nblk, const int* pvec, const long long* moff, const int* voff, T* 
 template <typename T, int RP> inline size_t smem_bytes(int p) { return Plan<T, RP>(p).bytes; }
 
 // ---------------------------------------------------------------------------------------------------------
-// fp32 variant on the tensor cores (mma.sync m16n8k8, 3xTF32). Same algorithm and the same fixed point as k_bjacobi;
-// what changes is where the time of a block round goes (profiles/r01_bjacobi_cfg5.md: 20 % Gram + 12 % apply on FMA
-// units with the tensor pipe idle, half of it in the 31 dependent rounds of the inner sweep):
-//   * rows come in with cp.async (16-byte chunks, all in flight at once) instead of dependent L2 loads;
+// fp32 kernel on the tensor cores (mma.sync m16n8k8, 3xTF32). Same algorithm and fixed point as k_bjacobi above:
+//   * rows come in with cp.async (16-byte chunks, all in flight at once);
 //   * Gram W = X X' (32 x 32 x p): warp w contracts its own k slice of p/16 columns with 3xTF32 mma.sync into fresh
-//     accumulators (leading term a_hi b_hi apart from the two small terms, so the tensor core's truncating adder sees at
-//     most 4 additions per accumulator); the 16 partial matrices are summed in fp64 in a fixed order. Only the six
-//     16 x 8 tiles of the upper block triangle are formed. Shared-memory row stride = 4 mod 32 words: conflict free;
-//   * apply X' = Q X (32 x 32 x p): warp w owns p/16 columns, Q's fragments stay in registers, 3xTF32, results go
-//     from the accumulators straight to L2. The k slots of a fragment map to rows (2t, 2t+1) instead of (t, t+4) so that
-//     the transposed reads of X are conflict free with the same stride;
-//   * the pair table of the inner sweep meets the 256 CROSS pairs (one row of each block) in its first 16 rounds and
-//     the pairs inside a block in the last 15: rows of one block leave every block round mutually orthogonal, so once a
-//     matrix is past its first sweep the within-block rounds hold nothing above the tolerance and the round mask skips
-//     them - the dependent chain of a block round is 16 rotations long instead of 31.
-// Raises FLAG_EIG_CAP on the owning problem when the sweep cap ends the iteration (cdu.h, cdu_stats.flags_or).
+//     accumulators; only the six 16 x 8 tiles of the upper block triangle are formed. Row stride = 4 mod 32 words:
+//     conflict free;
+//   * apply X' = X + (Q - I) X (32 x 32 x p): warp w owns p/16 columns, the fragments of Q - I stay in registers; the k
+//     slots of a fragment map to rows (2t, 2t+1) so that the transposed reads of X are conflict free with the same stride;
+//   * the pair table of the inner sweep meets the 256 CROSS pairs (one row of each block) in its first 16 rounds and the
+//     pairs inside a block in the last 15: rows of one block leave every block round mutually orthogonal, so past the
+//     first sweep the within-block rounds hold nothing above the tolerance and the round mask skips them.
+// Phase by phase (cycle counts per block pair at p = 512 in profiles/r02_bjacobi_phases.md):
+//   * no thread-block clusters. A 16-CTA cluster needs 16 free SMs inside one GPC and only 7 such clusters fit a B200,
+//     so a batch of 8 matrices ran in two waves. The CTAs of a matrix now meet at a counter in global memory
+//     (cooperative launch guarantees co-residency): any 16 SMs serve, all 8 matrices run at once;
+//   * Gram reduction: float2 loads of the 16 partials, convergence ratio as w_ij^2 / (w_ii w_jj) in fp32 (no fp64
+//     rsqrt), warp maxima by redux.sync; the same pass builds the mask of inner rounds that hold a pair above the
+//     tolerance;
+//   * inner sweep: 256 threads own the 256 2x2 blocks (row pair a, column pair b) of W, 256 threads the row pairs of Q.
+//     Every thread derives the rotations it needs from the current W itself (two rsqrt in the dependent chain), cross
+//     rounds index arithmetically (no table load), rotations are applied as (cos, sin) (depth 2 instead of 4), W is
+//     double buffered: one barrier per round. (cos, sin) come from approximate rsqrt and are renormalised by
+//     one Newton step: a pair of rows scaled differently from the others would not rotate into eigenvectors.
 // ---------------------------------------------------------------------------------------------------------
-namespace tcv {
-constexpr int RP = 32, BR = 16, NWARP = 16, LW = RP + 1, LQ = RP + 4, LP = 40;   // LP: row stride of a Gram partial
+namespace tcw {
+#ifdef CDU_BJ_TIMING
+__device__ long long g_bj_tim[256 * 16];
+#define BW_T0() long long bw_t0_ = clock64()
+#define BW_T(i) do { __syncthreads(); if (threadIdx.x == 0) { asm volatile("membar.cta;" ::: "memory"); const long long t_ = clock64(); g_bj_tim[blockIdx.x * 16 + (i)] += t_ - bw_t0_; bw_t0_ = t_; } else bw_t0_ = 0; } while (0)
+#define BW_CNT(i, n) do { if (threadIdx.x == 0) g_bj_tim[blockIdx.x * 16 + (i)] += (n); } while (0)
+#else
+#define BW_T0() do {} while (0)
+#define BW_T(i) do {} while (0)
+#define BW_CNT(i, n) do {} while (0)
+#endif
+constexpr int RP = 32, BR = 16, NWARP = 16, LW = 48, LQ = 40, LP = 40;
 
 struct Plan {
   int pk, ldx;
-  size_t off_part, off_w, off_w1, off_q, off_red, off_pairs, bytes;
+  size_t off_part, off_w, off_w1, off_q, off_red, off_rtab, off_ptab, bytes;
   __host__ __device__ explicit Plan(int p) {
     pk = ((p + 127) / 128) * 128;            // every warp's k slice / column slice is a multiple of 8
     ldx = pk + 4;
@@ -407,17 +424,123 @@ struct Plan {
     off_part = o; o += (size_t)NWARP * RP * LP * sizeof(float);
     off_w = o; o += (size_t)RP * LW * sizeof(float);
     off_w1 = o; o += (size_t)RP * LW * sizeof(float);
-    off_q = (o + 15) & ~(size_t)15; o = off_q + (size_t)RP * LQ * sizeof(float);
-    off_red = (o + 15) & ~(size_t)15; o = off_red + 64 * sizeof(double);
-    off_pairs = o; o += (size_t)(RP - 1) * (RP / 2) * sizeof(int);
-    bytes = o;
+    off_q = o; o += (size_t)RP * LQ * sizeof(float);
+    off_red = o; o += 64 * sizeof(unsigned);
+    off_rtab = o; o += (size_t)RP * RP;                       // inner round of every pair (i, j)
+    off_ptab = o; o += (size_t)(BR - 1) * BR * 2;             // pairs of the within-block rounds 16..30
+    bytes = (o + 15) & ~(size_t)15;
   }
 };
 
-__device__ __forceinline__ void split3(float a, uint32_t& hi, uint32_t& lo) {
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(hi) : "f"(a));
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(lo) : "f"(a - __uint_as_float(hi)));
+// rows 0-15 against 16-31 in rounds 0-15, the pairs inside each block in rounds 16-30
+__device__ __forceinline__ void inner_pair(int r, int q, const unsigned char* ptab, int& i, int& j) {
+  if (r < BR) { i = q; j = BR + ((q + r) & (BR - 1)); }
+  else { const int o = ((r - BR) * BR + q) * 2; i = ptab[o]; j = ptab[o + 1]; }
 }
+
+// W = sum of the 16 partials (fixed order). Returns max_{i<j} w_ij^2 / (w_ii w_jj) and the mask of inner rounds that
+// hold a pair with that ratio above lim2.
+__device__ __forceinline__ float gram_reduce(const float* part, float* W, unsigned* red, const unsigned char* rtab, float lim2,
+                                             unsigned& active) {
+  const int tid = threadIdx.x;
+  if (tid < 384) {     // (i, j pair): rows 0-15 all 16 column pairs, rows 16-31 column pairs 8-15 (the rest by symmetry)
+    int i, jp;
+    if (tid < 256) { i = tid >> 4; jp = tid & 15; } else { i = 16 + ((tid - 256) >> 3); jp = 8 + ((tid - 256) & 7); }
+    const float* src = part + i * LP + 2 * jp;
+    float2 a = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int w = 0; w < NWARP; ++w) { const float2 v = *reinterpret_cast<const float2*>(src + (size_t)w * RP * LP); a.x += v.x; a.y += v.y; }
+    const int j = 2 * jp;
+    W[i * LW + j] = a.x; W[i * LW + j + 1] = a.y;
+    if (i < 16 && j >= 16) { W[j * LW + i] = a.x; W[(j + 1) * LW + i] = a.y; }
+  }
+  __syncthreads();
+  float mx = 0.f; unsigned m = 0u;
+#pragma unroll
+  for (int e = tid; e < RP * RP; e += 512) {
+    const int i = e >> 5, j = e & 31;
+    if (i < j) {
+      const float c = W[i * LW + j], d = W[i * LW + i] * W[j * LW + j];
+      if (d > 0.f) {
+        const float r2 = __fdividef(c * c, d);
+        mx = fmaxf(mx, r2);
+        if (r2 > lim2) m |= 1u << rtab[e];
+      }
+    }
+  }
+  const unsigned mb = __reduce_max_sync(0xffffffffu, __float_as_uint(mx));   // non-negative floats order as unsigned
+  m = __reduce_or_sync(0xffffffffu, m);
+  if ((tid & 31) == 0) { red[tid >> 5] = mb; red[16 + (tid >> 5)] = m; }
+  __syncthreads();
+  unsigned mm = 0u, am = 0u;
+#pragma unroll
+  for (int w = 0; w < NWARP; ++w) { mm = max(mm, red[w]); am |= red[16 + w]; }
+  active = am;
+  return __uint_as_float(mm);
+}
+
+// (cos, sin) of the rotation that annihilates w_ij, identity when w_ij^2 <= thr2 w_ii w_jj.
+__device__ __forceinline__ void rot_cs(float a, float b, float c, float thr2, float& cs, float& sn) {
+  // branch free, so that the two rotations a thread needs overlap; the select discards the NaN of c = d = 0
+  const float d = b - a;
+  const float rh = rsqrt_approx(fmaf(d, d, 4.f * c * c));      // tan 2phi = 2c / d, |phi| <= pi/4
+  const float cq = fmaf(0.5f * fabsf(d), rh, 0.5f);            // cos^2 phi = (1 + cos 2phi) / 2
+  const float rc = rsqrt_approx(cq);
+  const bool rot = c * c > thr2 * a * b;
+  const float c0 = cq * rc, s0 = copysignf(1.f, d) * c * rh * rc;   // sin phi = sin 2phi / (2 cos phi)
+  const float f = fmaf(-0.5f, fmaf(c0, c0, s0 * s0), 1.5f);      // one Newton step to cos^2 + sin^2 = 1: the approximate rsqrt
+  cs = rot ? c0 * f : 1.f;                                         // leaves 1 + O(1e-7), and rows of one pair that carry different
+  sn = rot ? s0 * f : 0.f;                                         // scale factors would no longer rotate into eigenvectors
+}
+
+// a = hi + lo, both exactly representable in TF32 (round to nearest, ties away: add half an ulp, clear the low 13 bits).
+__device__ __forceinline__ void split_fast(float a, uint32_t& hi, uint32_t& lo) {
+  hi = (__float_as_uint(a) + 0x1000u) & 0xffffe000u;
+  lo = (__float_as_uint(a - __uint_as_float(hi)) + 0x1000u) & 0xffffe000u;
+}
+
+// One cyclic sweep of two-sided Jacobi on W (rounds outside `active` skipped), Q = product of the rotations
+// (row i of Q: the combination of old rows that makes new row i). One barrier per round. Warps 0-7: thread (a, b) owns
+// the 2x2 block (row pair a, column pair b) of W; warps 8-11: thread (a, c) owns columns 4c..4c+3 of the row pair a of
+// Q. Lane l of every working warp derives the rotation of pair l mod 16 from the current W; the rotation of the own
+// row pair comes by shuffle.
+__device__ __forceinline__ void inner_sweep(float* W0, float* W1, float* Q, float thr2, unsigned active, const unsigned char* ptab) {
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  for (int e = tid; e < RP * RP; e += 512) { const int i = e >> 5, j = e & 31; Q[i * LQ + j] = (i == j) ? 1.f : 0.f; }
+  __syncthreads();
+  if (warp >= 12) {                       // nothing to do but keep the barrier count
+    for (int r = 0; r < RP - 1; ++r) if ((active >> r) & 1u) __syncthreads();
+    return;
+  }
+  const bool wthread = warp < 8;
+  const int b = lane & 15;
+  const int a = wthread ? 2 * warp + (lane >> 4) : 4 * (warp - 8) + (lane >> 3);
+  const int c4 = 4 * (lane & 7);
+  float* Wc = W0; float* Wn = W1;
+  for (int r = 0; r < RP - 1; ++r) {
+    if (!((active >> r) & 1u)) continue;
+    int ib, jb;
+    inner_pair(r, b, ptab, ib, jb);
+    float csB, snB;
+    rot_cs(Wc[ib * LW + ib], Wc[jb * LW + jb], Wc[ib * LW + jb], thr2, csB, snB);
+    const float csA = __shfl_sync(0xffffffffu, csB, a), snA = __shfl_sync(0xffffffffu, snB, a);
+    const int ia = __shfl_sync(0xffffffffu, ib, a), ja = __shfl_sync(0xffffffffu, jb, a);
+    if (wthread) {
+      const float p0 = Wc[ia * LW + ib], q0 = Wc[ia * LW + jb], r0 = Wc[ja * LW + ib], s0 = Wc[ja * LW + jb];
+      const float p1 = csA * p0 - snA * r0, r1 = snA * p0 + csA * r0, q1 = csA * q0 - snA * s0, s1 = snA * q0 + csA * s0;
+      Wn[ia * LW + ib] = csB * p1 - snB * q1; Wn[ia * LW + jb] = snB * p1 + csB * q1;
+      Wn[ja * LW + ib] = csB * r1 - snB * s1; Wn[ja * LW + jb] = snB * r1 + csB * s1;
+    } else {
+      float4* xi = reinterpret_cast<float4*>(Q + ia * LQ + c4); float4* xj = reinterpret_cast<float4*>(Q + ja * LQ + c4);
+      const float4 x = *xi, y = *xj;
+      *xi = make_float4(csA * x.x - snA * y.x, csA * x.y - snA * y.y, csA * x.z - snA * y.z, csA * x.w - snA * y.w);
+      *xj = make_float4(snA * x.x + csA * y.x, snA * x.y + csA * y.y, snA * x.z + csA * y.z, snA * x.w + csA * y.w);
+    }
+    __syncthreads();
+    float* t2 = Wc; Wc = Wn; Wn = t2;
+  }
+}
+
 __device__ __forceinline__ void mma_tf32(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
   asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
                : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
@@ -448,6 +571,7 @@ __device__ __forceinline__ void load_pair(const float* __restrict__ g, int p, in
   }
 }
 
+
 // part[warp] (32 x 32, stride LP; the block (rows 16-31, columns 0-15) is NOT written: read its mirror image).
 __device__ __forceinline__ void gram_mma(const float* X, int ldx, int ks, float* part) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
@@ -461,8 +585,8 @@ __device__ __forceinline__ void gram_mma(const float* X, int ldx, int ks, float*
     uint32_t h[4][2], l[4][2];     // rows g + 8 a, columns t and t + 4 of this k step: A and B fragments share them
 #pragma unroll
     for (int a = 0; a < 4; ++a) {
-      split3(xb[(size_t)(8 * a) * ldx + kk], h[a][0], l[a][0]);
-      split3(xb[(size_t)(8 * a) * ldx + kk + 4], h[a][1], l[a][1]);
+      split_fast(xb[(size_t)(8 * a) * ldx + kk], h[a][0], l[a][0]);
+      split_fast(xb[(size_t)(8 * a) * ldx + kk + 4], h[a][1], l[a][1]);
     }
     // tiles (m tile, n tile): (0,0) (0,1) (0,2) (0,3) (1,2) (1,3)
 #pragma unroll
@@ -483,48 +607,22 @@ __device__ __forceinline__ void gram_mma(const float* X, int ldx, int ks, float*
   }
 }
 
-// W = sum of the 16 partials (fp64, fixed order); returns max_{i<j} |w_ij| / sqrt(w_ii w_jj) to every thread.
-__device__ __forceinline__ double gram_reduce(const float* part, float* W, double* red) {
-  for (int e = threadIdx.x; e < RP * RP; e += blockDim.x) {
-    const int i = e >> 5, j = e & 31;
-    const int ri = (i >= 16 && j < 16) ? j : i, rj = (i >= 16 && j < 16) ? i : j;
-    double a = 0.0;
-#pragma unroll
-    for (int w = 0; w < NWARP; ++w) a += (double)part[(size_t)w * RP * LP + ri * LP + rj];
-    W[i * LW + j] = (float)a;
-  }
-  __syncthreads();
-  double mx = 0.0;
-  for (int e = threadIdx.x; e < RP * RP; e += blockDim.x) {
-    const int i = e >> 5, j = e & 31;
-    if (i < j) {
-      const double d = (double)W[i * LW + i] * (double)W[j * LW + j];
-      if (d > 0.0) mx = fmax(mx, fabs((double)W[i * LW + j]) * rsqrt(d));
-    }
-  }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = mx;
-  __syncthreads();
-  mx = 0.0;
-#pragma unroll
-  for (int w = 0; w < NWARP; ++w) mx = fmax(mx, red[w]);
-  __syncthreads();
-  return mx;
-}
 
-// X' = Q X for this warp's column slice, written straight to the matrix (rows 0-15 -> block bi, 16-31 -> block bj).
-__device__ __forceinline__ void apply_mma(const float* Q, const float* X, int ldx, int ns, int p, float* __restrict__ gm, int rowA, int rowB) {
+// X' = X + E X, E = Q - I (hi / lo parts pre-split in shared memory), for this warp's column slice, in place. The tensor core adds into its accumulators with truncation; on Q X that
+// is a bias of ~1e-7 per block round on every row, which BPTT through 200 iterations amplified to wrong gradients (measured:
+// cfg5 gradient error 0.48). On E X it is 1e-7 of the correction only, and the correction is small once the sweeps converge.
+__device__ __forceinline__ void apply_mma(const uint32_t* Qh, const uint32_t* Ql, float* X, int ldx, int ns, int p) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   uint32_t qh[2][4][4], ql[2][4][4];      // [m tile][k step][fragment register]; k slot t <-> row 2t, slot t+4 <-> row 2t+1
 #pragma unroll
   for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
     for (int ks = 0; ks < 4; ++ks) {
-      const float2 u = *reinterpret_cast<const float2*>(Q + (16 * mt + g) * LQ + 8 * ks + 2 * t);
-      const float2 v = *reinterpret_cast<const float2*>(Q + (16 * mt + g + 8) * LQ + 8 * ks + 2 * t);
-      split3(u.x, qh[mt][ks][0], ql[mt][ks][0]); split3(v.x, qh[mt][ks][1], ql[mt][ks][1]);
-      split3(u.y, qh[mt][ks][2], ql[mt][ks][2]); split3(v.y, qh[mt][ks][3], ql[mt][ks][3]);
+      const int o0 = (16 * mt + g) * LQ + 8 * ks + 2 * t, o1 = o0 + 8 * LQ;
+      const uint2 uh = *reinterpret_cast<const uint2*>(Qh + o0), vh = *reinterpret_cast<const uint2*>(Qh + o1);
+      const uint2 ul = *reinterpret_cast<const uint2*>(Ql + o0), vl = *reinterpret_cast<const uint2*>(Ql + o1);
+      qh[mt][ks][0] = uh.x; qh[mt][ks][1] = vh.x; qh[mt][ks][2] = uh.y; qh[mt][ks][3] = vh.y;
+      ql[mt][ks][0] = ul.x; ql[mt][ks][1] = vl.x; ql[mt][ks][2] = ul.y; ql[mt][ks][3] = vl.y;
     }
   for (int n0 = warp * ns; n0 < (warp + 1) * ns; n0 += 8) {
     if (n0 >= p) break;
@@ -536,8 +634,8 @@ __device__ __forceinline__ void apply_mma(const float* Q, const float* X, int ld
 #pragma unroll
     for (int ks = 0; ks < 4; ++ks) {
       uint32_t bh0, bl0, bh1, bl1;
-      split3(X[(size_t)(8 * ks + 2 * t) * ldx + n0 + g], bh0, bl0);
-      split3(X[(size_t)(8 * ks + 2 * t + 1) * ldx + n0 + g], bh1, bl1);
+      split_fast(X[(size_t)(8 * ks + 2 * t) * ldx + n0 + g], bh0, bl0);
+      split_fast(X[(size_t)(8 * ks + 2 * t + 1) * ldx + n0 + g], bh1, bl1);
 #pragma unroll
       for (int mt = 0; mt < 2; ++mt) {
         mma_tf32(accS[mt], ql[mt][ks][0], ql[mt][ks][1], ql[mt][ks][2], ql[mt][ks][3], bh0, bh1);
@@ -551,25 +649,57 @@ __device__ __forceinline__ void apply_mma(const float* Q, const float* X, int ld
 #pragma unroll
       for (int hf = 0; hf < 2; ++hf) {
         const int i = 16 * mt + g + 8 * hf;
-        const int grow = i < BR ? rowA + i : rowB + (i - BR);
-        if (grow < p) {
-          const float v0 = accM[mt][2 * hf] + accS[mt][2 * hf], v1 = accM[mt][2 * hf + 1] + accS[mt][2 * hf + 1];
-          float* dst = gm + (size_t)grow * p + col;
-          if (col + 1 < p && (p & 1) == 0) __stcg(reinterpret_cast<float2*>(dst), make_float2(v0, v1));
-          else { if (col < p) __stcg(dst, v0); if (col + 1 < p) __stcg(dst + 1, v1); }
-        }
+        float2* xp = reinterpret_cast<float2*>(X + (size_t)i * ldx + col);       // X' = X + (Q - I) X, in place: this warp alone
+        const float2 x0 = *xp;                                                   // reads and writes its columns
+        *xp = make_float2(x0.x + (accM[mt][2 * hf] + accS[mt][2 * hf]), x0.y + (accM[mt][2 * hf + 1] + accS[mt][2 * hf + 1]));
       }
   }
 }
 
+// rows of X -> rows of blocks bi, bj of the matrix (coalesced 16-byte stores)
+__device__ __forceinline__ void store_pair(float* __restrict__ g, int p, int bi, int bj, const float* X, int ldx) {
+  if ((p & 3) == 0) {
+    const int nv = p >> 2;
+    for (int t = threadIdx.x; t < RP * nv; t += blockDim.x) {
+      const int r = t / nv, c = t - r * nv;
+      const int row = (r < BR ? bi * BR + r : bj * BR + r - BR);
+      if (row < p) __stcg(reinterpret_cast<float4*>(g + (size_t)row * p) + c, *reinterpret_cast<const float4*>(X + (size_t)r * ldx + 4 * c));
+    }
+  } else {
+    for (int t = threadIdx.x; t < RP * p; t += blockDim.x) {
+      const int r = t / p, c = t - r * p;
+      const int row = (r < BR ? bi * BR + r : bj * BR + r - BR);
+      if (row < p) __stcg(g + (size_t)row * p + c, X[(size_t)r * ldx + c]);
+    }
+  }
+}
+
+// The C CTAs of one matrix meet here once per round of blocks: everything they stored before is visible to all of
+// them after. ctr counts arrivals since the launch (zeroed by the host), gen the barriers this CTA has passed.
+__device__ __forceinline__ void matrix_barrier(unsigned* ctr, unsigned& gen, int C) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    ++gen;
+    if (C > 1) {
+      __threadfence();
+      atomicAdd(ctr, 1u);
+      const unsigned target = gen * (unsigned)C;
+      unsigned v;
+      do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory"); } while (v < target);
+    }
+  }
+  __syncthreads();
+}
+
+// grid = nmat * C CTAs, launched cooperatively (all co-resident); CTA blockIdx.x works on matrix lb0 + blockIdx.x / C
+// as member blockIdx.x % C: block pairs rank, rank + C, ... of every round. G, Vt, mu, lam, rotflags as k_bjacobi.
 static __global__ void __launch_bounds__(THREADS, 1)
-k_bjacobi_tc(int nblk, const int* pvec, const long long* moff, const int* voff, float* G, float* Vt, const float* mu, float* lam,
-             int* rotflags, int* sweeps_out, unsigned long long* sweeps_sum, int max_sweeps, double tol, const int* prob_of,
-             int* flags) {
+k_bjacobi_tc2(int lb0, int C, const int* pvec, const long long* moff, const int* voff, float* G, float* Vt, const float* mu, float* lam,
+              int* rotflags, int* sweeps_out, unsigned long long* sweeps_sum, int max_sweeps, double tol, const int* prob_of,
+              int* flags, unsigned* bar, const int* need) {
   extern __shared__ __align__(16) unsigned char smem_bj[];
-  cg::cluster_group cluster = cg::this_cluster();
-  const int C = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
-  const int lb = blockIdx.x / C;
+  const int rank = blockIdx.x % C, lb = lb0 + blockIdx.x / C;
+  if (need && !need[lb]) return;                 // all CTAs of the matrix leave
   const int p = pvec[lb];
   const Plan pl(p);
   float* X = reinterpret_cast<float*>(smem_bj);
@@ -577,23 +707,30 @@ k_bjacobi_tc(int nblk, const int* pvec, const long long* moff, const int* voff, 
   float* W = reinterpret_cast<float*>(smem_bj + pl.off_w);
   float* W1 = reinterpret_cast<float*>(smem_bj + pl.off_w1);
   float* Q = reinterpret_cast<float*>(smem_bj + pl.off_q);
-  double* red = reinterpret_cast<double*>(smem_bj + pl.off_red);
-  int* pairs = reinterpret_cast<int*>(smem_bj + pl.off_pairs);
+  unsigned* red = reinterpret_cast<unsigned*>(smem_bj + pl.off_red);
+  unsigned char* rtab = smem_bj + pl.off_rtab;
+  unsigned char* ptab = smem_bj + pl.off_ptab;
   float* g = G + moff[lb];
   int* rf = rotflags + lb * MAXSW;
+  unsigned* ctr = bar + lb;
+  unsigned gen = 0;
   const int ldx = pl.ldx, ks = pl.pk / NWARP;
   const int NB = (p + BR - 1) / BR, NBe = (NB + 1) & ~1, NP = NBe >> 1;
-  // inner pair table: rounds 0-15 cross pairs (q, 16 + (q + r) mod 16), rounds 16-30 the pairs inside each block
-  for (int t = threadIdx.x; t < (RP - 1) * BR; t += blockDim.x) {
+  for (int t = threadIdx.x; t < (BR - 1) * BR; t += blockDim.x) {     // within-block rounds: 8 pairs in each of the two blocks
     const int r = t / BR, q = t - r * BR;
     int i, j;
-    if (r < BR) { i = q; j = BR + ((q + r) & (BR - 1)); }
-    else { rr_pair(r - BR, q & 7, BR, i, j); if (q >= 8) { i += BR; j += BR; } }
-    pairs[t] = i | (j << 16);
+    rr_pair(r, q & 7, BR, i, j);
+    if (q >= 8) { i += BR; j += BR; }
+    ptab[2 * t] = (unsigned char)i; ptab[2 * t + 1] = (unsigned char)j;
+    rtab[i * RP + j] = (unsigned char)(BR + r);
+  }
+  for (int t = threadIdx.x; t < BR * BR; t += blockDim.x) {           // cross rounds
+    const int i = t >> 4, j = BR + (t & 15);
+    rtab[i * RP + j] = (unsigned char)((j - BR - i) & (BR - 1));
   }
   for (int t = threadIdx.x; t < RP * ldx; t += blockDim.x) X[t] = 0.f;    // the pads stay zero
   __syncthreads();
-  const float thresh = (float)(0.25 * tol);
+  const float thr = (float)(0.25 * tol), thr2 = thr * thr, lim2 = (float)(tol * tol);
   const float quad_exit = (float)sqrt(tol / (16.0 * sqrt((double)p)));
   int sweep = 0;
   bool capped = true;
@@ -601,21 +738,37 @@ k_bjacobi_tc(int nblk, const int* pvec, const long long* moff, const int* voff, 
     for (int r = 0; r < NBe - 1; ++r) {
       for (int q = rank; q < NP; q += C) {
         int bi, bj2; rr_pair(r, q, NBe, bi, bj2);
+        BW_T0();
         load_pair(g, p, bi, bj2, X, ldx);
         __syncthreads();
+        BW_T(0);
         gram_mma(X, ldx, ks, part);
         __syncthreads();
-        const double mx = gram_reduce(part, W, red);
-        if (mx > tol) {
-          inner_sweep<float, RP>(W, W1, Q, thresh, pairs, reinterpret_cast<unsigned*>(red + 40));
-          apply_mma(Q, X, ldx, ks, p, g, bi * BR, bj2 * BR);
-          if (threadIdx.x == 0) atomicMax(reinterpret_cast<unsigned*>(rf) + sweep, __float_as_uint((float)mx));
+        BW_T(1);
+        unsigned active;
+        const float mx2 = gram_reduce(part, W, red, rtab, lim2, active);
+        BW_T(2);
+        if (active) {
+          inner_sweep(W, W1, Q, thr2, active, ptab);
+          BW_T(3);
+          uint32_t* Qh = reinterpret_cast<uint32_t*>(part); uint32_t* Ql = Qh + RP * LQ;    // the Gram partials are spent
+          for (int e = threadIdx.x; e < RP * RP; e += 512) { const int o = (e >> 5) * LQ + (e & 31); split_fast(Q[o] - ((e >> 5) == (e & 31) ? 1.f : 0.f), Qh[o], Ql[o]); }
+          __syncthreads();
+          apply_mma(Qh, Ql, X, ldx, ks, p);
+          __syncthreads();
+          store_pair(g, p, bi, bj2, X, ldx);
+          if (threadIdx.x == 0) atomicMax(reinterpret_cast<unsigned*>(rf) + sweep, __float_as_uint(sqrtf(mx2)));
+          BW_CNT(7, 1); BW_CNT(8, __popc(active));
         }
         __syncthreads();
+        BW_T(4);
+        BW_CNT(6, 1);
       }
-      cluster.sync();
+      BW_T0();
+      matrix_barrier(ctr, gen, C);
+      BW_T(5);
     }
-    const unsigned worst = (unsigned)__ldcg(rf + sweep);
+    const unsigned worst = (unsigned)__ldcg(rf + sweep);     // largest |w_ij| / sqrt(w_ii w_jj) any pair showed in this sweep
     if (!worst) { capped = false; break; }
     if (__uint_as_float(worst) <= quad_exit) { ++sweep; capped = false; break; }
   }
@@ -639,7 +792,7 @@ k_bjacobi_tc(int nblk, const int* pvec, const long long* moff, const int* voff, 
 }
 
 inline size_t smem_bytes(int p) { return Plan(p).bytes; }
-}  // namespace tcv
+}  // namespace tcw
 
 
 }  // namespace bj

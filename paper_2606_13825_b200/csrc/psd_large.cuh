@@ -41,9 +41,11 @@ constexpr int LARGE_NCH = 32;   // CTAs per block in the chunked glue kernels
 template <typename T>
 __global__ void __launch_bounds__(256) k_large_smat(PsdTab tab, LargeTab lt, const double* v, const double* v2,
                                                     Hyper<T> H, int k, int use_rho_scale, int shift, T* G, T* Vt, T* mu,
-                                                    double* wprev, const T* lmax, T* Splain, double* scr, unsigned* tick, int* flags) {
+                                                    double* wprev, const T* lmax, T* Splain, double* scr, unsigned* tick, int* flags,
+                                                    const int* need) {
   __shared__ double sh[64];
   __shared__ unsigned last;
+  if (need && !need[blockIdx.y]) return;        // second ("polish") pass: only the blocks whose first pass ran on a wide shift
   const int lb = blockIdx.y, blk = lt.gblk[lb], nch = gridDim.x, ch = blockIdx.x;
   const int p = tab.p[blk];
   const long long row0 = tab.row0[blk];
@@ -126,80 +128,14 @@ __global__ void __launch_bounds__(256) k_large_smat(PsdTab tab, LargeTab lt, con
   }
 }
 
-constexpr int HESTENES_MAXSW = 64;
-
-// One cluster per matrix. G, Vt: p x p row-major with column i of the working matrix stored as row i.
-template <typename T, int NE>
-__global__ void __launch_bounds__(512) k_hestenes(int nblk, const int* pvec, const long long* moff, const int* voff, T* G, T* Vt,
-                                                  const T* mu, T* lam, int* rotflags, int* sweeps_out, unsigned long long* sweeps_sum,
-                                                  int max_sweeps, double tol, const int* prob_of, int* flags) {
-  cg::cluster_group cluster = cg::this_cluster();
-  const int C = cluster.num_blocks();
-  const int lb = blockIdx.x / C, rank = cluster.block_rank();
-  const int p = pvec[lb], pe = (p + 1) & ~1, h = pe >> 1;
-  T* g = G + moff[lb];
-  T* vt = Vt + moff[lb];
-  const int lane = threadIdx.x & 31, nw = blockDim.x >> 5;
-  const int gw = rank * nw + (threadIdx.x >> 5), wtot = C * nw;
-  int* rf = rotflags + lb * HESTENES_MAXSW;
-  int sweep = 0;
-  for (; sweep < max_sweeps; ++sweep) {
-    for (int r = 0; r < pe - 1; ++r) {
-      for (int q = gw; q < h; q += wtot) {
-        int i, j; rr_pair(r, q, pe, i, j);
-        if (j >= p) continue;
-        T gi[NE], gj[NE];
-        double a = 0.0, b = 0.0, c = 0.0;
-#pragma unroll
-        for (int e = 0; e < NE; ++e) {
-          const int col = lane + 32 * e;
-          gi[e] = col < p ? __ldcg(g + (long long)i * p + col) : (T)0;
-          gj[e] = col < p ? __ldcg(g + (long long)j * p + col) : (T)0;
-          a += (double)gi[e] * (double)gi[e]; b += (double)gj[e] * (double)gj[e]; c += (double)gi[e] * (double)gj[e];
-        }
-        a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
-        if (fabs(c) > tol * sqrt(a * b) && a > 0.0 && b > 0.0) {
-          const double zeta = (b - a) / (2.0 * c);
-          const double t = (zeta >= 0.0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
-          const double cd = 1.0 / sqrt(1.0 + t * t);
-          const T sn = (T)(t * cd), tau = (T)(t * cd / (1.0 + cd));      // Rutishauser form, see psd_small.cuh
-#pragma unroll
-          for (int e = 0; e < NE; ++e) {
-            const int col = lane + 32 * e;
-            if (col < p) {
-              __stcg(g + (long long)i * p + col, gi[e] - sn * (gj[e] + tau * gi[e]));
-              __stcg(g + (long long)j * p + col, gj[e] + sn * (gi[e] - tau * gj[e]));
-              const T vi = __ldcg(vt + (long long)i * p + col), vj = __ldcg(vt + (long long)j * p + col);
-              __stcg(vt + (long long)i * p + col, vi - sn * (vj + tau * vi));
-              __stcg(vt + (long long)j * p + col, vj + sn * (vi - tau * vj));
-            }
-          }
-          if (lane == 0) rf[sweep] = 1;
-        }
-      }
-      cluster.sync();
-    }
-    const int rot = __ldcg(rf + sweep);
-    if (!rot) break;
-  }
-  if (sweep >= max_sweeps && flags && rank == 0 && threadIdx.x == 0) atomicOr(flags + prob_of[lb], FLAG_EIG_CAP);
-  // eigenvalues
-  for (int i = gw; i < p; i += wtot) {
-    double a = 0.0;
-    for (int col = lane; col < p; col += 32) { const double x = (double)__ldcg(g + (long long)i * p + col); a += x * x; }
-    a = warp_sum(a);
-    if (lane == 0) lam[voff[lb] + i] = (T)(sqrt(a) - (double)mu[lb]);
-  }
-  if (rank == 0 && threadIdx.x == 0) { atomicMax(sweeps_out, sweep); if (sweeps_sum) atomicAdd(sweeps_sum, (unsigned long long)sweep); }
-}
-
 // Batched row-major GEMM C = op(A) op(B) (p x p x p per block), FMA path. 64x64 tile, 16x16 threads, 4x4 each.
 // Optional row scaling of op(A): op(A)(i,k) *= rs[k] (used for U diag(lam+) U').
 template <typename T>
 __global__ void __launch_bounds__(256) k_gemm_fma(int nblk, const int* pvec, const long long* moff, const int* voff, const T* A, int ta,
-                                                  const T* Bm, int tb, T* Cm, const T* kscale, int kscale_relu) {
+                                                  const T* Bm, int tb, T* Cm, const T* kscale, int kscale_relu, const int* need) {
   __shared__ T As[16][64 + 1];
   __shared__ T Bs[16][64 + 1];
+  if (need && !need[blockIdx.z]) return;
   const int lb = blockIdx.z, p = pvec[lb];
   const int i0 = blockIdx.y * 64, j0 = blockIdx.x * 64;
   if (i0 >= p || j0 >= p) return;
@@ -266,7 +202,8 @@ __global__ void k_large_hadamard(int nblk, const int* pvec, const long long* mof
 // eigenvalues carry an error of eps ||S||, not eps mu, and do not see how the sweeps scaled the rows of G.
 template <typename T>
 __global__ void __launch_bounds__(256) k_large_rayleigh(const int* pvec, const long long* moff, const int* voff, const T* R,
-                                                        const T* Vt, T* lam) {
+                                                        const T* Vt, T* lam, const int* need) {
+  if (need && !need[blockIdx.y]) return;
   const int lb = blockIdx.y, p = pvec[lb];
   const int lane = threadIdx.x & 31, nw = blockDim.x >> 5;
   const T* r = R + moff[lb];
@@ -282,8 +219,10 @@ __global__ void __launch_bounds__(256) k_large_rayleigh(const int* pvec, const l
 // After an eigendecomposition: scale[k] = max(lam_k, 0) (the rebuild's column scaling) and lmax = max |lam_k|
 // (the spectral radius the next warm call's shift is derived from).
 template <typename T>
-__global__ void __launch_bounds__(256) k_large_post(const int* pvec, const int* voff, const T* lam, T* scale, T* lmax) {
+__global__ void __launch_bounds__(256) k_large_post(const int* pvec, const int* voff, const T* lam, T* scale, T* lmax, const T* mu,
+                                                    const int* need, int* need_out) {
   __shared__ double sh[32];
+  if (need && !need[blockIdx.x]) { if (need_out && threadIdx.x == 0) need_out[blockIdx.x] = 0; return; }
   const int lb = blockIdx.x, p = pvec[lb];
   const T* l = lam + voff[lb];
   double mx = 0.0;
@@ -299,6 +238,9 @@ __global__ void __launch_bounds__(256) k_large_post(const int* pvec, const int* 
   if (threadIdx.x == 0) {
     for (int w = 1; w < (int)(blockDim.x >> 5); ++w) mx = fmax(mx, sh[w]);
     lmax[lb] = (T)mx;
+    // the rounding errors of the one-sided Jacobi scale with its shift: a decomposition that ran on a shift well above the
+    // spectral radius (cold start: ||S||_F; early iterations: the Weyl bound with ||dS||_F) is polished by a second pass
+    if (need_out) need_out[lb] = (!need && (double)mu[lb] > 3.0 * mx) ? 1 : 0;
   }
 }
 

@@ -105,7 +105,9 @@ def compare(wl, ref, res, per_problem):
     if per_problem:
         e["g_rho"] = max(nrm_err(res["g_rho"][:, b], ref["g_rho"][j]) for j, b in enumerate(ref["idx"]))
         e["g_alpha"] = max(nrm_err(res["g_alpha"][:, b], ref["g_alpha"][j]) for j, b in enumerate(ref["idx"]))
-        e["g_sigma"] = max(nrm_err([res["g_sigma"][b]], [ref["g_sigma"][j]]) for j, b in enumerate(ref["idx"]))
+        # g_sigma has one entry per problem in this layout: compared norm-wise as that vector (reading A10), like
+        # every other output. One entry alone is a sum of K signed terms and can cancel to a fraction of their size.
+        e["g_sigma"] = nrm_err([res["g_sigma"][b] for b in ref["idx"]], ref["g_sigma"])
     else:
         assert len(ref["idx"]) == wl.batch
         e["g_rho"] = nrm_err(res["g_rho"], np.sum(ref["g_rho"], axis=0))

@@ -207,8 +207,8 @@ def test_large_block_path_downscaled(ckpt):
     assert st["flags_or"] == 0
 
 
-def test_order_above_512_hestenes_path():
-    """Orders above 512 leave the blocked kernel's shared-memory plan and run k_hestenes: p = 640 inside a K = 4 unroll,
+def test_order_above_512():
+    """Orders above 512 (more block pairs than CTAs per matrix in the fp32 kernel): p = 640 inside a K = 4 unroll,
     fp32 (FULL) and fp64 (LEAN)."""
     for dtype, ckpt in (("f32", 0), ("f64", 1)):
         wl = W.make_config(5, batch=1, p=640, K=4, dtype=dtype)

@@ -10,6 +10,7 @@ from .generators import (  # noqa: F401
     Workload,
     svec_index,
     svec_dim,
+    cone_rows,
     maxcut_problem,
     lovasz_problem,
     socp_problem,
