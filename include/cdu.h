@@ -82,6 +82,9 @@ typedef struct {
                                linear-step kernels; <= 0: chosen from the batch size and the problem size         */
   int32_t no_batch;         /* 1: single-CTA teams read rows with lane groups straight from global memory instead of
                                the precomputed warp batches (debug / comparison)                                  */
+  int32_t no_diag_path;     /* 1: run the PCG kernels even when M = P + sigma I + rho A'A is diagonal (every row of A
+                               holds <= 1 entry, P diagonal, no SOC cones), where by default the single PCG iteration
+                               is evaluated in closed form (debug / comparison)                                    */
 } cdu_options;
 
 /* Copies and re-packs the batch onto the current CUDA device (transposed copy of A, diag(P), column square

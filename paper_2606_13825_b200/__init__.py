@@ -52,7 +52,7 @@ class _Problem(C.Structure):
 class _Options(C.Structure):
     _fields_ = [("cg_tol", C.c_double), ("cg_max_iter", C.c_int32), ("K_max", C.c_int32), ("ckpt_mode", C.c_int32),
                 ("cg_refine", C.c_int32), ("cg_refine_tol", C.c_double), ("psd_small_max", C.c_int32),
-                ("use_tensor_cores", C.c_int32), ("team_size", C.c_int32), ("no_batch", C.c_int32)]
+                ("use_tensor_cores", C.c_int32), ("team_size", C.c_int32), ("no_batch", C.c_int32), ("no_diag_path", C.c_int32)]
 
 
 class _Stats(C.Structure):
@@ -131,7 +131,7 @@ class Handle:
 
     def __init__(self, packed: dict, K_max: int, ckpt_mode: int = CDU_CKPT_FULL, cg_tol: float = 0.0,
                  cg_max_iter: int = 0, cg_refine: int = -1, cg_refine_tol: float = 0.0, psd_small_max: int = 0,
-                 use_tensor_cores: int = -1, team_size: int = 0, no_batch: int = 0):
+                 use_tensor_cores: int = -1, team_size: int = 0, no_batch: int = 0, no_diag_path: int = 0):
         torch = _torch()
         if not torch.cuda.is_available():
             raise CduError(CDU_ECUDA, "no CUDA device (there is no CPU fallback)")
@@ -151,7 +151,7 @@ class Handle:
                       **{k: v.ctypes.data for k, v in keep.items()})
         op = _Options(cg_tol=cg_tol, cg_max_iter=cg_max_iter, K_max=K_max, ckpt_mode=ckpt_mode, cg_refine=cg_refine,
                       cg_refine_tol=cg_refine_tol, psd_small_max=psd_small_max, use_tensor_cores=use_tensor_cores,
-                      team_size=team_size, no_batch=no_batch)
+                      team_size=team_size, no_batch=no_batch, no_diag_path=no_diag_path)
         h = C.c_void_p()
         st = self.lib.cdu_create(C.byref(pr), C.byref(op), _stream(), C.byref(h))
         if st != CDU_OK:

@@ -16,6 +16,7 @@
 #include "cdu.h"
 #include "handle_base.h"
 #include "lin.cuh"
+#include "lin_diag.cuh"
 #include "psd_large.cuh"
 #include "psd_bjacobi.cuh"
 #include "psd_small.cuh"
@@ -468,6 +469,9 @@ struct HandleT : cdu_handle_s {
   DevPool pool;
   BatchDev<T, IT> D{};
   int team_C = 1, lin_grid = 1;      // CTAs per team (cluster size), persistent grid size
+  bool diag_on = false;              // M is diagonal: closed-form linear step (lin_diag.cuh)
+  DiagTab DG{};
+  T* d_aval = nullptr;
   size_t lin_smem = 0;               // dynamic shared memory of the linear-step kernels
   PsdEngine<T> psd;
   int B = 0, K_max = 0, ckpt_mode = 0, lin_threads = 256;
@@ -547,7 +551,7 @@ cdu_status HandleT<T, IT>::init(const cdu_problem* pr, const cdu_options* op, cu
   if ((nnzA && (!pr->A_colidx || !pr->A_val)) || (nnzP && (!pr->P_colidx || !pr->P_val))) { err = "cdu_create: NULL CSR arrays"; return CDU_EINVAL; }
   cdu_options o{};
   if (op) o = *op;
-  else { o.cg_refine = -1; o.use_tensor_cores = -1; o.team_size = 0; o.no_batch = 0; }
+  else { o.cg_refine = -1; o.use_tensor_cores = -1; o.team_size = 0; o.no_batch = 0; o.no_diag_path = 0; }
   if (o.K_max < 1) { err = "cdu_create: options.K_max must be >= 1"; return CDU_EINVAL; }
   const bool f32 = std::is_same<T, float>::value;
   K_max = o.K_max; ckpt_mode = o.ckpt_mode == CDU_CKPT_LEAN ? CDU_CKPT_LEAN : CDU_CKPT_FULL;
@@ -669,6 +673,37 @@ cdu_status HandleT<T, IT>::init(const cdu_problem* pr, const cdu_options* op, cu
   cg_f = pool.zeros<int>(B, st); cg_b = pool.zeros<int>(B, st); cg_f0 = pool.zeros<int>(B, st); cg_b0 = pool.zeros<int>(B, st); cg_max = pool.zeros<int>(B, st); flags = pool.zeros<int>(B, st);
   D.cg_iters = cg_f; D.cg_iters0 = cg_f0; D.cg_max = cg_max; D.flags = flags;
   if (pool.last != cudaSuccess) { err = std::string("cdu_create: ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
+
+  // ---- diagonal M (lin_diag.cuh): every row of A holds <= 1 entry, P only diagonal entries, no SOC cones -------------
+  {
+    bool ok = o.no_diag_path == 0 && soc_start.empty();
+    for (long long r = 0; ok && r < Mtot; ++r) if (A_rp[r + 1] - A_rp[r] > 1) ok = false;
+    for (long long j = 0; ok && j < N; ++j) if (AT_rp[j + 1] - AT_rp[j] > DIAG_MAXCOL) ok = false;
+    for (int b = 0; ok && b < B; ++b) {
+      const long long v0 = pr->var_off[b], n = pr->var_off[b + 1] - v0;
+      for (long long i = 0; ok && i < n; ++i)
+        for (long long e = P_rp[v0 + i]; e < P_rp[v0 + i + 1]; ++e) if (pr->P_colidx[e] != i && Pv[e] != (T)0) { ok = false; break; }
+    }
+    if (ok) {
+      std::vector<int> acol((size_t)Mtot, -1), choff(B + 1, 0);
+      std::vector<T> aval((size_t)Mtot, (T)0);
+      std::vector<int4> chunks;
+      for (long long r = 0; r < Mtot; ++r) if (A_rp[r + 1] > A_rp[r]) { acol[r] = pr->A_colidx[A_rp[r]]; aval[r] = Av[A_rp[r]]; }
+      for (int b = 0; b < B; ++b) {
+        const int items = (int)std::max(pr->var_off[b + 1] - pr->var_off[b], pr->row_off[b + 1] - pr->row_off[b]);
+        int idx = 0;
+        for (int lo = 0; lo < items; lo += DIAG_CHUNK) chunks.push_back(make_int4(b, lo, std::min(items, lo + DIAG_CHUNK), idx++));
+        choff[b + 1] = (int)chunks.size();
+      }
+      DG.nchunk = (int)chunks.size();
+      DG.chunk = pool.upload(chunks, st); DG.chunk_off = pool.upload(choff, st); DG.acol = pool.upload(acol, st);
+      d_aval = pool.upload(aval, st);
+      DG.part = pool.zeros<double>((size_t)DG.nchunk * 4, st); DG.ticket = pool.zeros<unsigned>(B, st);
+      if (pool.last != cudaSuccess) { err = std::string("cdu_create (diagonal path): ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
+      CU_OK(cudaStreamSynchronize(st));   // staging vectors go out of scope
+      diag_on = true;
+    }
+  }
 
   // ---- team shape (lin.cuh): cluster size, CTA size, shared-memory residency, persistent grid -----------------
   {
@@ -887,7 +922,9 @@ cdu_status HandleT<T, IT>::forward(int K, const void* rho, int mode, double sigm
     I.Zk = z_at(k); I.Zk1 = z_at(k + 1);
     I.XT = XT + (full ? (size_t)k * N : 0); I.ST = ST + (full ? (size_t)k * Mtot : 0);
     prof.begin(PC_LIN_FWD, st);
-    cudaError_t le = launch_lin(k_fwd<T, IT, false>, k_fwd<T, IT, true>, st, Df, H, I, k);
+    cudaError_t le;
+    if (diag_on) { k_dfwd<T, IT><<<DG.nchunk, DIAG_THREADS, 0, st>>>(Df, DG, d_aval, H, I, k); le = cudaGetLastError(); }
+    else le = launch_lin(k_fwd<T, IT, false>, k_fwd<T, IT, true>, st, Df, H, I, k);
     prof.end(st);
     ++launches;
     CU_OK(le);
@@ -930,7 +967,7 @@ cdu_status HandleT<T, IT>::backward(const void* gx, const void* gs, const void* 
     Q.g_rho_pb = g_rho_pb; Q.g_alpha_pb = g_alpha_pb; Q.g_sigma_pb = g_sigma_pb; Q.part_pre = part_pre;
     Q.recompute = full ? 0 : 1;
     Q.warm_adjoint = k < K - 1 ? 1 : 0;
-    if (!has_psd) {
+    if (!has_psd && !diag_on) {
       prof.begin(PC_LIN_BWD, st);
       cudaError_t le = launch_lin(k_bwd<T, IT, false>, k_bwd<T, IT, true>, st, Db, H, Q, k, 0);
       prof.end(st);
@@ -938,10 +975,13 @@ cdu_status HandleT<T, IT>::backward(const void* gx, const void* gs, const void* 
       CU_OK(le);
     } else {
       prof.begin(PC_LIN_BWD, st);
-      cudaError_t le = launch_lin(k_bwd<T, IT, false>, k_bwd<T, IT, true>, st, Db, H, Q, k, 1);
+      cudaError_t le;
+      if (diag_on) { k_dbwd_pre<T, IT><<<DG.nchunk, DIAG_THREADS, 0, st>>>(Db, DG, d_aval, H, Q, k); le = cudaGetLastError(); }
+      else le = launch_lin(k_bwd<T, IT, false>, k_bwd<T, IT, true>, st, Db, H, Q, k, 1);
       prof.end(st);
       ++launches;
       CU_OK(le);
+      if (has_psd) {
       PsdBwdArgs A;
       A.W = D.W; A.Yk = z_at(k) + N + Mtot; A.S1 = z_at(k + 1) + N;
       A.Gs = Q.Gin + N; A.Gy = Q.Gin + N + Mtot; A.GW = D.GW; A.part = D.psd_part;
@@ -949,8 +989,10 @@ cdu_status HandleT<T, IT>::backward(const void* gx, const void* gs, const void* 
       A.recompute = full ? 0 : 1; A.flags = flags;
       s = psd.backward(H, k, A, st);
       if (s != CDU_OK) { err = psd.err; return s; }
+      }
       prof.begin(PC_LIN_BWD, st);
-      le = launch_lin(k_bwd<T, IT, false>, k_bwd<T, IT, true>, st, Db, H, Q, k, 2);
+      if (diag_on) { k_dbwd_post<T, IT><<<DG.nchunk, DIAG_THREADS, 0, st>>>(Db, DG, d_aval, H, Q, k); le = cudaGetLastError(); }
+      else le = launch_lin(k_bwd<T, IT, false>, k_bwd<T, IT, true>, st, Db, H, Q, k, 2);
       prof.end(st);
       ++launches;
       CU_OK(le);

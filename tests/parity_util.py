@@ -116,6 +116,16 @@ def compare(wl, ref, res, per_problem):
     return e
 
 
+def compare_each(wl, ref, res, per_problem=True):
+    """compare() problem by problem: list of error dicts in the order of ref['idx']."""
+    out = []
+    for j, b in enumerate(ref["idx"]):
+        one = {k: ([v[j]] if isinstance(v, list) else v) for k, v in ref.items()}
+        one["idx"] = [b]
+        out.append(compare(wl, one, res, per_problem))
+    return out
+
+
 def full_cotangent(wl, ref, fill_seed=None):
     """Cotangent list for the whole batch: the oracle's for compared problems; elsewhere zeros, or (fill_seed given)
     seeded N(0,1) scaled to the compared problems' cotangents, so that the backward of EVERY problem does real work."""
