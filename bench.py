@@ -408,13 +408,77 @@ def run_config(cfg, args, cdu, torch, dist, peaks, world, rank, local, ckpt, opt
     return res
 
 
+def run_fig2(args, cdu, torch, peaks):
+    """the linear-solve scaling experiment of PAPER.md Fig. 2 / App. B (L96, L247-255): one step
+    x-tilde = M^-1 xi (matrix-free PCG) and its matrix-free backward (adjoint PCG, Eq. 5-6), loss 1/2 ||x-tilde - x*||^2, for
+    n in {1k .. 50k}, m = n/2, diag P ~ U(0,10), A 1 % dense. Reports time, CG iterations, handle-owned device bytes (the
+    paper: < 300 MB at n = 50k on an RTX 4090 in fp64) and the algorithmic CSR stream rate of the two linear-step kernels."""
+    ns = [args.n] if args.n else [1000, 2000, 5000, 10000, 20000, 50000]
+    dtype = args.dtype or "f64"
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    points = []
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+    for n in ns:
+        wl = W.make_fig2(n, batch=args.batch or 1, dtype=dtype)
+        packed = W.pack_batch(wl.problems, wl.dtype)
+        h = cdu.cdu_create(packed, K_max=1, team_size=args.team_size, cg_refine=0 if args.cg_refine == -2 else args.cg_refine)
+        N, M = h.N, h.M
+        rng = np.random.default_rng(W.generators.BASE_SEED + 6001)
+        T = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=tdt, device="cuda")
+        rho, alpha = T(wl.rho), T(wl.alpha)
+        x0, s0, y0 = T(np.concatenate(wl.x0)), T(np.concatenate(wl.s0)), T(np.concatenate(wl.y0))
+        xstar = T(rng.standard_normal(N))
+        zero_m = torch.zeros(M, dtype=tdt, device="cuda")
+
+        def step():
+            x1, _, _ = h.forward(1, rho, alpha, wl.sigma, x0, s0, y0)
+            return h.backward(x1 - xstar, zero_m, zero_m)          # cotangent of 1/2 ||x-tilde - x*||^2
+
+        for _ in range(max(args.warmup, 3)):
+            step()
+        torch.cuda.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for i in range(args.steps):
+            flush.fill_(i)
+            ev[i][0].record(); step(); ev[i][1].record()
+        torch.cuda.synchronize()
+        ms = sorted(a.elapsed_time(b) for a, b in ev)[len(ev) // 2]
+        h.profile(True)
+        flush.fill_(0); step(); torch.cuda.synchronize()
+        prof = h.get_profile()
+        h.profile(False)
+        st = h.stats()
+        nf, nb = st["cg_iters_fwd"] / wl.batch, st["cg_iters_bwd"] / wl.batch
+        fb, bb = lin_bytes(wl, nf, nb, True)
+        pt = dict(n=n, m=n // 2, nnz_A=int(sum(pr.A.nnz for pr in wl.problems) / wl.batch), batch=wl.batch, ms_fwd_bwd=ms,
+                  cg_iters_fwd=nf, cg_iters_bwd=nb, device_mb=st["device_bytes"] / 2 ** 20, flags=st["flags_or"],
+                  lin_fwd_ms=prof.get("lin_fwd", {}).get("ms"), lin_bwd_ms=prof.get("lin_bwd", {}).get("ms"))
+        # executed stream: this build reads A and A' separately (a = 2 passes per operator application)
+        w = 4 if dtype == "f32" else 8
+        SA = sum(csr_stream_bytes(pr.A, w) for pr in wl.problems)
+        exe_f = SA * (2 + 2 * (nf + 1)); exe_b = SA * (3 + 2 * nb)
+        if pt["lin_fwd_ms"]:
+            pt["lin_fwd_model_gbs"] = fb / pt["lin_fwd_ms"] / 1e6; pt["lin_fwd_executed_gbs"] = exe_f / pt["lin_fwd_ms"] / 1e6
+        if pt["lin_bwd_ms"]:
+            pt["lin_bwd_model_gbs"] = bb / pt["lin_bwd_ms"] / 1e6; pt["lin_bwd_executed_gbs"] = exe_b / pt["lin_bwd_ms"] / 1e6
+        points.append(pt)
+        h.close()
+        torch.cuda.empty_cache()
+    print(json.dumps(dict(metric="fig2_linear_solve_fwd_bwd_ms", unit="ms", dtype=dtype, data="synthetic", higher_is_better=False,
+                          config=dict(workload="fig2-linsolve (PAPER.md App. B)", l2="flushed between timed steps", rho="scalar per instance (per-row rho: SURVEY 8(f) F3)"),
+                          hbm_peak_gbs=peaks.get("hbm_gbs"), paper_context="< 300 MB peak memory at n = 50k, RTX 4090, fp64, PyTorch (L96, L255)",
+                          points=points)))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="all", choices=["all"] + sorted(WORKLOADS))
+    ap.add_argument("--workload", default="all", choices=["all", "fig2"] + sorted(WORKLOADS))
+    ap.add_argument("--n", type=int, default=0, help="fig2: one problem size instead of the sweep 1k .. 50k")
+    ap.add_argument("--dtype", default=None, help="fig2: f64 (default, the paper's precision) or f32")
     ap.add_argument("--ckpt", default="full", choices=["full", "lean"])
     ap.add_argument("--batch", type=int, default=None, help="override the batch size (debug)")
     ap.add_argument("--unroll", type=int, default=None, help="override K_unroll (debug)")
@@ -428,7 +492,7 @@ def main():
     ap.add_argument("--no-batch", type=int, default=0, help="1: lane groups per row instead of warp row batches (debug)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    cfgs = [5, 3, 2] if args.workload == "all" else [WORKLOADS[args.workload]]
+    cfgs = [5, 3, 2] if args.workload in ("all", "fig2") else [WORKLOADS[args.workload]]
 
     def opts_of(cfg):
         o = dict(cg_refine=args.cg_refine, cg_refine_tol=args.cg_refine_tol)
@@ -452,6 +516,10 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     peaks = load_peaks(cdu)
+    if args.workload == "fig2":
+        if rank == 0:
+            run_fig2(args, cdu, torch, peaks)
+        return
     results = [run_config(c, args, cdu, torch, dist, peaks, world, rank, local, args.ckpt, opts_of(c)) for c in cfgs]
     if rank == 0:
         r = results[0]

@@ -34,9 +34,21 @@ constexpr int STAGES = 3;
 constexpr int TILE_BYTES = TILE * BK * 4;                    // 16 KB
 constexpr int STAGE_BYTES = 4 * TILE_BYTES;                  // A, A_lo, B, B_lo
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
-constexpr int THREADS = 320;
+constexpr int SPLIT_WARPS = 4;
+constexpr int DRAIN_WARPS = 8;          // (TMEM lane quarter, column half) each
+constexpr int THREADS = 32 * (2 + SPLIT_WARPS + DRAIN_WARPS);
 constexpr int TMEM_COLS = 512;        // H0, H1 (leading term, double buffered), L (small terms); power of two
 
+#ifdef CDU_GEMM_TIMING
+__device__ long long g_gemm_tim[128 * 16];
+#define GT_DECL() long long gt_a_ = 0, gt_b_ = 0, gt_c_ = 0, gt_t_ = clock64(), gt_0_ = gt_t_
+#define GT_MARK(x) do { const long long n_ = clock64(); x += n_ - gt_t_; gt_t_ = n_; } while (0)
+#define GT_OUT(base) do { const long long n_ = clock64(); g_gemm_tim[(blockIdx.x + gridDim.x * blockIdx.y) * 16 + (base)] = gt_a_; g_gemm_tim[(blockIdx.x + gridDim.x * blockIdx.y) * 16 + (base) + 1] = gt_b_; g_gemm_tim[(blockIdx.x + gridDim.x * blockIdx.y) * 16 + (base) + 2] = gt_c_; g_gemm_tim[(blockIdx.x + gridDim.x * blockIdx.y) * 16 + (base) + 3] = n_ - gt_0_; } while (0)
+#else
+#define GT_DECL() do {} while (0)
+#define GT_MARK(x) do {} while (0)
+#define GT_OUT(base) do {} while (0)
+#endif
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
@@ -103,6 +115,11 @@ __device__ __forceinline__ void split_tf32(float a, float& hi, float& lo) {
   asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(l) : "f"(a - hi));
   lo = __uint_as_float(l);
 }
+// lo part of the 3xTF32 split against the tensor core's own truncation of the hi operand
+__device__ __forceinline__ float lo_tf32(float a) {
+  const float r = a - __uint_as_float(__float_as_uint(a) & 0xffffe000u);
+  return __uint_as_float((__float_as_uint(r) + 0x1000u) & 0xffffe000u);
+}
 __device__ __forceinline__ float gamma_relu_f(float li, float lj) {   // same rule as psd_small.cuh (reading A11)
   const bool pi = li > 0.f, pj = lj > 0.f;
   if (pi && pj) return 1.f;
@@ -133,11 +150,18 @@ k_gemm_tc(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUte
   const int nk = p / BK;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < STAGES; ++s) { mbar_init(full(s), 1); mbar_init(split(s), 128); mbar_init(empty(s), 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(tfull(i), 1); mbar_init(tempty(i), 128); }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full(s), 1); mbar_init(split(s), 32 * SPLIT_WARPS); mbar_init(empty(s), 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(tfull(i), 1); mbar_init(tempty(i), 32 * DRAIN_WARPS); }
     mbar_init(lfull, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    // the first ring of operand tiles is requested before the TMEM allocation and the block-wide barrier below
+    for (int kb = 0; kb < STAGES && kb < p / BK; ++kb) {
+      mbar_expect_tx(full(kb), 2 * TILE_BYTES);
+      const uint32_t st = base + kb * STAGE_BYTES;
+      tma_load_3d(st, &mapA, full(kb), kb * BK, (int)(blockIdx.x / (p / TILE)) * TILE, blockIdx.y);
+      tma_load_3d(st + 2 * TILE_BYTES, &mapB, full(kb), kb * BK, (int)(blockIdx.x % (p / TILE)) * TILE, blockIdx.y);
+    }
   }
   if (warp == 1) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32((const void*)tmem_slot)), "n"(TMEM_COLS) : "memory");
@@ -150,23 +174,31 @@ k_gemm_tc(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUte
 
   if (warp == 0) {
     if (lane == 0) {
-      for (int kb = 0; kb < nk; ++kb) {
+      GT_DECL();
+      for (int kb = STAGES; kb < nk; ++kb) {
         const int s = kb % STAGES; const uint32_t ph = (uint32_t)(kb / STAGES) & 1u;
+        GT_MARK(gt_b_);
         mbar_wait(empty(s), ph ^ 1u);
+        GT_MARK(gt_a_);
         mbar_expect_tx(full(s), 2 * TILE_BYTES);
         const uint32_t st = base + s * STAGE_BYTES;
         tma_load_3d(st, &mapA, full(s), kb * BK, tm * TILE, lb);
         tma_load_3d(st + 2 * TILE_BYTES, &mapB, full(s), kb * BK, tn * TILE, lb);
       }
+      GT_OUT(0);
     }
   } else if (warp == 1) {
     if (lane == 0) {
       constexpr uint32_t idesc = umma_idesc_tf32();
+      GT_DECL();
       for (int kb = 0; kb < nk; ++kb) {
         const int s = kb % STAGES; const uint32_t ph = (uint32_t)(kb / STAGES) & 1u;
         const int slot = kb & 1;
+        GT_MARK(gt_c_);
         mbar_wait(tempty(slot), ((uint32_t)(kb >> 1) & 1u) ^ 1u);     // the drain warps have emptied H[slot]
+        GT_MARK(gt_a_);
         mbar_wait(split(s), ph);
+        GT_MARK(gt_b_);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const uint32_t st = base + s * STAGE_BYTES;
         const uint32_t dH = tmem + (uint32_t)slot * TILE, dL = tmem + 2u * TILE;
@@ -182,74 +214,99 @@ k_gemm_tc(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUte
         umma_commit(tfull(slot));
       }
       umma_commit(lfull);
+      GT_OUT(4);
     }
-  } else if (warp < 6) {
-    const int t = threadIdx.x - 64;   // 0..127
+  } else if (warp < 2 + SPLIT_WARPS) {
+    // split warps: the hi operand is the raw fp32 tile - the tensor core drops the low 13 mantissa bits of a kind::tf32
+    // input, i.e. it multiplies trunc(a) - and lo = a - trunc(a), rounded to nearest TF32, makes up for exactly that
+    // truncation (|error| <= 2^-21 |a|, unbiased). Only the lo tiles are written: 1 shared-memory write per element read.
+    const int t = threadIdx.x - 64;   // 0 .. 32 SPLIT_WARPS - 1
+    constexpr int NT = 32 * SPLIT_WARPS;
+    GT_DECL();
     for (int kb = 0; kb < nk; ++kb) {
       const int s = kb % STAGES; const uint32_t ph = (uint32_t)(kb / STAGES) & 1u;
+      GT_MARK(gt_b_);
       mbar_wait(full(s), ph);
+      GT_MARK(gt_a_);
       float4* st = reinterpret_cast<float4*>(gbase + s * STAGE_BYTES);
 #pragma unroll
       for (int half = 0; half < 2; ++half) {
-        float4* hi = st + half * (2 * TILE_BYTES / 16);
+        const float4* hi = st + half * (2 * TILE_BYTES / 16);
         float4* lo = st + half * (2 * TILE_BYTES / 16) + TILE_BYTES / 16;
 #pragma unroll
-        for (int i = 0; i < TILE_BYTES / 16 / 128; ++i) {
-          const float4 v = hi[t + 128 * i];
-          float4 h, l;
-          split_tf32(v.x, h.x, l.x); split_tf32(v.y, h.y, l.y); split_tf32(v.z, h.z, l.z); split_tf32(v.w, h.w, l.w);
-          hi[t + 128 * i] = h;
-          lo[t + 128 * i] = l;
+        for (int i = 0; i < TILE_BYTES / 16 / NT; ++i) {
+          const float4 v = hi[t + NT * i];
+          float4 l;
+          l.x = lo_tf32(v.x); l.y = lo_tf32(v.y); l.z = lo_tf32(v.z); l.w = lo_tf32(v.w);
+          lo[t + NT * i] = l;
         }
       }
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       mbar_arrive(split(s));
     }
+    if (t == 0) GT_OUT(8);
   } else {
     // drain warps: the tensor core adds into its accumulator with truncation, which over K/8 additions biases the
     // result by ~1e-5 relative - too much for BPTT through hundreds of steps. So the leading term is accumulated in
     // TMEM over one 32-wide K chunk only (4 additions) and the chunks are summed here, in registers, round-to-nearest.
     // TMEM lane = tile row; a warp may only touch lanes 32 (warp % 4) .. +31.
-    const int q = warp & 3, row = q * 32 + lane;
+    const int q = warp & 3, row = q * 32 + lane, half = (warp - (2 + SPLIT_WARPS)) >> 2;
+    constexpr int HC = TILE / 2;       // columns per drain warp
     const uint32_t lane_off = (uint32_t)(q * 32) << 16;
-    float acc[TILE];
+    float acc[HC];
 #pragma unroll
-    for (int j = 0; j < TILE; ++j) acc[j] = 0.f;
+    for (int j = 0; j < HC; ++j) acc[j] = 0.f;
+    GT_DECL();
     for (int kb = 0; kb < nk; ++kb) {
       const int slot = kb & 1;
+      GT_MARK(gt_b_);
       mbar_wait(tfull(slot), (uint32_t)(kb >> 1) & 1u);
+      GT_MARK(gt_a_);
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll
-      for (int c = 0; c < TILE / 32; ++c) {
+      for (int c = 0; c < HC / 32; ++c) {
         uint32_t r[32];
-        tmem_ld32(tmem + lane_off + (uint32_t)(slot * TILE + c * 32), r);
+        tmem_ld32(tmem + lane_off + (uint32_t)(slot * TILE + half * HC + c * 32), r);
 #pragma unroll
         for (int j = 0; j < 32; ++j) acc[c * 32 + j] += __uint_as_float(r[j]);
       }
       asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
       mbar_arrive(tempty(slot));
     }
+    GT_MARK(gt_b_);
     mbar_wait(lfull, 0);
+    GT_MARK(gt_a_);
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const int gi = tm * TILE + row;
-    float* crow = C + (size_t)lb * p * p + (size_t)gi * p + tn * TILE;
     const float* l = lam ? lam + (size_t)lb * p : nullptr;
     const float li = l ? l[gi] : 0.f;
+    // every MMA has completed (lfull): the operand ring is free and stages the tile, so that the global stores are whole
+    // 256-byte row segments per half warp instead of one 16-byte piece per lane and row
+    constexpr int LDS_ = TILE + 4;
+    float* stg = reinterpret_cast<float*>(gbase);
 #pragma unroll
-    for (int c = 0; c < TILE / 32; ++c) {
+    for (int c = 0; c < HC / 32; ++c) {
       uint32_t r[32];
-      tmem_ld32(tmem + lane_off + (uint32_t)(2 * TILE + c * 32), r);
+      tmem_ld32(tmem + lane_off + (uint32_t)(2 * TILE + half * HC + c * 32), r);
 #pragma unroll
       for (int j = 0; j < 32; j += 4) {
         float4 o = make_float4(acc[c * 32 + j] + __uint_as_float(r[j]), acc[c * 32 + j + 1] + __uint_as_float(r[j + 1]),
                                acc[c * 32 + j + 2] + __uint_as_float(r[j + 2]), acc[c * 32 + j + 3] + __uint_as_float(r[j + 3]));
         if (l) {
-          const float4 lj = *reinterpret_cast<const float4*>(l + tn * TILE + c * 32 + j);
+          const float4 lj = *reinterpret_cast<const float4*>(l + tn * TILE + half * HC + c * 32 + j);
           o.x *= gamma_relu_f(li, lj.x); o.y *= gamma_relu_f(li, lj.y); o.z *= gamma_relu_f(li, lj.z); o.w *= gamma_relu_f(li, lj.w);
         }
-        *reinterpret_cast<float4*>(crow + c * 32 + j) = o;
+        *reinterpret_cast<float4*>(stg + row * LDS_ + half * HC + c * 32 + j) = o;
       }
     }
+    __syncwarp();      // a warp stages and stores the same 32 rows x 64 columns
+    float* cbase = C + (size_t)lb * p * p + (size_t)(tm * TILE + q * 32) * p + tn * TILE + half * HC;
+    const int r2 = lane >> 4, c4 = 4 * (lane & 15);
+#pragma unroll 4
+    for (int rr = 0; rr < 32; rr += 2)
+      *reinterpret_cast<float4*>(cbase + (size_t)(rr + r2) * p + c4) = *reinterpret_cast<const float4*>(stg + (q * 32 + rr + r2) * LDS_ + half * HC + c4);
+    GT_MARK(gt_c_);
+    if (row == 0 && half == 0) GT_OUT(12);
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();

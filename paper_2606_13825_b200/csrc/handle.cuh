@@ -498,9 +498,16 @@ struct HandleT : cdu_handle_s {
 
   double* z_at(int k) { return Z + (size_t)k * zstride; }
 
-  // One launch of a linear-step kernel over the whole batch: persistent CTAs (team_C == 1) or clusters of team_C CTAs.
+  // One launch of a linear-step kernel over the whole batch: persistent CTAs (team_C == 1), clusters of team_C CTAs, or
+  // wide teams (cooperative launch; their arrival counters are zeroed first).
   template <typename... Args>
-  cudaError_t launch_lin(void (*single)(Args...), void (*multi)(Args...), cudaStream_t st, Args... args) {
+  cudaError_t launch_lin(void (*single)(Args...), void (*multi)(Args...), void (*widek)(Args...), cudaStream_t st, Args... args) {
+    if (wide_on) {
+      cudaError_t e = cudaMemsetAsync(D.wide.bar, 0, sizeof(unsigned) * (size_t)(lin_grid / team_C), st);
+      if (e != cudaSuccess) return e;
+      void* ptrs[] = {(void*)&args...};
+      return cudaLaunchCooperativeKernel((const void*)widek, dim3(lin_grid), dim3(lin_threads), ptrs, lin_smem, st);
+    }
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(lin_grid); cfg.blockDim = dim3(lin_threads); cfg.dynamicSmemBytes = lin_smem; cfg.stream = st;
     cudaLaunchAttribute at[1];
@@ -511,6 +518,7 @@ struct HandleT : cdu_handle_s {
     }
     return cudaLaunchKernelEx(&cfg, single, args...);
   }
+  bool wide_on = false;
 
   cdu_status init(const cdu_problem* pr, const cdu_options* op, cudaStream_t st);
   Hyper<T> hyper() const {
@@ -714,6 +722,11 @@ cdu_status HandleT<T, IT>::init(const cdu_problem* pr, const cdu_options* op, cu
     const long long big = std::max(nmax, mmax);
     int C = 1;
     while (C < 16 && (long long)B * C * 2 <= nsm && big / (C * 2) >= 2048) C *= 2;
+    // few problems whose matrices would leave a 16-CTA cluster with > 100k entries per CTA: wide teams over the whole GPU
+    int wideC = 0;
+    if (o.team_size > 16) wideC = o.team_size;
+    else if (o.team_size <= 0 && (long long)B * 32 <= nsm && nnz_max >= 100000)
+      wideC = (int)std::min<long long>(nsm / B, std::max<long long>(17, nnz_max / 4096));
     if (o.team_size > 0) { C = 1; while (C * 2 <= std::min(o.team_size, 16)) C *= 2; }
     else if (C > 1 && (long long)B * 4 >= nsm &&
              (5 * (((size_t)nmax + 3) & ~(size_t)3) + (((size_t)mmax + 3) & ~(size_t)3)) * sizeof(T) <= (size_t)smem_optin - 2048)
@@ -793,15 +806,30 @@ cdu_status HandleT<T, IT>::init(const cdu_problem* pr, const cdu_options* op, cu
         CU_OK(cudaStreamSynchronize(st));   // the staging vectors go out of scope
       }
     }
-    const void* fns[4] = {(const void*)k_fwd<T, IT, false>, (const void*)k_bwd<T, IT, false>, (const void*)k_fwd<T, IT, true>,
-                          (const void*)k_bwd<T, IT, true>};
-    for (int i = 0; i < 4; ++i) {
+    if (wideC > 1 && !D.batched) {
+      D.vec_smem = 0; D.P_smem = 0; lin_smem = 0;     // wide teams keep their vectors in global memory (L2)
+      int occ = 0;
+      CU_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bwd<T, IT, 2>, lin_threads, lin_smem));
+      const int resident = nsm * std::max(occ, 0);
+      wideC = std::min(wideC, resident / B);
+      if (wideC > 16) {
+        wide_on = true; team_C = C = wideC; lin_grid = B * wideC;
+        D.wide.C = wideC;
+        D.wide.bar = pool.zeros<unsigned>(B, st);
+        D.wide.slots = pool.zeros<double>((size_t)B * 2 * wideC * 4, st);
+        if (pool.last != cudaSuccess) { err = "cudaMalloc (wide teams)"; return CDU_ENOMEM; }
+      }
+    }
+    const void* fns[4] = {(const void*)k_fwd<T, IT, 0>, (const void*)k_bwd<T, IT, 0>, (const void*)k_fwd<T, IT, 1>,
+                          (const void*)k_bwd<T, IT, 1>};
+    for (int i = 0; i < 4 && !wide_on; ++i) {
       CU_OK(cudaFuncSetAttribute(fns[i], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(lin_smem, 1024)));
       if (i >= 2 && C > 8) CU_OK(cudaFuncSetAttribute(fns[i], cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     }
-    if (C == 1) {
+    if (wide_on) {
+    } else if (C == 1) {
       int occ = 1;
-      CU_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bwd<T, IT, false>, lin_threads, lin_smem));
+      CU_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bwd<T, IT, 0>, lin_threads, lin_smem));
       occ = std::max(occ, 1);
       // keep the matrices of the problems in flight inside L2 (126 MB): they are re-read every CG iteration
       const double ws = ((double)nnzA * 2.0 * (sizeof(T) + sizeof(IT)) + (D.P_smem ? 0.0 : (double)nnzP * (sizeof(T) + (p_dense ? 0 : sizeof(IT))))) / B;
@@ -814,7 +842,7 @@ cdu_status HandleT<T, IT>::init(const cdu_problem* pr, const cdu_options* op, cu
       at[0].id = cudaLaunchAttributeClusterDimension; at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
       cfg.attrs = at; cfg.numAttrs = 1;
       int ncl = 0;
-      cudaError_t e = cudaOccupancyMaxActiveClusters(&ncl, k_bwd<T, IT, true>, &cfg);
+      cudaError_t e = cudaOccupancyMaxActiveClusters(&ncl, k_bwd<T, IT, 1>, &cfg);
       if (e != cudaSuccess || ncl < 1) { (void)cudaGetLastError(); err = "cdu_create: cluster launch not possible for the linear-step kernels"; return CDU_ECUDA; }
       lin_grid = std::min(B, ncl) * C;
     }
@@ -924,7 +952,7 @@ cdu_status HandleT<T, IT>::forward(int K, const void* rho, int mode, double sigm
     prof.begin(PC_LIN_FWD, st);
     cudaError_t le;
     if (diag_on) { k_dfwd<T, IT><<<DG.nchunk, DIAG_THREADS, 0, st>>>(Df, DG, d_aval, H, I, k); le = cudaGetLastError(); }
-    else le = launch_lin(k_fwd<T, IT, false>, k_fwd<T, IT, true>, st, Df, H, I, k);
+    else le = launch_lin(k_fwd<T, IT, 0>, k_fwd<T, IT, 1>, k_fwd<T, IT, 2>, st, Df, H, I, k);
     prof.end(st);
     ++launches;
     CU_OK(le);
@@ -969,7 +997,7 @@ cdu_status HandleT<T, IT>::backward(const void* gx, const void* gs, const void* 
     Q.warm_adjoint = k < K - 1 ? 1 : 0;
     if (!has_psd && !diag_on) {
       prof.begin(PC_LIN_BWD, st);
-      cudaError_t le = launch_lin(k_bwd<T, IT, false>, k_bwd<T, IT, true>, st, Db, H, Q, k, 0);
+      cudaError_t le = launch_lin(k_bwd<T, IT, 0>, k_bwd<T, IT, 1>, k_bwd<T, IT, 2>, st, Db, H, Q, k, 0);
       prof.end(st);
       ++launches;
       CU_OK(le);
@@ -977,7 +1005,7 @@ cdu_status HandleT<T, IT>::backward(const void* gx, const void* gs, const void* 
       prof.begin(PC_LIN_BWD, st);
       cudaError_t le;
       if (diag_on) { k_dbwd_pre<T, IT><<<DG.nchunk, DIAG_THREADS, 0, st>>>(Db, DG, d_aval, H, Q, k); le = cudaGetLastError(); }
-      else le = launch_lin(k_bwd<T, IT, false>, k_bwd<T, IT, true>, st, Db, H, Q, k, 1);
+      else le = launch_lin(k_bwd<T, IT, 0>, k_bwd<T, IT, 1>, k_bwd<T, IT, 2>, st, Db, H, Q, k, 1);
       prof.end(st);
       ++launches;
       CU_OK(le);
@@ -992,7 +1020,7 @@ cdu_status HandleT<T, IT>::backward(const void* gx, const void* gs, const void* 
       }
       prof.begin(PC_LIN_BWD, st);
       if (diag_on) { k_dbwd_post<T, IT><<<DG.nchunk, DIAG_THREADS, 0, st>>>(Db, DG, d_aval, H, Q, k); le = cudaGetLastError(); }
-      else le = launch_lin(k_bwd<T, IT, false>, k_bwd<T, IT, true>, st, Db, H, Q, k, 2);
+      else le = launch_lin(k_bwd<T, IT, 0>, k_bwd<T, IT, 1>, k_bwd<T, IT, 2>, st, Db, H, Q, k, 2);
       prof.end(st);
       ++launches;
       CU_OK(le);

@@ -36,6 +36,13 @@ struct Sell {
   const int4* mrow;      // (row, first slot, number of slots, -)
 };
 
+// wide teams (Team<2> below): CTAs of a cooperative launch that meet at a global counter
+struct WideTab {
+  int C;                 // CTAs per wide team
+  unsigned* bar;         // [teams] arrival counters, zeroed by the host before every launch
+  double* slots;         // [teams][2][C][4]
+};
+
 template <typename T, typename IT>
 struct BatchDev {
   int B;
@@ -59,6 +66,7 @@ struct BatchDev {
   int *cg_iters, *cg_iters0, *cg_max, *flags;          // [B] statistics (cg_iters0: iterations of pass 0 only, i.e. without refinement)
   double* psd_part;                                    // [nblk][2] partial dots written by the PSD backward
   long long N, Mtot;
+  WideTab wide;                                        // wide teams (MULTI == 2)
 };
 
 template <typename T>
@@ -68,20 +76,40 @@ struct Hyper {  // per-iteration hyper-parameters as the caller laid them out (c
   __device__ double alpha_at(int k, int b) const { return (double)alpha[(size_t)k * kstride + (size_t)b * pstride]; }
 };
 
-// ---- team = CTA or cluster ---------------------------------------------------------------------------------
-template <bool MULTI>
+// ---- team = CTA (MULTI 0), thread-block cluster (1) or "wide" team (2) ---------------------------------------
+// A wide team is any number of co-resident CTAs (cooperative launch) that meet at a counter in global memory and
+// exchange partial sums through global memory: for the few-large-problems regime (Fig. 2 workload, L247-255), where a
+// 16-CTA cluster would leave most of the GPU idle and the matrices do not fit L2.
+template <int MULTI>
 struct Team {
   int C, rank, parity;
   double* sh;       // [3*32] block_sum scratch
   double* slots;    // [2][4] partials exchanged through DSMEM
   double* bc;       // [4] broadcast
-  __device__ void init(double* sh_, double* slots_, double* bc_) {
-    sh = sh_; slots = slots_; bc = bc_; parity = 0;
-    if (MULTI) { cg::cluster_group cl = cg::this_cluster(); C = (int)cl.num_blocks(); rank = (int)cl.block_rank(); }
-    else { C = 1; rank = 0; }
+  unsigned* wbar; unsigned wgen; double* wslots;     // wide teams
+  __device__ void init(double* sh_, double* slots_, double* bc_, const WideTab& W) {
+    sh = sh_; slots = slots_; bc = bc_; parity = 0; wbar = nullptr; wgen = 0; wslots = nullptr;
+    if (MULTI == 1) { cg::cluster_group cl = cg::this_cluster(); C = (int)cl.num_blocks(); rank = (int)cl.block_rank(); }
+    else if (MULTI == 2) {
+      C = W.C; rank = (int)blockIdx.x % C;
+      const int team = (int)blockIdx.x / C;
+      wbar = W.bar + team; wslots = W.slots + (size_t)team * 2 * C * 4;
+    } else { C = 1; rank = 0; }
   }
-  __device__ __forceinline__ void sync() const {
-    if (MULTI) cg::this_cluster().sync(); else __syncthreads();
+  __device__ __forceinline__ void sync() {
+    if (MULTI == 1) cg::this_cluster().sync();
+    else if (MULTI == 2) {
+      __syncthreads();
+      if (threadIdx.x == 0) {
+        ++wgen;
+        __threadfence();
+        atomicAdd(wbar, 1u);
+        const unsigned target = wgen * (unsigned)C;
+        unsigned v;
+        do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(wbar) : "memory"); } while (v < target);
+      }
+      __syncthreads();
+    } else __syncthreads();
   }
   __device__ __forceinline__ void range(int len, int& lo, int& hi) const {
     if (MULTI) { lo = (int)((long long)len * rank / C); hi = (int)((long long)len * (rank + 1) / C); }
@@ -90,7 +118,7 @@ struct Team {
   // Deterministic team-wide sum; every thread of every CTA returns the same bits.
   template <int NV> __device__ void sum(double (&v)[NV]) {
     block_sum<NV>(v, sh);
-    if (MULTI) {
+    if (MULTI == 1) {
       double* slot = slots + parity * 4;
       if (threadIdx.x == 0) {
 #pragma unroll
@@ -114,17 +142,39 @@ struct Team {
       for (int i = 0; i < NV; ++i) v[i] = bc[i];
       __syncthreads();
       parity ^= 1;
+    } else if (MULTI == 2) {
+      double* mine = wslots + ((size_t)parity * C + rank) * 4;
+      if (threadIdx.x == 0) {
+#pragma unroll
+        for (int i = 0; i < NV; ++i) mine[i] = v[i];
+      }
+      sync();
+      if (threadIdx.x < 32) {       // lane l adds ranks l, l + 32, ... in order, then a fixed shuffle tree
+        const int lane = threadIdx.x;
+#pragma unroll
+        for (int i = 0; i < NV; ++i) {
+          double t = 0.0;
+          for (int r = lane; r < C; r += 32) t += __ldcg(wslots + ((size_t)parity * C + r) * 4 + i);
+          t = warp_sum(t);
+          if (lane == 0) bc[i] = t;
+        }
+      }
+      __syncthreads();
+#pragma unroll
+      for (int i = 0; i < NV; ++i) v[i] = bc[i];
+      __syncthreads();
+      parity ^= 1;
     }
   }
 };
 
-template <bool MULTI, typename TX> __device__ __forceinline__ TX ldv(const TX* x) {
-  if (MULTI) return __ldcg(x);   // written by another CTA of the cluster during this launch: read at L2
-  return *x;
+template <int MULTI, typename TX> __device__ __forceinline__ TX ldv(const TX* x) {
+  if (MULTI == 1) return __ldcg(x);   // written by another CTA of the cluster during this launch: read at L2
+  return *x;                          // wide teams: every phase ends in Team::sync, whose gpu-scope fence drops the SM's L1 lines
 }
 
 // y = op(rows [lo,hi)) . x with a group of G (power of two <= 32) lanes per row; emit(row, dot) runs on lane 0.
-template <typename TACC, bool MULTI, typename TV, typename IT, typename TX, typename F>
+template <typename TACC, int MULTI, typename TV, typename IT, typename TX, typename F>
 __device__ __forceinline__ void spmv_rows(int lo, int hi, const int* __restrict__ rp, const IT* __restrict__ ci,
                                           const TV* __restrict__ v, const TX* x, int G, F emit) {
   const int tid = threadIdx.x;
@@ -135,16 +185,23 @@ __device__ __forceinline__ void spmv_rows(int lo, int hi, const int* __restrict_
     TACC acc = (TACC)0;
     if (row < hi) {
       const int e0 = __ldg(rp + row), e1 = __ldg(rp + row + 1);
-      int e = e0 + gl;
-      for (; e + 3 * G < e1; e += 4 * G) {       // four independent loads in flight per lane
-        const TV v0 = __ldg(v + e), v1 = __ldg(v + e + G), v2 = __ldg(v + e + 2 * G), v3 = __ldg(v + e + 3 * G);
-        const int c0 = __ldg(ci + e), c1 = __ldg(ci + e + G), c2 = __ldg(ci + e + 2 * G), c3 = __ldg(ci + e + 3 * G);
-        acc += (TACC)v0 * (TACC)ldv<MULTI>(x + c0);
-        acc += (TACC)v1 * (TACC)ldv<MULTI>(x + c1);
-        acc += (TACC)v2 * (TACC)ldv<MULTI>(x + c2);
-        acc += (TACC)v3 * (TACC)ldv<MULTI>(x + c3);
+      // eight independent (value, index) loads in flight per lane, then the eight gathers; out-of-row slots read element
+      // e0 with weight 0, so a row of any length costs ceil(len / 8G) round trips and no serial tail
+      for (int e = e0 + gl; e < e1; e += 8 * G) {
+        TV vv[8]; int cc[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+          const int idx = e + u * G;
+          const bool ok = idx < e1;
+          vv[u] = ok ? __ldg(v + idx) : (TV)0;
+          cc[u] = ok ? (int)__ldg(ci + idx) : (int)__ldg(ci + e0);
+        }
+        TX xx[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) xx[u] = ldv<MULTI>(x + cc[u]);
+#pragma unroll
+        for (int u = 0; u < 8; ++u) acc += (TACC)vv[u] * (TACC)xx[u];
       }
-      for (; e < e1; e += G) acc += (TACC)__ldg(v + e) * (TACC)ldv<MULTI>(x + (int)__ldg(ci + e));
     }
     for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
     if (row < hi && gl == 0) emit(row, acc);
@@ -152,7 +209,7 @@ __device__ __forceinline__ void spmv_rows(int lo, int hi, const int* __restrict_
 }
 
 // Dense row-major block (n x n, global or shared): one warp per row.
-template <typename TACC, bool MULTI, typename TV, typename TX, typename F>
+template <typename TACC, int MULTI, typename TV, typename TX, typename F>
 __device__ __forceinline__ void dense_rows(int lo, int hi, int n, const TV* __restrict__ Pm, const TX* x, F emit) {
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
   for (int row = lo + wid; row < hi; row += nw) {
@@ -219,7 +276,7 @@ __device__ __forceinline__ void sell_rows(const Sell<TV, IT>& S, int b, const TX
   __syncthreads();
 }
 
-template <typename T, typename IT, bool MULTI>
+template <typename T, typename IT, int MULTI>
 struct Prob {  // one problem's view of the batch, as seen by one CTA of its team
   int n, m, b;
   int nlo, nhi, mlo, mhi;             // this CTA's share of the variables / rows
@@ -262,17 +319,17 @@ struct Prob {  // one problem's view of the batch, as seen by one CTA of its tea
 };
 
 // One pass over the rows of A, A^T or P owned by this CTA: warp batches (single-CTA teams) or lane groups per row.
-template <typename TACC, typename T, typename IT, bool MULTI, typename TX, typename F>
+template <typename TACC, typename T, typename IT, int MULTI, typename TX, typename F>
 __device__ __forceinline__ void rows_A(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const TX* x, F emit) {
   if (D.batched) sell_rows<TACC>(D.SA, c.b, x, reinterpret_cast<TACC*>(c.scratch), emit);
   else spmv_rows<TACC, MULTI>(c.mlo, c.mhi, c.A_rp, D.A_ci, D.A_v, x, D.A_G, emit);
 }
-template <typename TACC, typename T, typename IT, bool MULTI, typename TX, typename F>
+template <typename TACC, typename T, typename IT, int MULTI, typename TX, typename F>
 __device__ __forceinline__ void rows_AT(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const TX* x, F emit) {
   if (D.batched) sell_rows<TACC>(D.SAT, c.b, x, reinterpret_cast<TACC*>(c.scratch), emit);
   else spmv_rows<TACC, MULTI>(c.nlo, c.nhi, c.AT_rp, D.AT_ci, D.AT_v, x, D.AT_G, emit);
 }
-template <typename TACC, typename T, typename IT, bool MULTI, typename TX, typename F>
+template <typename TACC, typename T, typename IT, int MULTI, typename TX, typename F>
 __device__ __forceinline__ void rows_P(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const TX* x, F emit) {
   if (c.Pd) dense_rows<TACC, MULTI>(c.nlo, c.nhi, c.n, c.Pd, x, emit);
   else if (D.batched) sell_rows<TACC>(D.SP, c.b, x, reinterpret_cast<TACC*>(c.scratch), emit);
@@ -280,7 +337,7 @@ __device__ __forceinline__ void rows_P(const BatchDev<T, IT>& D, const Prob<T, I
 }
 
 // q = M p for the CG: tA = rho A p ; Ap = A' tA + P p + sigma p ; returns the team-wide <p, Ap>.
-template <typename T, typename IT, bool MULTI>
+template <typename T, typename IT, int MULTI>
 __device__ __forceinline__ double apply_M(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c) {
   const T rhoT = (T)c.rho, sigT = (T)c.sigma;
   rows_A<T>(D, c, c.p, [&](int row, T a) { c.tA[row] = rhoT * a; });
@@ -301,7 +358,7 @@ __device__ __forceinline__ double apply_M(const BatchDev<T, IT>& D, const Prob<T
 
 // Jacobi-preconditioned CG on M d = r, d0 = 0. r (T) holds the right-hand side on entry (owner rows).
 // Stops when the recursive residual satisfies ||r|| <= thresh (reading A5). Returns iterations.
-template <typename T, typename IT, bool MULTI>
+template <typename T, typename IT, int MULTI>
 __device__ int pcg(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, double thresh, double rr0, int* flag) {
   const int tid = threadIdx.x, nt = blockDim.x;
   double acc[2] = {0.0, 0.0};
@@ -345,7 +402,7 @@ __device__ int pcg(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, double
 // (identical to CG started at xbase); each further pass re-evaluates the residual in fp64 and corrects
 // (iterative refinement). Guards ||rhs|| = 0 => out = 0 (reading A5).
 // rhs: owner rows valid. out: every row valid team-wide on return (after a team sync).
-template <typename T, typename IT, bool MULTI>
+template <typename T, typename IT, int MULTI>
 __device__ int solve_M(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const double* rhs, const double* xbase,
                        double* out, int* flag, int* it0) {
   const int tid = threadIdx.x, nt = blockDim.x;
@@ -403,7 +460,7 @@ __device__ int solve_M(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, co
 }
 
 // xi and x-tilde of one step from z^k = (x, s, y): S1 + S2. Writes xt; st is produced by the caller's A pass.
-template <typename T, typename IT, bool MULTI>
+template <typename T, typename IT, int MULTI>
 __device__ int lin_solve_step(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const double* x, const double* s,
                               const double* y, double* xt, int* flag, int* it0) {
   const int tid = threadIdx.x, nt = blockDim.x;
@@ -429,10 +486,10 @@ struct IterPtrs {
   __shared__ double bc_[4];                                                                    \
   extern __shared__ __align__(16) unsigned char dsm_[];                                        \
   Team<MULTI> team;                                                                            \
-  team.init(sh_, slots_, bc_);                                                                 \
+  team.init(sh_, slots_, bc_, D.wide);                                                         \
   const int nteams = (int)gridDim.x / team.C, team_id = (int)blockIdx.x / team.C;
 
-template <typename T, typename IT, bool MULTI>
+template <typename T, typename IT, int MULTI>
 __global__ void __launch_bounds__(1024) k_fwd(BatchDev<T, IT> D, Hyper<T> H, IterPtrs I, int k) {
   CDU_TEAM_PROLOGUE();
   const int tid = threadIdx.x, nt = blockDim.x;
@@ -514,7 +571,7 @@ struct BwdPtrs {
 };
 
 // Phase 1 of the reverse step: (LEAN: re-solve), w, and B1/B2/B4 for zero, nonneg and SOC rows.
-template <typename T, typename IT, bool MULTI>
+template <typename T, typename IT, int MULTI>
 __device__ void bwd_pre(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const BwdPtrs& Q, double* out_part, int* flag,
                         int* iters, int* it0) {
   const int b = c.b, tid = threadIdx.x, nt = blockDim.x;
@@ -585,7 +642,7 @@ __device__ void bwd_pre(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const B
 }
 
 // Phase 2: B5-B9 with the adjoint solve; needs GW complete on every row (PSD rows written by the PSD kernels).
-template <typename T, typename IT, bool MULTI>
+template <typename T, typename IT, int MULTI>
 __device__ void bwd_post(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const BwdPtrs& Q, const double* part, int k,
                          int* flag, int* iters, int* it0) {
   const int b = c.b, tid = threadIdx.x, nt = blockDim.x;
@@ -631,7 +688,7 @@ __device__ void bwd_post(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const 
   }
 }
 
-template <typename T, typename IT, bool MULTI>
+template <typename T, typename IT, int MULTI>
 __global__ void __launch_bounds__(1024) k_bwd(BatchDev<T, IT> D, Hyper<T> H, BwdPtrs Q, int k, int phase) {
   // phase 0: pre + post fused (no PSD blocks anywhere); 1: pre only; 2: post only
   CDU_TEAM_PROLOGUE();

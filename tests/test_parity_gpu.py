@@ -247,6 +247,25 @@ def test_diagonal_M_path_and_pcg_path_agree():
         PU.assert_within(e, "f64")
 
 
+def test_fig2_linear_solve_and_wide_teams():
+    """PAPER.md Fig. 2 workload (L247-255) at n = 2000, fp64: one step x-tilde = M^-1 xi and its matrix-free backward against
+    the dense oracle, with the default team shape and with wide teams (CTAs of a cooperative launch meeting at a global
+    counter, lin.cuh Team<2>) of 24 and of 5 CTAs. Wide teams are also run on a mixed-cone batch (SOC rows cross CTAs)."""
+    wl = W.make_fig2(2000, batch=2)
+    for ts in (0, 24, 5 + 16):
+        e, st = PU.check(wl, team_size=ts)
+        print(wl.name, ts, e, st)
+        PU.assert_within(e, "f64")
+        assert st["flags_or"] == 0
+    wl = _mixed_workload("f64", seed=11)
+    e, st = PU.check(wl, team_size=20)
+    PU.assert_within(e, "f64")
+    wl32 = W.make_fig2(3000, batch=1, dtype="f32")
+    e, st = PU.check(wl32, team_size=40)
+    print(wl32.name, e, st)
+    PU.assert_within(e, "f32")
+
+
 def test_ragged_large_blocks_two_orders():
     """Two different large orders in one batch (136 and 160): per-block offsets of the large path, FMA GEMMs."""
     a = W.make_config(5, batch=1, p=136, K=5)

@@ -17,6 +17,7 @@ from .generators import (  # noqa: F401
     erdos_renyi,
     ar1_rho_schedule,
     make_config,
+    make_fig2,
     pack_batch,
     CONFIG_NAMES,
     BASE_SEED,

@@ -312,6 +312,25 @@ def make_config(cfg: int, batch: Optional[int] = None, K: Optional[int] = None,
                     rho=_round_to(rho, dtype), alpha=_round_to(alpha, dtype), sigma=sigma, x0=x0, s0=s0, y0=y0)
 
 
+def make_fig2(n: int, batch: int = 1, dtype: str = "f64", seed_offset: int = 0) -> Workload:
+    """The linear-solve scaling workload of PAPER.md Fig. 2 / App. B (L96, L247-255): `batch` instances of
+    fig2_linear_problem(n) (m = n/2, diag P ~ U(0,10), A 1 % dense N(0,1), b ~ N(0,1)), ONE step (K = 1) with
+    rho ~ U(0,1) (a scalar per instance: per-row rho is SURVEY 8(f) F3), alpha = 1 (x_1 = x-tilde), sigma = 1e-6, from a
+    N(0,1) iterate. The loss of the experiment, 1/2 ||x-tilde - x*||^2, lives with the caller (x* ~ N(0,1))."""
+    problems, x0, s0, y0 = [], [], [], []
+    for b in range(batch):
+        rng = np.random.default_rng(BASE_SEED + 6000 + 97 * n + b + seed_offset)
+        pr = fig2_linear_problem(rng, n)
+        pr.name = f"fig2-n{n}-b{b}"
+        problems.append(_round_problem(pr, dtype))
+        x0.append(_round_to(rng.standard_normal(pr.n), dtype)); s0.append(_round_to(rng.standard_normal(pr.m), dtype))
+        y0.append(_round_to(rng.standard_normal(pr.m), dtype))
+    hrng = np.random.default_rng(BASE_SEED + 6000 + 999)
+    return Workload(name=f"fig2-linsolve-n{n}-b{batch}-{dtype}-K1", dtype=dtype, problems=problems, K=1,
+                    rho=_round_to(hrng.uniform(0.05, 1.0, 1), dtype), alpha=_round_to(np.ones(1), dtype), sigma=1e-6,
+                    x0=x0, s0=s0, y0=y0)
+
+
 # ----------------------------------------------------------------------------------------------
 # batched-CSR packing (layout of include/cdu.h `cdu_problem`)
 # ----------------------------------------------------------------------------------------------
