@@ -112,6 +112,31 @@ cdu_status cdu_backward(cdu_handle h, const void* g_xK, const void* g_sK, const 
                         void* g_rho, void* g_sigma, void* g_alpha, void* g_x0, void* g_s0, void* g_y0,
                         int32_t io_on_host, void* cuda_stream);
 
+/* cdu_backward with a cotangent on every intermediate iterate, for losses that read all iterates (Eq. 12,
+ * L146-148): inj_x [K-1][sum n_b], inj_s, inj_y [K-1][sum m_b] (row k-1 = dL/dz^k of the part of the loss that reads z^k,
+ * k = 1..K-1; any of the three may be NULL). Same outputs as cdu_backward. */
+cdu_status cdu_backward_inject(cdu_handle h, const void* g_xK, const void* g_sK, const void* g_yK,
+                               const void* inj_x, const void* inj_s, const void* inj_y,
+                               void* g_rho, void* g_sigma, void* g_alpha, void* g_x0, void* g_s0, void* g_y0,
+                               int32_t io_on_host, void* cuda_stream);
+
+/* The self-supervised training loss of PAPER.md Eq. 12 (L146) on the iterates of the last cdu_forward,
+ *   L_b = sum_{k=1..K} log( ||P x^k + q + A'y^k||^2 / det(||r_d^0||^2) + ||A x^k + s^k - b||^2 / det(||r_p^0||^2) )
+ * (det = stop-gradient: the residuals of z^0 enter as constants; a term whose denominator is 0 is dropped), and its reverse
+ * sweep: the cotangent of every z^k is formed from the stored iterate when the sweep reaches k, so memory stays O(n + nnz)
+ * per unrolled iteration (L92). loss: [batch] (NULL: not wanted); gradient outputs as cdu_backward (sums over the batch in
+ * CDU_RHO_PER_ITER mode are gradients of sum_b L_b). */
+cdu_status cdu_backward_eq12(cdu_handle h, void* loss, void* g_rho, void* g_sigma, void* g_alpha,
+                             void* g_x0, void* g_s0, void* g_y0, int32_t io_on_host, void* cuda_stream);
+
+/* Policy features of PAPER.md App. E (L321-339) for iterate k (0 <= k <= K of the last forward), each output may be NULL:
+ *   rp_bar [sum m_b] = (A x^k + s^k - b) / max(|A x^k|_inf, |s^k|_inf, |b|_inf)      (per problem, OSQP-style scaling)
+ *   rd_bar [sum n_b] = (P x^k + q + A'y^k) / max(|P x^k|_inf, |q|_inf, |A'y^k|_inf)
+ *   delta_p [sum m_b] = s^k - s-tilde^k (k >= 1, FULL checkpoints only: CDU_ESTATE otherwise), delta_d = s^k - s^(k-1) (k >= 1)
+ *   scal [batch][3]   = log(|rp_bar|_inf + 1e-12), log(|rd_bar|_inf + 1e-12), log(|delta_p|_inf + 1e-12) */
+cdu_status cdu_get_features(cdu_handle h, int32_t k, void* rp_bar, void* rd_bar, void* delta_p, void* delta_d, void* scal,
+                            int32_t io_on_host, void* cuda_stream);
+
 typedef struct {
   int64_t cg_iters_fwd;      /* CG iterations summed over problems and iterations, last forward            */
   int64_t cg_iters_bwd;      /* same for the adjoint solves (and LEAN re-solves) of the last backward       */

@@ -262,3 +262,60 @@ def run_workload(wl, cot_fn=None, x_star: Optional[Sequence[np.ndarray]] = None,
     res["g_alpha"] = np.sum(res["g_alpha_pb"], axis=0)
     res["g_sigma"] = float(np.sum(res["g_sigma_pb"]))
     return res
+
+
+# ---------------------------------------------------------------------------------------------
+# training loss of Eq. 12 (L146-148) and the policy features of App. E (L321-339)
+# ---------------------------------------------------------------------------------------------
+def eq12_loss(pr, un: Unroll) -> float:
+    """L = sum_{k=1..K} log(||r_d^k||^2 / det(||r_d^0||^2) + ||r_p^k||^2 / det(||r_p^0||^2))  (Eq. 12); a term whose
+    denominator is zero is dropped (paper silent; reading A12)."""
+    rp0, rd0 = residuals(pr, un.xs[0], un.ss[0], un.ys[0])
+    a0, b0 = rd0 @ rd0, rp0 @ rp0
+    L = 0.0
+    for k in range(1, len(un.xs)):
+        rp, rd = residuals(pr, un.xs[k], un.ss[k], un.ys[k])
+        Dk = (rd @ rd / a0 if a0 > 0 else 0.0) + (rp @ rp / b0 if b0 > 0 else 0.0)
+        if Dk > 0:
+            L += np.log(Dk)
+    return float(L)
+
+
+def eq12_cotangents(pr, un: Unroll):
+    """dL/dz^k of Eq. 12 for k = 1..K with the denominators detached ("det", L148): dict k -> (gx, gs, gy).
+    d/dx = (2/D_k)(P' r_d / a_0 + A' r_p / b_0), d/ds = (2/D_k) r_p / b_0, d/dy = (2/D_k) A r_d / a_0."""
+    rp0, rd0 = residuals(pr, un.xs[0], un.ss[0], un.ys[0])
+    a0, b0 = rd0 @ rd0, rp0 @ rp0
+    out = {}
+    for k in range(1, len(un.xs)):
+        rp, rd = residuals(pr, un.xs[k], un.ss[k], un.ys[k])
+        Dk = (rd @ rd / a0 if a0 > 0 else 0.0) + (rp @ rp / b0 if b0 > 0 else 0.0)
+        if not Dk > 0:
+            out[k] = (np.zeros(pr.n), np.zeros(pr.m), np.zeros(pr.m))
+            continue
+        c1 = 2.0 / (Dk * a0) if a0 > 0 else 0.0
+        c2 = 2.0 / (Dk * b0) if b0 > 0 else 0.0
+        out[k] = (c1 * (pr.P.T @ rd) + c2 * (pr.A.T @ rp), c2 * rp, c1 * (pr.A @ rd))
+    return out
+
+
+def backward_eq12(pr, un: Unroll) -> Grads:
+    """BPTT of the Eq. 12 loss: its cotangent on z^K is the terminal one, those on z^1..z^(K-1) are injected."""
+    cots = eq12_cotangents(pr, un)
+    K = len(un.tapes)
+    return backward(pr, un, *cots[K], inject={k: cots[k] for k in range(1, K)})
+
+
+def features(pr, un: Unroll, k: int, eps: float = 1e-12):
+    """App. E (L323-335): OSQP-scaled KKT residuals of z^k, the ADMM residuals delta_d = s^k - s^(k-1) and
+    delta_p = s^k - s-tilde^k, and the three log-infinity-norms the alpha policy reads."""
+    x, s, y = un.xs[k], un.ss[k], un.ys[k]
+    Ax, Px, ATy = pr.A @ x, pr.P @ x, pr.A.T @ y
+    inf = lambda v: float(np.max(np.abs(v), initial=0.0))
+    dp, dd = max(inf(Ax), inf(s), inf(pr.b)), max(inf(Px), inf(pr.q), inf(ATy))
+    rp_bar = (Ax + s - pr.b) / (dp if dp > 0 else 1.0)
+    rd_bar = (Px + pr.q + ATy) / (dd if dd > 0 else 1.0)
+    delta_d = s - un.ss[k - 1] if k >= 1 else np.zeros(pr.m)
+    delta_p = s - un.tapes[k - 1].st if k >= 1 else np.zeros(pr.m)
+    scal = np.log(np.array([inf(rp_bar), inf(rd_bar), inf(delta_p)]) + eps)
+    return dict(rp_bar=rp_bar, rd_bar=rd_bar, delta_p=delta_p, delta_d=delta_d, scal=scal)

@@ -28,7 +28,7 @@ _STATUS = {0: "CDU_OK", 1: "CDU_EINVAL", 2: "CDU_ENOMEM", 3: "CDU_ECUDA", 4: "CD
 
 EXPORTED_SYMBOLS = ("cdu_create", "cdu_forward", "cdu_backward", "cdu_get_stats", "cdu_get_iterate", "cdu_last_error",
                     "cdu_destroy", "cdu_version", "cdu_psd_project", "cdu_psd_vjp", "cdu_profile", "cdu_get_profile",
-                    "cdu_measure_peak")
+                    "cdu_measure_peak", "cdu_backward_inject", "cdu_backward_eq12", "cdu_get_features")
 
 
 class CduError(RuntimeError):
@@ -81,6 +81,12 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.cdu_forward.argtypes = [vp, i32, vp, i32, f64, vp, vp, vp, vp, vp, vp, vp, i32, vp]
     lib.cdu_backward.restype = i32
     lib.cdu_backward.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i32, vp]
+    lib.cdu_backward_inject.restype = i32
+    lib.cdu_backward_inject.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i32, vp]
+    lib.cdu_backward_eq12.restype = i32
+    lib.cdu_backward_eq12.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, vp]
+    lib.cdu_get_features.restype = i32
+    lib.cdu_get_features.argtypes = [vp, i32, vp, vp, vp, vp, vp, i32, vp]
     lib.cdu_get_stats.restype = i32
     lib.cdu_get_stats.argtypes = [vp, C.POINTER(_Stats)]
     lib.cdu_get_iterate.restype = i32
@@ -194,6 +200,42 @@ class Handle:
                                           _ptr(out.get("g_sigma")), _ptr(out.get("g_alpha")), _ptr(out.get("g_x0")),
                                           _ptr(out.get("g_s0")), _ptr(out.get("g_y0")), 1 if host else 0, _stream()))
         return out
+
+    def _grad_out(self, host):
+        torch = _torch()
+        cnt = self.K * (self.B if self.rho_mode == CDU_RHO_PER_PROBLEM else 1)
+        scnt = self.B if self.rho_mode == CDU_RHO_PER_PROBLEM else 1
+        sizes = dict(g_rho=cnt, g_alpha=cnt, g_sigma=scnt, g_x0=self.N, g_s0=self.M, g_y0=self.M)
+        if host:
+            return {k: torch.empty(n, dtype=self.torch_dtype).pin_memory() for k, n in sizes.items()}
+        return {k: torch.empty(n, dtype=self.torch_dtype, device="cuda") for k, n in sizes.items()}
+
+    def backward_inject(self, g_xK=None, g_sK=None, g_yK=None, inj_x=None, inj_s=None, inj_y=None, host=False):
+        """cdu_backward_inject: inj_x [K-1, N], inj_s, inj_y [K-1, M] are cotangents on z^1 .. z^(K-1)."""
+        out = self._grad_out(host)
+        self._check(self.lib.cdu_backward_inject(self.h, _ptr(g_xK), _ptr(g_sK), _ptr(g_yK), _ptr(inj_x), _ptr(inj_s), _ptr(inj_y),
+                                                 _ptr(out["g_rho"]), _ptr(out["g_sigma"]), _ptr(out["g_alpha"]), _ptr(out["g_x0"]),
+                                                 _ptr(out["g_s0"]), _ptr(out["g_y0"]), 1 if host else 0, _stream()))
+        return out
+
+    def backward_eq12(self, host=False):
+        """cdu_backward_eq12 -> (loss [B], gradients dict): the Eq. 12 training loss of the last forward and its reverse sweep."""
+        torch = _torch()
+        out = self._grad_out(host)
+        loss = torch.empty(self.B, dtype=self.torch_dtype).pin_memory() if host else torch.empty(self.B, dtype=self.torch_dtype, device="cuda")
+        self._check(self.lib.cdu_backward_eq12(self.h, _ptr(loss), _ptr(out["g_rho"]), _ptr(out["g_sigma"]), _ptr(out["g_alpha"]),
+                                               _ptr(out["g_x0"]), _ptr(out["g_s0"]), _ptr(out["g_y0"]), 1 if host else 0, _stream()))
+        return loss, out
+
+    def features(self, k: int):
+        """cdu_get_features of iterate k -> dict(rp_bar [M], rd_bar [N], delta_p [M], delta_d [M], scal [B, 3])."""
+        torch = _torch()
+        mk = lambda n: torch.empty(n, dtype=self.torch_dtype, device="cuda")
+        o = dict(rp_bar=mk(self.M), rd_bar=mk(self.N), delta_p=mk(self.M), delta_d=mk(self.M), scal=mk(self.B * 3))
+        self._check(self.lib.cdu_get_features(self.h, k, _ptr(o["rp_bar"]), _ptr(o["rd_bar"]), _ptr(o["delta_p"]), _ptr(o["delta_d"]),
+                                              _ptr(o["scal"]), 0, _stream()))
+        o["scal"] = o["scal"].view(self.B, 3)
+        return o
 
     def iterate(self, k: int):
         torch = _torch()

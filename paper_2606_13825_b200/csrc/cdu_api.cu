@@ -65,6 +65,30 @@ cdu_status cdu_backward(cdu_handle h, const void* g_xK, const void* g_sK, const 
   return h->backward(g_xK, g_sK, g_yK, g_rho, g_sigma, g_alpha, g_x0, g_s0, g_y0, io_on_host, reinterpret_cast<cudaStream_t>(cuda_stream));
 }
 
+cdu_status cdu_backward_inject(cdu_handle h, const void* g_xK, const void* g_sK, const void* g_yK, const void* inj_x,
+                               const void* inj_s, const void* inj_y, void* g_rho, void* g_sigma, void* g_alpha, void* g_x0,
+                               void* g_s0, void* g_y0, int32_t io_on_host, void* cuda_stream) {
+  if (!h) return CDU_EINVAL;
+  DeviceGuard g(h->device);
+  cdu_handle_s::Extra ex; ex.ix = inj_x; ex.is = inj_s; ex.iy = inj_y;
+  return h->backward(g_xK, g_sK, g_yK, g_rho, g_sigma, g_alpha, g_x0, g_s0, g_y0, io_on_host, reinterpret_cast<cudaStream_t>(cuda_stream), &ex);
+}
+
+cdu_status cdu_backward_eq12(cdu_handle h, void* loss, void* g_rho, void* g_sigma, void* g_alpha, void* g_x0, void* g_s0,
+                             void* g_y0, int32_t io_on_host, void* cuda_stream) {
+  if (!h) return CDU_EINVAL;
+  DeviceGuard g(h->device);
+  cdu_handle_s::Extra ex; ex.eq12 = 1; ex.loss = loss;
+  return h->backward(nullptr, nullptr, nullptr, g_rho, g_sigma, g_alpha, g_x0, g_s0, g_y0, io_on_host, reinterpret_cast<cudaStream_t>(cuda_stream), &ex);
+}
+
+cdu_status cdu_get_features(cdu_handle h, int32_t k, void* rp_bar, void* rd_bar, void* delta_p, void* delta_d, void* scal,
+                            int32_t io_on_host, void* cuda_stream) {
+  if (!h) return CDU_EINVAL;
+  DeviceGuard g(h->device);
+  return h->features(k, rp_bar, rd_bar, delta_p, delta_d, scal, io_on_host, reinterpret_cast<cudaStream_t>(cuda_stream));
+}
+
 cdu_status cdu_get_stats(cdu_handle h, cdu_stats* out) {
   if (!h) return CDU_EINVAL;
   DeviceGuard g(h->device);

@@ -17,6 +17,7 @@
 #include "handle_base.h"
 #include "lin.cuh"
 #include "lin_diag.cuh"
+#include "eq12.cuh"
 #include "psd_large.cuh"
 #include "psd_bjacobi.cuh"
 #include "psd_small.cuh"
@@ -472,6 +473,7 @@ struct HandleT : cdu_handle_s {
   bool diag_on = false;              // M is diagonal: closed-form linear step (lin_diag.cuh)
   DiagTab DG{};
   T* d_aval = nullptr;
+  double *feat_part = nullptr, *nrm_all = nullptr, *nrm_one = nullptr;   // eq12.cuh scratch
   size_t lin_smem = 0;               // dynamic shared memory of the linear-step kernels
   PsdEngine<T> psd;
   int B = 0, K_max = 0, ckpt_mode = 0, lin_threads = 256;
@@ -530,7 +532,9 @@ struct HandleT : cdu_handle_s {
   cdu_status forward(int K, const void* rho, int mode, double sigma, const void* alpha, const void* x0, const void* s0,
                      const void* y0, void* xK, void* sK, void* yK, int host, cudaStream_t st) override;
   cdu_status backward(const void* gx, const void* gs, const void* gy, void* g_rho, void* g_sigma, void* g_alpha,
-                      void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st) override;
+                      void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st, const Extra* ex) override;
+  cdu_status features(int k, void* rp_bar, void* rd_bar, void* delta_p, void* delta_d, void* scal, int host, cudaStream_t st) override;
+  cdu_status add_extra(int k, double* Gz, const Extra* ex, int host, cudaStream_t st);
   cdu_status stats(cdu_stats* out) override;
   cdu_status iterate(int k, void* x, void* s, void* y, int host, cudaStream_t st) override;
   void profile_enable(int on) override { prof.on = on != 0; }
@@ -692,11 +696,9 @@ cdu_status HandleT<T, IT>::init(const cdu_problem* pr, const cdu_options* op, cu
       for (long long i = 0; ok && i < n; ++i)
         for (long long e = P_rp[v0 + i]; e < P_rp[v0 + i + 1]; ++e) if (pr->P_colidx[e] != i && Pv[e] != (T)0) { ok = false; break; }
     }
-    if (ok) {
-      std::vector<int> acol((size_t)Mtot, -1), choff(B + 1, 0);
-      std::vector<T> aval((size_t)Mtot, (T)0);
+    {   // chunk table: also serves the residual / Eq. 12 / feature kernels (eq12.cuh) of every handle
+      std::vector<int> choff(B + 1, 0);
       std::vector<int4> chunks;
-      for (long long r = 0; r < Mtot; ++r) if (A_rp[r + 1] > A_rp[r]) { acol[r] = pr->A_colidx[A_rp[r]]; aval[r] = Av[A_rp[r]]; }
       for (int b = 0; b < B; ++b) {
         const int items = (int)std::max(pr->var_off[b + 1] - pr->var_off[b], pr->row_off[b + 1] - pr->row_off[b]);
         int idx = 0;
@@ -704,9 +706,20 @@ cdu_status HandleT<T, IT>::init(const cdu_problem* pr, const cdu_options* op, cu
         choff[b + 1] = (int)chunks.size();
       }
       DG.nchunk = (int)chunks.size();
-      DG.chunk = pool.upload(chunks, st); DG.chunk_off = pool.upload(choff, st); DG.acol = pool.upload(acol, st);
+      DG.chunk = pool.upload(chunks, st); DG.chunk_off = pool.upload(choff, st);
+      DG.part = pool.zeros<double>((size_t)DG.nchunk * RES_NV, st); DG.ticket = pool.zeros<unsigned>(B, st);
+      feat_part = pool.zeros<double>((size_t)DG.nchunk * 4, st);
+      nrm_all = pool.zeros<double>((size_t)(K_max + 1) * B * RES_NV, st);
+      nrm_one = pool.zeros<double>((size_t)B * RES_NV, st);
+      if (pool.last != cudaSuccess) { err = std::string("cdu_create (chunk table): ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
+      CU_OK(cudaStreamSynchronize(st));
+    }
+    if (ok) {
+      std::vector<int> acol((size_t)Mtot, -1);
+      std::vector<T> aval((size_t)Mtot, (T)0);
+      for (long long r = 0; r < Mtot; ++r) if (A_rp[r + 1] > A_rp[r]) { acol[r] = pr->A_colidx[A_rp[r]]; aval[r] = Av[A_rp[r]]; }
+      DG.acol = pool.upload(acol, st);
       d_aval = pool.upload(aval, st);
-      DG.part = pool.zeros<double>((size_t)DG.nchunk * 4, st); DG.ticket = pool.zeros<unsigned>(B, st);
       if (pool.last != cudaSuccess) { err = std::string("cdu_create (diagonal path): ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
       CU_OK(cudaStreamSynchronize(st));   // staging vectors go out of scope
       diag_on = true;
@@ -869,7 +882,7 @@ cdu_status HandleT<T, IT>::init(const cdu_problem* pr, const cdu_options* op, cu
   g_rho_pb = pool.zeros<double>((size_t)K_max * B, st); g_alpha_pb = pool.zeros<double>((size_t)K_max * B, st);
   g_sigma_pb = pool.zeros<double>((size_t)K_max * B, st); part_pre = pool.zeros<double>(2 * (size_t)B, st);
   d_rho = pool.alloc<T>((size_t)K_max * B); d_alpha = pool.alloc<T>((size_t)K_max * B);
-  stage = pool.alloc<T>(zstride); stage_g = pool.alloc<T>(2 * (size_t)K_max * B + B);
+  stage = pool.alloc<T>(zstride + Mtot); stage_g = pool.alloc<T>(2 * (size_t)K_max * B + B);
   if (pool.last != cudaSuccess || !GZ[0] || !GZ[1] || !stage || !stage_g) { err = std::string("cdu_create: ") + cudaGetErrorString(pool.last); return CDU_ENOMEM; }
   CU_OK(cudaStreamSynchronize(st));   // host vectors above go out of scope
   return CDU_OK;
@@ -974,13 +987,83 @@ cdu_status HandleT<T, IT>::forward(int K, const void* rho, int mode, double sigm
 }
 
 template <typename T, typename IT>
+cdu_status HandleT<T, IT>::add_extra(int k, double* Gz, const Extra* ex, int host, cudaStream_t st) {
+  // cotangent of z^k += the caller's row k-1 (1 <= k <= K-1) and / or dL/dz^k of Eq. 12 (1 <= k <= K)
+  if (!ex || k < 1) return CDU_OK;
+  if (k <= K_last - 1) {
+    const void* src[3] = {ex->ix, ex->is, ex->iy};
+    const long long len[3] = {N, Mtot, Mtot};
+    double* dst[3] = {Gz, Gz + N, Gz + N + Mtot};
+    T* stg = stage;
+    for (int i = 0; i < 3; ++i) {
+      if (!src[i] || len[i] == 0) continue;
+      const T* d = reinterpret_cast<const T*>(src[i]) + (size_t)(k - 1) * len[i];
+      if (host) { CU_OK(cudaMemcpyAsync(stg, d, len[i] * sizeof(T), cudaMemcpyHostToDevice, st)); d = stg; stg += len[i]; }
+      k_add_vec<T><<<(int)std::min<long long>((len[i] + 255) / 256, 2048), 256, 0, st>>>(dst[i], d, len[i]);
+      ++launches;
+      CU_OK(cudaGetLastError());
+    }
+  }
+  if (ex->eq12) {
+    prof.begin(PC_MISC, st);
+    k_residuals<T, IT><<<DG.nchunk, DIAG_THREADS, 0, st>>>(D, DG, z_at(k), D.tm, D.rd, nrm_one);
+    k_eq12_cot<T, IT><<<DG.nchunk, DIAG_THREADS, 0, st>>>(D, DG, D.tm, D.rd, nrm_all + (size_t)k * B * RES_NV, nrm_all, Gz);
+    prof.end(st);
+    launches += 2;
+    CU_OK(cudaGetLastError());
+  }
+  return CDU_OK;
+}
+
+template <typename T, typename IT>
+cdu_status HandleT<T, IT>::features(int k, void* rp_bar, void* rd_bar, void* delta_p, void* delta_d, void* scal, int host, cudaStream_t st) {
+  if (k < 0 || k > K_last || K_last < 1) { err = "cdu_get_features: k out of range (or no forward pass)"; return CDU_EINVAL; }
+  if (delta_p && k >= 1 && ckpt_mode != CDU_CKPT_FULL) { err = "cdu_get_features: delta_p needs FULL checkpoints (s-tilde is not stored in LEAN mode)"; return CDU_ESTATE; }
+  last_stream = st;
+  k_residuals<T, IT><<<DG.nchunk, DIAG_THREADS, 0, st>>>(D, DG, z_at(k), D.tm, D.rd, nrm_one);
+  T* o_rp = host ? stage : (T*)rp_bar; T* o_rd = host ? stage + Mtot : (T*)rd_bar;
+  T* o_dp = host ? stage + Mtot + N : (T*)delta_p; T* o_dd = host ? stage + 2 * Mtot + N : (T*)delta_d;
+  T* o_sc = host ? stage_g : (T*)scal;
+  if (host) { if (!rp_bar) o_rp = nullptr; if (!rd_bar) o_rd = nullptr; if (!delta_p) o_dp = nullptr; if (!delta_d) o_dd = nullptr; }
+  const double* sk = z_at(k) + N;
+  const double* skm1 = k >= 1 ? z_at(k - 1) + N : nullptr;
+  const double* stk = (k >= 1 && ckpt_mode == CDU_CKPT_FULL) ? ST + (size_t)(k - 1) * Mtot : nullptr;
+  k_features<T, IT><<<DG.nchunk, DIAG_THREADS, 0, st>>>(D, DG, D.tm, D.rd, nrm_one, sk, skm1, stk, o_rp, o_rd, o_dp, o_dd, feat_part);
+  if (scal) k_features_fin<T><<<(B + 127) / 128, 128, 0, st>>>(DG, B, feat_part, o_sc);
+  launches += 3;
+  CU_OK(cudaGetLastError());
+  if (host) {
+    if (rp_bar) CU_OK(cudaMemcpyAsync(rp_bar, o_rp, Mtot * sizeof(T), cudaMemcpyDeviceToHost, st));
+    if (rd_bar) CU_OK(cudaMemcpyAsync(rd_bar, o_rd, N * sizeof(T), cudaMemcpyDeviceToHost, st));
+    if (delta_p) CU_OK(cudaMemcpyAsync(delta_p, o_dp, Mtot * sizeof(T), cudaMemcpyDeviceToHost, st));
+    if (delta_d) CU_OK(cudaMemcpyAsync(delta_d, o_dd, Mtot * sizeof(T), cudaMemcpyDeviceToHost, st));
+    if (scal) CU_OK(cudaMemcpyAsync(scal, o_sc, (size_t)B * 3 * sizeof(T), cudaMemcpyDeviceToHost, st));
+    CU_OK(cudaStreamSynchronize(st));
+  }
+  return CDU_OK;
+}
+
+template <typename T, typename IT>
 cdu_status HandleT<T, IT>::backward(const void* gx, const void* gs, const void* gy, void* g_rho, void* g_sigma, void* g_alpha,
-                                void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st) {
+                                void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st, const Extra* ex) {
   if (K_last < 1) { err = "cdu_backward: no forward pass on this handle"; return CDU_ESTATE; }
   const int K = K_last;
   last_stream = st;
   cdu_status s = import_state(GZ[K & 1], gx, gs, gy, host, st);
   if (s != CDU_OK) return s;
+  if (ex && ex->eq12) {   // residual norms of every iterate (loss value; a_0, b_0 and a_k, b_k of the cotangents)
+    for (int k = 0; k <= K; ++k)
+      k_residuals<T, IT><<<DG.nchunk, DIAG_THREADS, 0, st>>>(D, DG, z_at(k), D.tm, D.rd, nrm_all + (size_t)k * B * RES_NV);
+    launches += K + 1;
+    if (ex->loss) {
+      T* o = host ? stage_g : reinterpret_cast<T*>(ex->loss);
+      k_eq12_loss<T><<<(B + 127) / 128, 128, 0, st>>>(nrm_all, K, B, o);
+      ++launches;
+      if (host) CU_OK(cudaMemcpyAsync(ex->loss, o, (size_t)B * sizeof(T), cudaMemcpyDeviceToHost, st));
+    }
+    CU_OK(cudaGetLastError());
+  }
+  if ((s = add_extra(K, GZ[K & 1], ex, host, st)) != CDU_OK) return s;     // Eq. 12 term of z^K (caller rows stop at K-1)
   CU_OK(cudaMemsetAsync(cg_b, 0, B * sizeof(int), st));
   CU_OK(cudaMemsetAsync(cg_b0, 0, B * sizeof(int), st));
   const Hyper<T> H = hyper();
@@ -1025,6 +1108,7 @@ cdu_status HandleT<T, IT>::backward(const void* gx, const void* gs, const void* 
       ++launches;
       CU_OK(le);
     }
+    if ((s = add_extra(k, Q.Gout, ex, host, st)) != CDU_OK) return s;     // cotangents that enter at z^k
   }
   const int pp = mode_last == CDU_RHO_PER_PROBLEM;
   const size_t cnt = (size_t)K * (pp ? B : 1), scnt = pp ? B : 1;

@@ -11,8 +11,14 @@ struct cdu_handle_s {
   virtual ~cdu_handle_s() {}
   virtual cdu_status forward(int K, const void* rho, int mode, double sigma, const void* alpha, const void* x0,
                              const void* s0, const void* y0, void* xK, void* sK, void* yK, int host, cudaStream_t st) = 0;
+  struct Extra {             // cotangents on the intermediate iterates (cdu_backward_inject / cdu_backward_eq12)
+    const void *ix = nullptr, *is = nullptr, *iy = nullptr;   // [K-1][.]: row k-1 is added to the cotangent of z^k
+    int eq12 = 0;            // add dL/dz^k of PAPER.md Eq. 12 for k = 1..K
+    void* loss = nullptr;    // eq12: [B] loss values out
+  };
   virtual cdu_status backward(const void* gx, const void* gs, const void* gy, void* g_rho, void* g_sigma, void* g_alpha,
-                              void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st) = 0;
+                              void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st, const Extra* ex = nullptr) = 0;
+  virtual cdu_status features(int k, void* rp_bar, void* rd_bar, void* delta_p, void* delta_d, void* scal, int host, cudaStream_t st) = 0;
   virtual cdu_status stats(cdu_stats* out) = 0;
   virtual cdu_status iterate(int k, void* x, void* s, void* y, int host, cudaStream_t st) = 0;
   virtual void profile_enable(int on) = 0;

@@ -230,3 +230,70 @@ def test_injected_cotangents_match_central_differences():
     un = O.unroll(pr, K, rho, alpha, sigma)
     g = O.backward(pr, un, *sp_(cs[K]), inject={k: sp_(cs[k]) for k in range(1, K)})
     assert nrm_rel_err(g.g_alpha, central_diff_grad(loss, alpha, 1e-6, rel=False)) < 2e-6
+
+
+# ---- Eq. 12 loss and App. E features (L321-339) -----------------------------------------------------
+def test_eq12_cotangents_and_total_gradient_match_central_differences():
+    """(a) eq12_cotangents = dL/dz^k with L as a function of the iterates alone (denominators detached) by central
+    differences on a few coordinates; (b) backward_eq12 = d eq12_loss / d(rho_k, alpha_k, x0) of the whole unroll by central
+    differences, again with detached denominators (the loss is re-evaluated against the unperturbed z^0 residuals)."""
+    from workloads import random_mixed_problem
+    rng = np.random.default_rng(12)
+    pr = random_mixed_problem(rng, n=7)
+    K = 5
+    rho = np.exp(rng.uniform(-1, 1, K)); alpha = rng.uniform(1.0, 1.8, K); sigma = 1e-6
+    z0 = (0.3 * rng.standard_normal(pr.n), 0.3 * rng.standard_normal(pr.m), 0.3 * rng.standard_normal(pr.m))
+    un = O.unroll(pr, K, rho, alpha, sigma, *z0)
+    rp0, rd0 = O.residuals(pr, *z0)
+    a0, b0 = rd0 @ rd0, rp0 @ rp0
+
+    def loss_of_iterates(xs, ss, ys):            # denominators fixed at the unperturbed z^0
+        L = 0.0
+        for k in range(1, K + 1):
+            rp, rd = O.residuals(pr, xs[k], ss[k], ys[k])
+            L += np.log(rd @ rd / a0 + rp @ rp / b0)
+        return L
+
+    assert abs(loss_of_iterates(un.xs, un.ss, un.ys) - O.eq12_loss(pr, un)) < 1e-12
+    cots = O.eq12_cotangents(pr, un)
+    h = 1e-6
+    for k in (1, 3, K):
+        for part, vecs in enumerate((un.xs, un.ss, un.ys)):
+            for i in (0, len(vecs[k]) - 1):
+                def pert(d):
+                    cp = [[v.copy() for v in un.xs], [v.copy() for v in un.ss], [v.copy() for v in un.ys]]
+                    cp[part][k][i] += d
+                    return loss_of_iterates(*cp)
+                fd = (pert(h) - pert(-h)) / (2 * h)
+                assert abs(fd - cots[k][part][i]) <= 1e-6 * max(1.0, abs(fd)), (k, part, i, fd, cots[k][part][i])
+    g = O.backward_eq12(pr, un)
+
+    def total(rho_, alpha_, x0_):
+        u = O.unroll(pr, K, rho_, alpha_, sigma, x0_, z0[1], z0[2], keep_tape=False)
+        return loss_of_iterates(u.xs, u.ss, u.ys)
+
+    for k in (0, 2, K - 1):
+        d = np.zeros(K); d[k] = 1e-6
+        fd = (total(rho + d, alpha, z0[0]) - total(rho - d, alpha, z0[0])) / 2e-6
+        assert abs(fd - g.g_rho_scalar[k]) <= 2e-5 * max(1.0, abs(fd)), (k, fd, g.g_rho_scalar[k])
+        fd = (total(rho, alpha + d, z0[0]) - total(rho, alpha - d, z0[0])) / 2e-6
+        assert abs(fd - g.g_alpha[k]) <= 2e-5 * max(1.0, abs(fd)), (k, fd, g.g_alpha[k])
+    # x0 enters the loss only through the iterates (z^0's own residuals are detached and k starts at 1)
+    d = np.zeros(pr.n); d[1] = 1e-6
+    fd = (total(rho, alpha, z0[0] + d) - total(rho, alpha, z0[0] - d)) / 2e-6
+    assert abs(fd - g.g_x0[1]) <= 2e-5 * max(1.0, abs(fd))
+
+
+def test_features_hand_case():
+    """App. E on a two-variable problem typed out by hand: A = I, P = 2 I, q = (1, -1), b = (0, 3)."""
+    import scipy.sparse as sp
+    from workloads.generators import Problem, NONNEG
+    pr = Problem(P=sp.csr_matrix(2.0 * np.eye(2)), q=np.array([1.0, -1.0]), A=sp.csr_matrix(np.eye(2)), b=np.array([0.0, 3.0]),
+                 cones=[(NONNEG, 2)], name="hand")
+    un = O.unroll(pr, 2, np.array([1.0, 1.0]), np.array([1.0, 1.0]), 1e-6, np.array([1.0, 2.0]), np.array([0.5, 0.5]), np.array([0.0, 4.0]))
+    f0 = O.features(pr, un, 0)
+    # z^0: Ax = (1, 2), s = (.5, .5), b = (0, 3): r_p = (1.5, -0.5), scale 3; Px = (2, 4), q = (1, -1), A'y = (0, 4): r_d = (3, 7), scale 4
+    assert np.allclose(f0["rp_bar"], [0.5, -1.0 / 6.0]) and np.allclose(f0["rd_bar"], [0.75, 1.75])
+    f1 = O.features(pr, un, 1)
+    assert np.allclose(f1["delta_d"], un.ss[1] - un.ss[0]) and np.allclose(f1["delta_p"], un.ss[1] - un.tapes[0].st)
+    assert np.allclose(f1["scal"][2], np.log(np.abs(f1["delta_p"]).max() + 1e-12))
