@@ -470,13 +470,37 @@ def run_fig2(args, cdu, torch, peaks):
                           points=points)))
 
 
+def run_dk(args, cdu, torch):
+    """the micro-benchmark of PAPER.md App. C / Fig. 4 right (L277): wall-clock of the PSD projection and of
+    its Dalecki-Krein backward on 100 matrices of Eq. 13 (gap 1e-5) for n in {10 .. 320}, fp64 (the paper's precision) and fp32."""
+    pts = []
+    for dtype in ("f64", "f32"):
+        tdt = torch.float32 if dtype == "f32" else torch.float64
+        for n in (10, 20, 40, 80, 160, 320):
+            rng = np.random.default_rng(W.generators.BASE_SEED + 1300 + n)
+            S = torch.as_tensor(np.stack([W.clustered_spectrum_matrix(rng, n, 1e-5) for _ in range(100)]), dtype=tdt, device="cuda")
+            A = rng.standard_normal((100, n, n))
+            G = torch.as_tensor(0.5 * (A + A.transpose(0, 2, 1)), dtype=tdt, device="cuda")
+            Pi, U, lam = cdu.cdu_psd_project(S)
+            tf, tb = [], []
+            for _ in range(max(args.steps, 5) + 2):
+                e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+                e[0].record(); Pi, U, lam = cdu.cdu_psd_project(S); e[1].record(); cdu.cdu_psd_vjp(U, lam, G); e[2].record()
+                torch.cuda.synchronize()
+                tf.append(e[0].elapsed_time(e[1])); tb.append(e[1].elapsed_time(e[2]))
+            pts.append(dict(dtype=dtype, n=n, matrices=100, project_ms=float(np.median(tf[2:])), dk_vjp_ms=float(np.median(tb[2:]))))
+    print(json.dumps(dict(metric="dk_microbenchmark_ms_per_100_matrices", unit="ms", data="synthetic (PAPER.md Eq. 13, gap 1e-5)",
+                          higher_is_better=False, config=dict(workload="dk-microbench (PAPER.md App. C, Fig. 4 right)"),
+                          paper_context="Fig. 4: DK ~ autograd ~ Tikhonov, Newton-Schulz ~10x slower; RTX 4090, fp64, curves only", points=pts)))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="all", choices=["all", "fig2"] + sorted(WORKLOADS))
+    ap.add_argument("--workload", default="all", choices=["all", "fig2", "dk"] + sorted(WORKLOADS))
     ap.add_argument("--n", type=int, default=0, help="fig2: one problem size instead of the sweep 1k .. 50k")
     ap.add_argument("--dtype", default=None, help="fig2: f64 (default, the paper's precision) or f32")
     ap.add_argument("--ckpt", default="full", choices=["full", "lean"])
@@ -492,7 +516,7 @@ def main():
     ap.add_argument("--no-batch", type=int, default=0, help="1: lane groups per row instead of warp row batches (debug)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    cfgs = [5, 3, 2] if args.workload in ("all", "fig2") else [WORKLOADS[args.workload]]
+    cfgs = [5, 3, 2] if args.workload in ("all", "fig2", "dk") else [WORKLOADS[args.workload]]
 
     def opts_of(cfg):
         o = dict(cg_refine=args.cg_refine, cg_refine_tol=args.cg_refine_tol)
@@ -516,9 +540,9 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     peaks = load_peaks(cdu)
-    if args.workload == "fig2":
+    if args.workload in ("fig2", "dk"):
         if rank == 0:
-            run_fig2(args, cdu, torch, peaks)
+            run_fig2(args, cdu, torch, peaks) if args.workload == "fig2" else run_dk(args, cdu, torch)
         return
     results = [run_config(c, args, cdu, torch, dist, peaks, world, rank, local, args.ckpt, opts_of(c)) for c in cfgs]
     if rank == 0:

@@ -1220,25 +1220,48 @@ cdu_status psd_op_t(bool vjp, int count, int p, const void* in1, const void* in2
   // projection: in1 = S           -> out1 = PiS, out2 = U, out3 = lam
   // vjp       : in1 = U, in2 = lam, in3 = Gbar -> out1 = Sbar
   if (count < 1 || p < 1 || !in1 || !out1 || (vjp && (!in2 || !in3))) { err = "cdu_psd_*: bad arguments"; return CDU_EINVAL; }
-  DevPool pool;
-  PsdEngine<T> eng;
+  // engine, tables and scratch are kept for the next call of the same shape (the DK micro-benchmark of PAPER.md App. C times
+  // the operator, not cudaMalloc); every call starts cold, so results do not depend on the calls before it
+  struct Ctx { DevPool pool; PsdEngine<T> eng; int count = 0, p = 0, path = 0, tc = 0, dev = -1;
+               double *W, *S1, *Y1, *GW, *part, *Gs; T *Us, *Ls, *d_one; int* flags; };
+  static thread_local Ctx* ctx = nullptr;
+  int dev = 0;
+  CU_OK(cudaGetDevice(&dev));
   const int nsv = p * (p + 1) / 2;
-  std::vector<int> prob(count), row0(count), pv(count, p);
-  for (int i = 0; i < count; ++i) { prob[i] = i; row0[i] = i * nsv; }
-  const bool f32 = std::is_same<T, float>::value;
-  int small_max = f32 ? 128 : 88;
-  if (path == 1) small_max = 1 << 30; else if (path == 2) small_max = 0;
-  cdu_status s = eng.build(pool, prob, row0, pv, small_max, use_tc, st);
-  if (s != CDU_OK) { err = eng.err; return s; }
   const size_t tot = (size_t)count * nsv;
-  double* W = pool.zeros<double>(tot, st); double* S1 = pool.zeros<double>(tot, st); double* Y1 = pool.zeros<double>(tot, st);
-  double* GW = pool.zeros<double>(tot, st); double* part = pool.zeros<double>(2 * (size_t)count, st);
-  double* Gs = pool.zeros<double>(tot, st);
-  T* Us = pool.alloc<T>((size_t)count * p * p); T* Ls = pool.alloc<T>((size_t)count * p);
-  int* flags = pool.zeros<int>(count, st);
-  std::vector<T> one(1, (T)1);
-  T* d_one = pool.upload(one, st);
-  if (pool.last != cudaSuccess || !W || !S1 || !Y1 || !GW || !part || !Gs || !Us || !Ls || !flags || !d_one) { err = "cudaMalloc (psd op)"; return CDU_ENOMEM; }
+  if (!ctx || ctx->count != count || ctx->p != p || ctx->path != path || ctx->tc != use_tc || ctx->dev != dev) {
+    if (ctx) { cudaDeviceSynchronize(); delete ctx; ctx = nullptr; }
+    Ctx* c = new (std::nothrow) Ctx();
+    if (!c) { err = "out of host memory"; return CDU_ENOMEM; }
+    c->count = count; c->p = p; c->path = path; c->tc = use_tc; c->dev = dev;
+    std::vector<int> prob(count), row0(count), pv(count, p);
+    for (int i = 0; i < count; ++i) { prob[i] = i; row0[i] = i * nsv; }
+    const bool f32 = std::is_same<T, float>::value;
+    int small_max = f32 ? 128 : 88;
+    if (path == 1) small_max = 1 << 30; else if (path == 2) small_max = 0;
+    cdu_status s0 = c->eng.build(c->pool, prob, row0, pv, small_max, use_tc, st);
+    if (s0 != CDU_OK) { err = c->eng.err; delete c; return s0; }
+    DevPool& pool = c->pool;
+    c->W = pool.zeros<double>(tot, st); c->S1 = pool.zeros<double>(tot, st); c->Y1 = pool.zeros<double>(tot, st);
+    c->GW = pool.zeros<double>(tot, st); c->part = pool.zeros<double>(2 * (size_t)count, st); c->Gs = pool.zeros<double>(tot, st);
+    c->Us = pool.alloc<T>((size_t)count * p * p); c->Ls = pool.alloc<T>((size_t)count * p);
+    c->flags = pool.zeros<int>(count, st);
+    std::vector<T> one(1, (T)1);
+    c->d_one = pool.upload(one, st);
+    if (pool.last != cudaSuccess || !c->W || !c->S1 || !c->Y1 || !c->GW || !c->part || !c->Gs || !c->Us || !c->Ls || !c->flags || !c->d_one) {
+      err = "cudaMalloc (psd op)"; delete c; return CDU_ENOMEM;
+    }
+    CU_OK(cudaStreamSynchronize(st));
+    ctx = c;
+  }
+  PsdEngine<T>& eng = ctx->eng;
+  eng.warm = false;
+  double *W = ctx->W, *S1 = ctx->S1, *Y1 = ctx->Y1, *GW = ctx->GW, *part = ctx->part, *Gs = ctx->Gs;
+  T *Us = ctx->Us, *Ls = ctx->Ls, *d_one = ctx->d_one;
+  int* flags = ctx->flags;
+  CU_OK(cudaMemsetAsync(W, 0, tot * sizeof(double), st)); CU_OK(cudaMemsetAsync(Y1, 0, tot * sizeof(double), st));
+  CU_OK(cudaMemsetAsync(S1, 0, tot * sizeof(double), st)); CU_OK(cudaMemsetAsync(flags, 0, count * sizeof(int), st));
+  cdu_status s;
   Hyper<T> H; H.rho = d_one; H.alpha = d_one; H.kstride = 0; H.pstride = 0; H.sigma = 1.0;
   if (!vjp) {
     k_dense_to_svec<T><<<count, 256, 0, st>>>(p, (const T*)in1, W);

@@ -72,3 +72,31 @@ def test_repeated_and_zero_eigenvalues(dtype, path):
     assert torch.isfinite(Sb).all()
     assert torch.allclose(Sb[2], Gt[2], atol=tol * 10)             # S > 0: the VJP is the identity
     assert torch.all(Sb[1] == 0)                                   # S = 0: f'(0) := 0 (reading A11)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_dk_vjp_error_does_not_depend_on_the_eigenvalue_gap(dtype):
+    """PAPER.md App. C / Fig. 4 left (L270-277): matrices of Eq. 13 at n = 40, gap delta from 1 down to 1e-10. The GPU's
+    projection and DK VJP (its own eigendecomposition) against the oracle's (LAPACK eigh): the error, relative to the size
+    of the matrix / of the cotangent, stays at rounding level for every delta."""
+    import torch
+    import paper_2606_13825_b200 as cdu
+    import workloads as W
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    rng = np.random.default_rng(40)
+    n, cnt = 40, 4
+    tolp, tolv = (5e-6, 2e-4) if dtype == "f32" else (1e-13, 1e-11)
+    for delta in (1.0, 1e-2, 1e-5, 1e-8, 1e-10):
+        S = np.stack([W.clustered_spectrum_matrix(rng, n, delta) for _ in range(cnt)])
+        G = _sym(rng, cnt, n)
+        if dtype == "f32":
+            S = S.astype(np.float32).astype(np.float64); G = G.astype(np.float32).astype(np.float64)
+        Pi, U, lam = cdu.cdu_psd_project(torch.as_tensor(S, dtype=tdt, device="cuda"))
+        Sb = cdu.cdu_psd_vjp(U, lam, torch.as_tensor(G, dtype=tdt, device="cuda")).double().cpu().numpy()
+        assert np.isfinite(Sb).all()
+        for i in range(cnt):
+            ref = C.smat(C.proj_psd(C.svec(S[i]))[0])
+            assert np.abs(Pi[i].double().cpu().numpy() - ref).max() <= tolp * delta, (delta, i)
+            lam_ref, U_ref = np.linalg.eigh(S[i])
+            vref = C.dk_vjp_matrix(U_ref, lam_ref, G[i])
+            assert np.abs(Sb[i] - vref).max() <= tolv * np.abs(G[i]).max(), (delta, i, np.abs(Sb[i] - vref).max())

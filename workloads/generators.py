@@ -312,6 +312,16 @@ def make_config(cfg: int, batch: Optional[int] = None, K: Optional[int] = None,
                     rho=_round_to(rho, dtype), alpha=_round_to(alpha, dtype), sigma=sigma, x0=x0, s0=s0, y0=y0)
 
 
+def clustered_spectrum_matrix(rng: np.random.Generator, n: int, delta: float) -> np.ndarray:
+    """The sampler of PAPER.md Eq. 13 (App. C): n even, eigenvalues -delta/2 + u_i (first half) and +delta/2 + u_i,
+    u_i ~ U(-sigma, sigma) with sigma = 1e-3 delta, S = Q diag(lambda) Q' for a random orthogonal Q."""
+    sig = 1e-3 * delta
+    lam = np.concatenate([-delta / 2 + rng.uniform(-sig, sig, n // 2), delta / 2 + rng.uniform(-sig, sig, n - n // 2)])
+    Q, _ = np.linalg.qr(rng.standard_normal((n, n)))
+    S = (Q * lam) @ Q.T
+    return 0.5 * (S + S.T)
+
+
 def make_fig2(n: int, batch: int = 1, dtype: str = "f64", seed_offset: int = 0) -> Workload:
     """The linear-solve scaling workload of PAPER.md Fig. 2 / App. B (L96, L247-255): `batch` instances of
     fig2_linear_problem(n) (m = n/2, diag P ~ U(0,10), A 1 % dense N(0,1), b ~ N(0,1)), ONE step (K = 1) with
