@@ -297,3 +297,22 @@ def test_features_hand_case():
     f1 = O.features(pr, un, 1)
     assert np.allclose(f1["delta_d"], un.ss[1] - un.ss[0]) and np.allclose(f1["delta_p"], un.ss[1] - un.tapes[0].st)
     assert np.allclose(f1["scal"][2], np.log(np.abs(f1["delta_p"]).max() + 1e-12))
+
+
+def test_lyapunov_lmi_closed_form():
+    """PAPER.md App. F.2 (L422-428) with A = -a I: A'P + PA = -2aP <= -I and P >= I give P* = max(1, 1/(2a)) I, so the optimal
+    value is n max(1, 1/(2a)). Pins the generator's svec map of P -> A'P + PA together with the oracle's two-PSD-block step."""
+    from workloads import lyapunov_lmi_problem
+    n = 4
+    for a, val in ((0.25, 2.0 * n), (2.0, 1.0 * n)):
+        pr = lyapunov_lmi_problem(np.random.default_rng(0), n=n, A_sys=-a * np.eye(n))
+        x, s, y = O.solve_to_convergence(pr, iters=4000, rho=1.0, alpha=1.6)
+        assert abs(pr.q @ x - val) <= 1e-6 * val
+        Pm = C.smat(x)
+        assert np.allclose(Pm, max(1.0, 1.0 / (2 * a)) * np.eye(n), atol=1e-6)
+    # a generated Hurwitz A: the converged P certifies stability
+    pr = lyapunov_lmi_problem(np.random.default_rng(1), n=4, kind="oscillator")
+    x, s, y = O.solve_to_convergence(pr, iters=20000, rho=1.0, alpha=1.6)
+    rp, rd = O.residuals(pr, x, s, y)
+    assert np.linalg.norm(rp) < 1e-6 and np.linalg.norm(rd) < 1e-6
+    assert np.linalg.eigvalsh(C.smat(x)).min() >= 1.0 - 1e-6

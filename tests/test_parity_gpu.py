@@ -266,6 +266,23 @@ def test_fig2_linear_solve_and_wide_teams():
     PU.assert_within(e, "f32")
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_lyapunov_lmi_two_psd_blocks(dtype):
+    """Minimum-trace Lyapunov LMI (App. F.2): two PSD blocks per problem coupled by a dense
+    svec map, one instance of each generator kind, n = 12 (small-block kernels) and n = 12 through the large-block path."""
+    rng = np.random.default_rng(77)
+    probs = [_round_problem(W.lyapunov_lmi_problem(rng, n=12, kind=k), dtype) for k in ("triangular", "oscillator")]
+    K = 12
+    rd = lambda a: PU.round_to(a, dtype)
+    wl = Workload("lyapunov", dtype, probs, K, rd(W.ar1_rho_schedule(rng, K, 1.0)), rd(np.full(K, 1.6)), 1e-6,
+                  [np.zeros(p.n) for p in probs], [np.zeros(p.m) for p in probs], [np.zeros(p.m) for p in probs])
+    for opts in ({}, dict(psd_small_max=8)):
+        e, st = PU.check(wl, **opts)
+        print(wl.name, dtype, opts, e, st)
+        PU.assert_within(e, dtype)
+        assert st["flags_or"] == 0
+
+
 def test_ragged_large_blocks_two_orders():
     """Two different large orders in one batch (136 and 160): per-block offsets of the large path, FMA GEMMs."""
     a = W.make_config(5, batch=1, p=136, K=5)

@@ -18,6 +18,7 @@ from .generators import (  # noqa: F401
     ar1_rho_schedule,
     make_config,
     make_fig2,
+    lyapunov_lmi_problem,
     clustered_spectrum_matrix,
     pack_batch,
     CONFIG_NAMES,

@@ -312,6 +312,43 @@ def make_config(cfg: int, batch: Optional[int] = None, K: Optional[int] = None,
                     rho=_round_to(rho, dtype), alpha=_round_to(alpha, dtype), sigma=sigma, x0=x0, s0=s0, y0=y0)
 
 
+def lyapunov_lmi_problem(rng: np.random.Generator, n: int = 40, kind: str = "triangular", A_sys: Optional[np.ndarray] = None) -> Problem:
+    """Minimum-trace Lyapunov LMI of PAPER.md App. F.2 (L422-434): min tr(P) s.t. A'P + PA <= -I, P >= I, for a Hurwitz A
+    generated as Q T Q' (T upper triangular, T_ii ~ U(-2,-0.1), N(0,1) above the diagonal; kind "triangular") or Q R Q' (R =
+    blkdiag of damped oscillators [[-z w, w], [-w, -z w]], w ~ U(0.5,5), z ~ U(0.05,0.5); kind "oscillator"; the paper prints
+    +z w in the lower right entry, which is not Hurwitz - read as -z w). Conic form: x = svec(P), q = svec(I),
+    rows [svec(A'PA-map); -I], b = [-svec(I); -svec(I)], two PSD_n cones."""
+    if A_sys is None:
+        Q, _ = np.linalg.qr(rng.standard_normal((n, n)))
+        if kind == "triangular":
+            Tm = np.triu(rng.standard_normal((n, n)), 1) + np.diag(rng.uniform(-2.0, -0.1, n))
+            A_sys = Q @ Tm @ Q.T
+        else:
+            R = np.zeros((n, n))
+            for i in range(n // 2):
+                w, z = rng.uniform(0.5, 5.0), rng.uniform(0.05, 0.5)
+                R[2 * i:2 * i + 2, 2 * i:2 * i + 2] = [[-z * w, w], [-w, -z * w]]
+            if n % 2:
+                R[-1, -1] = -rng.uniform(0.1, 2.0)
+            A_sys = Q @ R @ Q.T
+    d = svec_dim(n)
+    cols = []
+    for j in range(n):
+        for i in range(j + 1):
+            E = np.zeros((n, n))
+            if i == j:
+                E[i, i] = 1.0
+            else:
+                E[i, j] = E[j, i] = 1.0 / np.sqrt(2.0)
+            cols.append(_svec_of_symmetric(A_sys.T @ E + E @ A_sys))
+    L = np.stack(cols, axis=1)
+    L[np.abs(L) < 1e-15] = 0.0
+    eye = _svec_of_symmetric(np.eye(n))
+    A = sp.vstack([sp.csr_matrix(L), -sp.identity(d, format="csr")], format="csr")
+    return Problem(P=sp.csr_matrix((d, d)), q=eye.copy(), A=A, b=np.concatenate([-eye, -eye]), cones=[(PSD, n), (PSD, n)],
+                   name=f"lyapunov-n{n}-{kind}")
+
+
 def clustered_spectrum_matrix(rng: np.random.Generator, n: int, delta: float) -> np.ndarray:
     """The sampler of PAPER.md Eq. 13 (App. C): n even, eigenvalues -delta/2 + u_i (first half) and +delta/2 + u_i,
     u_i ~ U(-sigma, sigma) with sigma = 1e-3 delta, S = Q diag(lambda) Q' for a random orthogonal Q."""
