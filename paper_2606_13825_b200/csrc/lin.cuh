@@ -462,13 +462,13 @@ __device__ int solve_M(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, co
 // xi and x-tilde of one step from z^k = (x, s, y): S1 + S2. Writes xt; st is produced by the caller's A pass.
 template <typename T, typename IT, int MULTI>
 __device__ int lin_solve_step(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const double* x, const double* s,
-                              const double* y, double* xt, int* flag, int* it0) {
+                              const double* y, double* xt, int* flag, int* it0, const double* xstart = nullptr) {
   const int tid = threadIdx.x, nt = blockDim.x;
   for (int i = c.mlo + tid; i < c.mhi; i += nt) c.tm[i] = c.rho * ((double)c.bv[i] - s[i]) - y[i];
   c.team->sync();
   rows_AT<double>(D, c, c.tm, [&](int row, double a) { c.xi[row] = c.sigma * x[row] - (double)c.q[row] + a; });
   c.team->sync();   // tm is reused by solve_M's residual pass
-  return solve_M(D, c, c.xi, x, xt, flag, it0);
+  return solve_M(D, c, c.xi, xstart ? xstart : x, xt, flag, it0);
 }
 
 __device__ __forceinline__ int soc_branch(double t, double nu) { return (nu <= t) ? 0 : ((nu <= -t) ? 1 : 2); }
@@ -478,6 +478,7 @@ struct IterPtrs {
   double* Zk1;        // z^{k+1}
   double* XT;         // x-tilde store (checkpoint slot or scratch), size N
   double* ST;         // s-tilde store, size Mtot
+  const double* XTprev = nullptr;   // x-tilde of the previous step (CG start), NULL: start from x^k
 };
 
 #define CDU_TEAM_PROLOGUE()                                                                   \
@@ -501,7 +502,7 @@ __global__ void __launch_bounds__(1024) k_fwd(BatchDev<T, IT> D, Hyper<T> H, Ite
     double *x1 = I.Zk1 + v0, *s1 = I.Zk1 + D.N + r0, *y1 = I.Zk1 + D.N + D.Mtot + r0;
     double *xt = I.XT + v0, *st = I.ST + r0;
     int flag = 0, it0 = 0;
-    const int iters = lin_solve_step(D, c, x, s, y, xt, &flag, &it0);
+    const int iters = lin_solve_step(D, c, x, s, y, xt, &flag, &it0, I.XTprev ? I.XTprev + v0 : nullptr);
     const double al = c.alpha, rho = c.rho;
     const uint8_t* kind = D.rowkind + r0;
     rows_A<double>(D, c, xt, [&](int row, double a) {

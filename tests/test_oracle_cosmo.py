@@ -316,3 +316,20 @@ def test_lyapunov_lmi_closed_form():
     rp, rd = O.residuals(pr, x, s, y)
     assert np.linalg.norm(rp) < 1e-6 and np.linalg.norm(rd) < 1e-6
     assert np.linalg.eigvalsh(C.smat(x)).min() >= 1.0 - 1e-6
+
+
+def test_robust_mpc_solution_is_a_feasible_trajectory():
+    """PAPER.md App. F.6 (L470-486), N = 6: at the oracle's fixed point the trajectory obeys the double-integrator dynamics
+    from x_init, the tightened boxes, |u| <= 0.5, and the epigraph variables equal the norms they bound (gamma > 0)."""
+    from workloads import robust_mpc_problem
+    N = 6
+    pr = robust_mpc_problem(np.random.default_rng(3), N=N)
+    x, s, y = O.solve_to_convergence(pr, iters=20000, rho=1.0, alpha=1.6)
+    rp, rd = O.residuals(pr, x, s, y)
+    assert np.linalg.norm(rp) < 1e-7 and np.linalg.norm(rd) < 1e-7
+    X = x[:2 * (N + 1)].reshape(N + 1, 2); U = x[2 * (N + 1):2 * (N + 1) + N]; tau = x[2 * (N + 1) + N:-1]
+    Ad = np.array([[1.0, 1.0], [0.0, 1.0]]); Bd = np.array([0.5, 0.1])
+    for t in range(N):
+        assert np.allclose(X[t + 1], Ad @ X[t] + Bd * U[t], atol=1e-7)
+    assert np.all(np.abs(U) <= 0.5 + 1e-7) and np.all(np.abs(X[:, 0]) <= 5 + 1e-7) and np.all(np.abs(X[:, 1]) <= 1 + 1e-7)
+    assert np.allclose(tau, np.abs(U), atol=1e-6) and abs(x[-1] - np.linalg.norm(X[N])) < 1e-6

@@ -283,6 +283,22 @@ def test_lyapunov_lmi_two_psd_blocks(dtype):
         assert st["flags_or"] == 0
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_robust_mpc_socp(dtype):
+    """Robust MPC (App. F.6): zero + nonneg + many small SOC cones, diagonal P, N = 12."""
+    rng = np.random.default_rng(78)
+    probs = [_round_problem(W.robust_mpc_problem(rng, N=12), dtype) for _ in range(3)]
+    K = 15
+    rd = lambda a: PU.round_to(a, dtype)
+    wl = Workload("robust-mpc", dtype, probs, K, rd(W.ar1_rho_schedule(rng, K, 1.0)), rd(np.full(K, 1.6)), 1e-6,
+                  [np.zeros(p.n) for p in probs], [np.zeros(p.m) for p in probs], [np.zeros(p.m) for p in probs])
+    for ckpt in (0, 1):
+        e, st = PU.check(wl, ckpt_mode=ckpt)
+        print(wl.name, dtype, ckpt, e, st)
+        PU.assert_within(e, dtype)
+        assert st["flags_or"] == 0
+
+
 def test_ragged_large_blocks_two_orders():
     """Two different large orders in one batch (136 and 160): per-block offsets of the large path, FMA GEMMs."""
     a = W.make_config(5, batch=1, p=136, K=5)

@@ -19,6 +19,7 @@ from .generators import (  # noqa: F401
     make_config,
     make_fig2,
     lyapunov_lmi_problem,
+    robust_mpc_problem,
     clustered_spectrum_matrix,
     pack_batch,
     CONFIG_NAMES,

@@ -349,6 +349,58 @@ def lyapunov_lmi_problem(rng: np.random.Generator, n: int = 40, kind: str = "tri
                    name=f"lyapunov-n{n}-{kind}")
 
 
+def robust_mpc_problem(rng: np.random.Generator, N: int = 50, kappa: float = 1.0) -> Problem:
+    """Robust MPC SOCP of PAPER.md App. F.6 (L470-486): 1-D double integrator A = [[1,1],[0,1]], B = (0.5, 0.1), Q = Q_N = R = I,
+    box constraints |x_1| <= 5, |x_2| <= 1, |u| <= 0.5 tightened by kappa d_t with Sigma_{t+1} = A Sigma_t A' + sigma^2 I
+    (sigma = 0.01, Sigma_0 = 0), ||u_t|| <= tau_t, ||x_N|| <= tau_term, x_init ~ U(-(1, 0.3), (1, 0.3)), gamma ~ U(0.01, 0.1),
+    gamma_term ~ U(1, 10). kappa is not given in the paper (reading: 1). Variables (x_0..x_N, u_0..u_{N-1}, tau_0..tau_{N-1},
+    tau_term); rows: dynamics and x_0 (ZERO), state and input half-spaces (NONNEG), N cones SOC_2, one SOC_3."""
+    Ad = np.array([[1.0, 1.0], [0.0, 1.0]]); Bd = np.array([0.5, 0.1])
+    Ax = np.array([[1.0, 0.0], [0.0, 1.0], [-1.0, 0.0], [0.0, -1.0]]); bx = np.array([5.0, 1.0, 5.0, 1.0])
+    bu = 0.5
+    x_init = rng.uniform(-1.0, 1.0, 2) * np.array([1.0, 0.3])
+    gam, gam_t = rng.uniform(0.01, 0.1), rng.uniform(1.0, 10.0)
+    nx, nu = 2 * (N + 1), N
+    ix = lambda t: 2 * t
+    iu = lambda t: nx + t
+    it = lambda t: nx + nu + t
+    itt = nx + 2 * nu
+    n = itt + 1
+    Pd = np.zeros(n); Pd[:nx + nu] = 2.0                      # x'Qx + u'Ru = 1/2 z'(2I)z on the x and u entries
+    q = np.zeros(n); q[nx + nu:itt] = gam; q[itt] = gam_t
+    rows, cols, vals, b = [], [], [], []
+
+    def add(entries, rhs):
+        r = len(b)
+        for c, v in entries:
+            rows.append(r); cols.append(c); vals.append(v)
+        b.append(rhs)
+
+    for t in range(N):                                        # x_{t+1} - A x_t - B u_t = 0
+        for i in range(2):
+            add([(ix(t + 1) + i, 1.0)] + [(ix(t) + j, -Ad[i, j]) for j in range(2) if Ad[i, j] != 0.0] + [(iu(t), -Bd[i])], 0.0)
+    for i in range(2):
+        add([(ix(0) + i, 1.0)], x_init[i])
+    n_zero = len(b)
+    Sig = np.zeros((2, 2))
+    for t in range(N + 1):                                    # A_x x_t + s = b_x - kappa d_t
+        d = np.sqrt(np.maximum(np.einsum("ij,jk,ik->i", Ax, Sig, Ax), 0.0))
+        for i in range(4):
+            add([(ix(t) + j, Ax[i, j]) for j in range(2) if Ax[i, j] != 0.0], bx[i] - kappa * d[i])
+        Sig = Ad @ Sig @ Ad.T + 0.01 ** 2 * np.eye(2)
+    for t in range(N):                                        # +-u_t + s = b_u
+        add([(iu(t), 1.0)], bu); add([(iu(t), -1.0)], bu)
+    n_nonneg = len(b) - n_zero
+    for t in range(N):                                        # (tau_t, u_t) in SOC_2
+        add([(it(t), -1.0)], 0.0); add([(iu(t), -1.0)], 0.0)
+    add([(itt, -1.0)], 0.0)                                   # (tau_term, x_N - 0) in SOC_3
+    for i in range(2):
+        add([(ix(N) + i, -1.0)], 0.0)
+    A = sp.csr_matrix((vals, (rows, cols)), shape=(len(b), n))
+    cones = [(ZERO, n_zero), (NONNEG, n_nonneg)] + [(SOC, 2)] * N + [(SOC, 3)]
+    return Problem(P=sp.diags(Pd, format="csr"), q=q, A=A, b=np.array(b), cones=cones, name=f"robust-mpc-N{N}")
+
+
 def clustered_spectrum_matrix(rng: np.random.Generator, n: int, delta: float) -> np.ndarray:
     """The sampler of PAPER.md Eq. 13 (App. C): n even, eigenvalues -delta/2 + u_i (first half) and +delta/2 + u_i,
     u_i ~ U(-sigma, sigma) with sigma = 1e-3 delta, S = Q diag(lambda) Q' for a random orthogonal Q."""
