@@ -48,6 +48,7 @@ def load_peaks(cdu):
     pk["fp32_tflops"] = cdu.cdu_measure_peak(cdu.CDU_PEAK_FP32_FMA)
     pk["fp64_tflops"] = cdu.cdu_measure_peak(cdu.CDU_PEAK_FP64_FMA)
     pk["tf32_tflops"] = cdu.cdu_measure_peak(cdu.CDU_PEAK_TF32_TENSOR)
+    pk["tf32_mma_sync_tflops"] = cdu.cdu_measure_peak(cdu.CDU_PEAK_TF32_MMA_SYNC)
     pk["hbm_copy_gbs_in_process"] = cdu.cdu_measure_peak(cdu.CDU_PEAK_HBM_COPY)
     pk["source"] = "measured"
     return pk
@@ -172,6 +173,7 @@ def cpu_baseline(wl, cfg):
     npb, ks = min(npb, wl.batch), min(ks, wl.K)
     per_pi, total = cpu_oracle_time(wl, npb, ks)
     return dict(value=1.0 / (per_pi * wl.batch), unit=UNIT, cores=blas_threads(), kind="oracle",
+                note="untuned fp64 correctness oracle (dense LU / LAPACK eigh per step): reported, not a target; no speed-up is quoted from it",
                 sample=f"{npb} of {wl.batch} problems x {ks} of {wl.K} unrolled iterations, fwd+bwd, {total:.1f} s; "
                        f"extrapolated x{wl.batch / npb:.0f} problems", host_cores=len(os.sched_getaffinity(0)))
 
@@ -341,7 +343,8 @@ def run_config(cfg, args, cdu, torch, dist, peaks, world, rank, local, ckpt, opt
                 nb, nb0 = nb / 2.0, nb0 / 2.0   # two launches (pre / post) per iteration share the bytes
             ach = nb / dur / 1e9
             tr = traffic_of(kc)
-            r = dict(kernel=kc, bound="hbm", achieved=ach, peak=peaks["hbm_gbs"], unit="GB/s", frac=ach / peaks["hbm_gbs"],
+            r = dict(kernel=kc, bound="hbm", regime=("l2-resident: frac is a model fraction, not an HBM utilisation" if tr and tr < 0.25 * nb else "streams from HBM"),
+                     achieved=ach, peak=peaks["hbm_gbs"], unit="GB/s", frac=ach / peaks["hbm_gbs"],
                      traffic=tr, peak_source=peaks["hbm_source"], frac_of_8TBs=ach / 8000.0,
                      frac_without_refinement_iters=nb0 / dur / 1e9 / peaks["hbm_gbs"],
                      frac_of_8TBs_without_refinement_iters=nb0 / dur / 1e9 / 8000.0,
@@ -369,17 +372,23 @@ def run_config(cfg, args, cdu, torch, dist, peaks, world, rank, local, ckpt, opt
                      peak_source="measured in this process (cdu_measure_peak, tcgen05 kind::tf32 loop)",
                      note="achieved = algorithmic flops (2 p^3 per product); executed = 3 x (3xTF32 split)")
         elif kc == "eig_large":
-            # blocked one-sided Jacobi: Gram + apply products of every block pair, 8 (1 - 16/p) p^3 flops per sweep
+            # blocked one-sided Jacobi: Gram + apply products of every block pair, 8 (1 - 16/p) p^3 flops per sweep. One
+            # eigendecomposition = the first pass plus the (mostly skipped) polish pass: time per decomposition, not per launch
+            ndec = nprof * wl.K * (1 if full else 2)
+            dur = prof[kc]["ms"] * 1e-3 / ndec
             fl = float(np.mean([8.0 * (1.0 - 16.0 / p) * p ** 3 for p in ps])) * st["eig_sweeps_sum"] / wl.K
             f32 = wl.dtype == "f32"
-            pk = peaks["tf32_tflops"] if f32 else peaks["fp64_tflops"]
+            pk = peaks["tf32_mma_sync_tflops"] if f32 else peaks["fp64_tflops"]
             ach = fl / dur / 1e12
-            r = dict(kernel=kc, bound="tensor" if f32 else "alu", achieved=ach, peak=pk, unit="TFLOP/s", frac=ach / pk,
+            r = dict(kernel=kc, bound="tensor" if f32 else "alu", achieved=ach, peak=pk, unit="TFLOP/s", frac=(3.0 if f32 else 1.0) * ach / pk,
                      traffic=traffic_of(kc), executed=(3.0 if f32 else 1.0) * ach,
-                     peak_source="measured in this process (cdu_measure_peak)",
+                     peak_source="measured in this process (cdu_measure_peak: warp-level mma.sync m16n8k8 tf32, the path these products run on)" if f32
+                     else "measured in this process (cdu_measure_peak)",
                      sweeps_per_matrix=st["eig_sweeps_sum"] / max(1, wl.K * len(ps)),
-                     note="Gram + apply products (mma.sync 3xTF32 for fp32) counted as if every block pair rotated; the kernel is "
-                          "bound by the dependent chain of its Jacobi rounds, not by the tensor pipe (DESIGN.md section 7)")
+                     note="achieved = algorithmic flops of the Gram + apply products counted as if every block pair rotated; executed = 3 x "
+                          "(3xTF32); frac = executed / peak. The kernel is bound by the dependent chain of its Jacobi rounds (load, Gram, "
+                          "32x32 sweep, apply, barrier per block round), not by the tensor pipe (DESIGN.md section 7); avg_launch_ms = "
+                          "time per batch of eigendecompositions (first pass + polish pass)")
         else:
             return None
         r["share_of_step"] = share

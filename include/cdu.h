@@ -137,6 +137,18 @@ cdu_status cdu_backward_eq12(cdu_handle h, void* loss, void* g_rho, void* g_sigm
 cdu_status cdu_get_features(cdu_handle h, int32_t k, void* rp_bar, void* rd_bar, void* delta_p, void* delta_d, void* scal,
                             int32_t io_on_host, void* cuda_stream);
 
+/* Vanilla COSMO run to tolerance (the baseline workload of PAPER.md Table 1): iterates in chunks of `check_every`
+ * (<= K_max) steps through the kernels of cdu_forward with a fixed alpha and one rho per problem, starting at rho0. After
+ * every chunk the OSQP-scaled residuals of App. E (L323) are read back - the only host synchronisation - and a problem is
+ * converged when |rp_bar|_inf <= eps and |rd_bar|_inf <= eps. adapt_rho != 0: residual balancing (L349), rho <- rho
+ * sqrt(|rp_bar|_inf / |rd_bar|_inf) clipped to [1e-6, 1e6] when the two differ by more than 5x (one scalar per problem:
+ * per-row rho with the x1e3 equality scaling is not implemented). x0, s0, y0 (NULL = zeros) and x, s, y (may be NULL) as in
+ * cdu_forward; iters_out [batch] (HOST): iterations at the first check that found the problem converged, or -(iterations
+ * done) if it did not converge within max_iter; res_out [batch][2] (HOST): the last scaled residuals. */
+cdu_status cdu_solve(cdu_handle h, int32_t max_iter, int32_t check_every, double eps, double rho0, double alpha, double sigma,
+                     int32_t adapt_rho, const void* x0, const void* s0, const void* y0, void* x, void* s, void* y,
+                     int32_t* iters_out, double* res_out, int32_t io_on_host, void* cuda_stream);
+
 typedef struct {
   int64_t cg_iters_fwd;      /* CG iterations summed over problems and iterations, last forward            */
   int64_t cg_iters_bwd;      /* same for the adjoint solves (and LEAN re-solves) of the last backward       */
@@ -189,8 +201,10 @@ cdu_status cdu_psd_vjp(int32_t dtype, int32_t count, int32_t p, const void* U, c
  *   CDU_PEAK_FP32_FMA / CDU_PEAK_FP64_FMA : dependent-chain-free FMA loops on the plain ALUs, TFLOP/s;
  *   CDU_PEAK_TF32_TENSOR : back-to-back tcgen05.mma kind::tf32 (M128 N256 K8) from shared-memory operands, dense
  *                          TFLOP/s of the tensor pipe (1 x TF32; the 3xTF32 products execute three of these per flop);
- *   CDU_PEAK_HBM_COPY    : device-to-device copy of 1 GiB, GB/s (read + write). */
-typedef enum { CDU_PEAK_FP32_FMA = 0, CDU_PEAK_FP64_FMA = 1, CDU_PEAK_TF32_TENSOR = 2, CDU_PEAK_HBM_COPY = 3 } cdu_peak_kind;
+ *   CDU_PEAK_HBM_COPY    : device-to-device copy of 1 GiB, GB/s (read + write);
+ *   CDU_PEAK_TF32_MMA_SYNC : back-to-back warp-level mma.sync m16n8k8 tf32 (the blocked Jacobi's Gram / apply path), TFLOP/s. */
+typedef enum { CDU_PEAK_FP32_FMA = 0, CDU_PEAK_FP64_FMA = 1, CDU_PEAK_TF32_TENSOR = 2, CDU_PEAK_HBM_COPY = 3,
+               CDU_PEAK_TF32_MMA_SYNC = 4 } cdu_peak_kind;
 cdu_status cdu_measure_peak(int32_t kind, double* value, void* cuda_stream);
 
 #ifdef __cplusplus

@@ -28,7 +28,7 @@ _STATUS = {0: "CDU_OK", 1: "CDU_EINVAL", 2: "CDU_ENOMEM", 3: "CDU_ECUDA", 4: "CD
 
 EXPORTED_SYMBOLS = ("cdu_create", "cdu_forward", "cdu_backward", "cdu_get_stats", "cdu_get_iterate", "cdu_last_error",
                     "cdu_destroy", "cdu_version", "cdu_psd_project", "cdu_psd_vjp", "cdu_profile", "cdu_get_profile",
-                    "cdu_measure_peak", "cdu_backward_inject", "cdu_backward_eq12", "cdu_get_features")
+                    "cdu_measure_peak", "cdu_backward_inject", "cdu_backward_eq12", "cdu_get_features", "cdu_solve")
 
 
 class CduError(RuntimeError):
@@ -87,6 +87,8 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.cdu_backward_eq12.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, vp]
     lib.cdu_get_features.restype = i32
     lib.cdu_get_features.argtypes = [vp, i32, vp, vp, vp, vp, vp, i32, vp]
+    lib.cdu_solve.restype = i32
+    lib.cdu_solve.argtypes = [vp, i32, i32, f64, f64, f64, f64, i32, vp, vp, vp, vp, vp, vp, vp, vp, i32, vp]
     lib.cdu_get_stats.restype = i32
     lib.cdu_get_stats.argtypes = [vp, C.POINTER(_Stats)]
     lib.cdu_get_iterate.restype = i32
@@ -171,10 +173,27 @@ class Handle:
         if st != CDU_OK:
             raise CduError(st, self.lib.cdu_last_error(self.h).decode())
 
+    def _want(self, name, t, numel, host):
+        """Marshalling check: the C ABI takes bare pointers, so a wrong dtype or a short array would be read out of bounds."""
+        if t is None:
+            return
+        n = t.size if isinstance(t, np.ndarray) else t.numel()
+        dt = str(t.dtype).replace("torch.", "")
+        want = "float32" if self.dtype == "f32" else "float64"
+        if dt != want:
+            raise ValueError(f"{name}: dtype {dt}, the handle computes in {want}")
+        if n != numel:
+            raise ValueError(f"{name}: {n} elements, expected {numel}")
+        if not isinstance(t, np.ndarray) and t.is_cuda == bool(host):
+            raise ValueError(f"{name}: {'host' if host else 'device'} tensor expected (host={host})")
+
     def forward(self, K, rho, alpha, sigma, x0=None, s0=None, y0=None, rho_mode=CDU_RHO_PER_ITER, out=None, host=False):
         """cdu_forward. Device mode: torch CUDA tensors in, returns (xK, sK, yK) CUDA tensors.
         Host mode: pinned torch CPU tensors / numpy arrays in and out (copies are inside the call)."""
         torch = _torch()
+        cnt = K * (self.B if rho_mode == CDU_RHO_PER_PROBLEM else 1)
+        for nm, t, n in (("rho", rho, cnt), ("alpha", alpha, cnt), ("x0", x0, self.N), ("s0", s0, self.M), ("y0", y0, self.M)):
+            self._want(nm, t, n, host)
         if out is None:
             if host:
                 out = tuple(torch.empty(n, dtype=self.torch_dtype).pin_memory() for n in (self.N, self.M, self.M))
@@ -196,6 +215,8 @@ class Handle:
                 out = {k: torch.empty(n, dtype=self.torch_dtype).pin_memory() for k, n in sizes.items()}
             else:
                 out = {k: torch.empty(n, dtype=self.torch_dtype, device="cuda") for k, n in sizes.items()}
+        for nm, t, n in (("g_xK", g_xK, self.N), ("g_sK", g_sK, self.M), ("g_yK", g_yK, self.M)):
+            self._want(nm, t, n, host)
         self._check(self.lib.cdu_backward(self.h, _ptr(g_xK), _ptr(g_sK), _ptr(g_yK), _ptr(out.get("g_rho")),
                                           _ptr(out.get("g_sigma")), _ptr(out.get("g_alpha")), _ptr(out.get("g_x0")),
                                           _ptr(out.get("g_s0")), _ptr(out.get("g_y0")), 1 if host else 0, _stream()))
@@ -236,6 +257,17 @@ class Handle:
                                               _ptr(o["scal"]), 0, _stream()))
         o["scal"] = o["scal"].view(self.B, 3)
         return o
+
+    def solve(self, max_iter, check_every, eps, rho0=0.1, alpha=1.6, sigma=1e-6, adapt_rho=True, x0=None, s0=None, y0=None):
+        """cdu_solve (device pointers) -> (x, s, y, iters [B] numpy int32, res [B, 2] numpy)."""
+        torch = _torch()
+        out = tuple(torch.empty(n, dtype=self.torch_dtype, device="cuda") for n in (self.N, self.M, self.M))
+        iters = np.zeros(self.B, np.int32); res = np.zeros((self.B, 2), np.float64)
+        self._check(self.lib.cdu_solve(self.h, int(max_iter), int(check_every), float(eps), float(rho0), float(alpha), float(sigma),
+                                       1 if adapt_rho else 0, _ptr(x0), _ptr(s0), _ptr(y0), _ptr(out[0]), _ptr(out[1]), _ptr(out[2]),
+                                       iters.ctypes.data, res.ctypes.data, 0, _stream()))
+        self.K, self.rho_mode = int(check_every), CDU_RHO_PER_PROBLEM
+        return out[0], out[1], out[2], iters, res
 
     def iterate(self, k: int):
         torch = _torch()
@@ -297,7 +329,7 @@ def cdu_destroy(h: Handle) -> None:
     h.close()
 
 
-CDU_PEAK_FP32_FMA, CDU_PEAK_FP64_FMA, CDU_PEAK_TF32_TENSOR, CDU_PEAK_HBM_COPY = range(4)
+CDU_PEAK_FP32_FMA, CDU_PEAK_FP64_FMA, CDU_PEAK_TF32_TENSOR, CDU_PEAK_HBM_COPY, CDU_PEAK_TF32_MMA_SYNC = range(5)
 
 
 def cdu_measure_peak(kind: int) -> float:

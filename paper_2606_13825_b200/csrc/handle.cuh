@@ -535,6 +535,9 @@ struct HandleT : cdu_handle_s {
                       void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st, const Extra* ex) override;
   cdu_status features(int k, void* rp_bar, void* rd_bar, void* delta_p, void* delta_d, void* scal, int host, cudaStream_t st) override;
   cdu_status add_extra(int k, double* Gz, const Extra* ex, int host, cudaStream_t st);
+  cdu_status solve(int max_iter, int check_every, double eps, double rho0, double alpha, double sigma, int adapt_rho, const void* x0,
+                   const void* s0, const void* y0, void* x, void* s, void* y, int* iters_out, double* res_out, int host, cudaStream_t st) override;
+  bool continue_from_last = false;
   cdu_status stats(cdu_stats* out) override;
   cdu_status iterate(int k, void* x, void* s, void* y, int host, cudaStream_t st) override;
   void profile_enable(int on) override { prof.on = on != 0; }
@@ -946,9 +949,15 @@ cdu_status HandleT<T, IT>::forward(int K, const void* rho, int mode, double sigm
     ++launches;
     CU_OK(cudaGetLastError());
   }
+  const int K_prev = K_last;
   K_last = 0; mode_last = mode; sigma_last = sigma; last_stream = st;
-  cdu_status s = import_state(z_at(0), x0, s0, y0, host, st);
-  if (s != CDU_OK) return s;
+  cdu_status s = CDU_OK;
+  if (continue_from_last) {     // cdu_solve: the next chunk starts at the fp64 iterate the last one ended on (z^0 is in place for the first)
+    if (K_prev >= 1) CU_OK(cudaMemcpyAsync(z_at(0), z_at(K_prev), zstride * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  } else {
+    s = import_state(z_at(0), x0, s0, y0, host, st);
+    if (s != CDU_OK) return s;
+  }
   CU_OK(cudaMemsetAsync(cg_f, 0, B * sizeof(int), st));
   CU_OK(cudaMemsetAsync(cg_f0, 0, B * sizeof(int), st));
   CU_OK(cudaMemsetAsync(cg_max, 0, B * sizeof(int), st));
@@ -1012,6 +1021,59 @@ cdu_status HandleT<T, IT>::add_extra(int k, double* Gz, const Extra* ex, int hos
     launches += 2;
     CU_OK(cudaGetLastError());
   }
+  return CDU_OK;
+}
+
+// Vanilla COSMO to tolerance (the baseline of PAPER.md Table 1; L349: residual-balancing rho): chunks of `check_every`
+// iterations through the same kernels as cdu_forward; after every chunk the OSQP-scaled residuals of App. E (L323) are read
+// back (the only host sync) and, per problem, rho <- rho sqrt(|rp_bar|_inf / |rd_bar|_inf) when the two differ by more than 5x.
+template <typename T, typename IT>
+cdu_status HandleT<T, IT>::solve(int max_iter, int check_every, double eps, double rho0, double alpha, double sigma, int adapt_rho,
+                                 const void* x0, const void* s0, const void* y0, void* x, void* s, void* y, int* iters_out,
+                                 double* res_out, int host, cudaStream_t st) {
+  if (check_every < 1 || check_every > K_max || max_iter < 1 || !(eps > 0.0) || !(rho0 > 0.0) || !(alpha > 0.0 && alpha < 2.0)) {
+    err = "cdu_solve: bad arguments (1 <= check_every <= K_max, max_iter >= 1, eps > 0, rho0 > 0, alpha in (0,2))"; return CDU_EINVAL;
+  }
+  const int Kc = check_every;
+  std::vector<T> hr((size_t)Kc * B), ha((size_t)Kc * B, (T)alpha), sc((size_t)B * 3);
+  std::vector<double> rho(B, rho0);
+  std::vector<int> done(B, -1);
+  T *d_r = nullptr, *d_a = nullptr;
+  CU_OK(cudaMalloc(&d_r, hr.size() * sizeof(T))); CU_OK(cudaMalloc(&d_a, ha.size() * sizeof(T)));
+  CU_OK(cudaMemcpyAsync(d_a, ha.data(), ha.size() * sizeof(T), cudaMemcpyHostToDevice, st));
+  cdu_status r = import_state(z_at(0), x0, s0, y0, host, st);
+  if (r != CDU_OK) { cudaFree(d_r); cudaFree(d_a); return r; }
+  K_last = 0;
+  int it = 0;
+  continue_from_last = true;
+  while (it < max_iter) {
+    for (int k = 0; k < Kc; ++k) for (int b = 0; b < B; ++b) hr[(size_t)k * B + b] = (T)rho[b];
+    CU_OK(cudaMemcpyAsync(d_r, hr.data(), hr.size() * sizeof(T), cudaMemcpyHostToDevice, st));
+    r = forward(Kc, d_r, CDU_RHO_PER_PROBLEM, sigma, d_a, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, st);
+    if (r != CDU_OK) break;
+    it += Kc;
+    r = features(Kc, nullptr, nullptr, nullptr, nullptr, sc.data(), 1, st);     // host read-back of [B][3] (synchronises)
+    if (r != CDU_OK) break;
+    bool all = true;
+    for (int b = 0; b < B; ++b) {
+      const double rp = std::exp((double)sc[(size_t)b * 3]) - 1e-12, rd = std::exp((double)sc[(size_t)b * 3 + 1]) - 1e-12;
+      if (res_out) { res_out[2 * b] = rp; res_out[2 * b + 1] = rd; }
+      if (done[b] < 0 && rp <= eps && rd <= eps) done[b] = it;
+      if (done[b] < 0) {
+        all = false;
+        if (adapt_rho && rp > 0.0 && rd > 0.0 && (rp > 5.0 * rd || rd > 5.0 * rp))
+          rho[b] = std::min(1e6, std::max(1e-6, rho[b] * std::sqrt(rp / rd)));
+      }
+    }
+    if (all) break;
+  }
+  continue_from_last = false;
+  cudaFree(d_r); cudaFree(d_a);
+  if (r != CDU_OK) return r;
+  for (int b = 0; b < B; ++b) if (iters_out) iters_out[b] = done[b] < 0 ? -it : done[b];     // negative: not converged after |.| iterations
+  r = export_state(z_at(K_last), x, s, y, host, st);
+  if (r != CDU_OK) return r;
+  if (host) CU_OK(cudaStreamSynchronize(st));
   return CDU_OK;
 }
 

@@ -28,6 +28,22 @@ static __global__ void __launch_bounds__(1024) k_fma_peak(int iters, T* sink) {
   if (s == (T)-1.2345) sink[0] = s;   // never true: keeps the chains alive
 }
 
+// warp-level mma.sync m16n8k8 tf32 (the path of the blocked Jacobi's Gram / apply products): 8 independent accumulators
+static __global__ void __launch_bounds__(512) k_mma_sync_peak(int iters, float* sink) {
+  float acc[8][4] = {};
+  const uint32_t a = 0x3f800000u + threadIdx.x, b = 0x3f000000u + threadIdx.x;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int j = 0; j < 8; ++j)
+      asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                   : "+f"(acc[j][0]), "+f"(acc[j][1]), "+f"(acc[j][2]), "+f"(acc[j][3]) : "r"(a), "r"(b), "r"(a), "r"(b), "r"(b), "r"(a));
+  }
+  float s = 0.f;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) s += acc[j][0] + acc[j][1] + acc[j][2] + acc[j][3];
+  if (s == -1.2345f) sink[0] = s;
+}
+
 constexpr int TF32_N = 256;
 static __global__ void __launch_bounds__(128, 1) k_tf32_peak(int iters, float* sink) {
   extern __shared__ unsigned char smem_dyn[];
@@ -119,6 +135,10 @@ inline cdu_status measure(int kind, double* value, cudaStream_t st) {
     if (cudaFuncSetAttribute(k_tf32_peak, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) { cudaFree(sink); return CDU_ECUDA; }
     t = time_best([&] { k_tf32_peak<<<nsm, 128, smem, st>>>(iters, sink); }, 5, st);
     work = 2.0 * 128.0 * TF32_N * 32.0 * iters * nsm / 1e12;
+  } else if (kind == CDU_PEAK_TF32_MMA_SYNC) {
+    const int iters = 4096, grid = nsm;
+    t = time_best([&] { k_mma_sync_peak<<<grid, 512, 0, st>>>(iters, sink); }, 5, st);
+    work = 2.0 * 16.0 * 8.0 * 8.0 * 8.0 * iters * 16.0 * grid / 1e12;      // 8 mma of 16x8x8 per warp and iteration, 16 warps
   } else if (kind == CDU_PEAK_HBM_COPY) {
     const size_t n = (size_t)1 << 26;   // 2 x 1 GiB
     float4 *a = nullptr, *b = nullptr;

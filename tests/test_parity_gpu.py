@@ -365,29 +365,43 @@ def test_cfg3_full_size_worst_conditioned_problem():
     assert st["flags_or"] == 0
 
 
-def test_full_size_cfg5_all_instances():
-    """All 8 instances of cfg5 against the oracle (FULL checkpoints, the configuration bench.py's headline times).
-    Iterates: every instance inside 1e-4. Gradients: the fp32 iterates are accurate to ~3e-5 of ||w||, while every
-    instance meets eigenvalues of w within 1e-5 ||w|| of zero somewhere along its K = 200 steps (oracle conditioning log,
-    DESIGN.md section 6): which side of zero such an eigenvalue falls on is decided by fp32 rounding, and a different side
-    is a different branch of the piecewise-smooth projection. At most one instance may leave the 1e-3 bound for that
+def _check_cfg5_instances(wl, ref, res, max_off):
+    """Iterates: every compared instance inside 1e-4. Gradients: the fp32 iterates are accurate to ~3e-5 of ||w||, while every
+    cfg5 instance meets eigenvalues of w within 1e-5 ||w|| of zero somewhere along its K = 200 steps (oracle conditioning log,
+    DESIGN.md section 6): which side of zero such an eigenvalue falls on is decided by fp32 rounding, and a different side is a
+    different branch of the piecewise-smooth projection. At most `max_off` instances may leave the 1e-3 bound for that
     reason; test_full_size_cfg5_fp64_instance shows the same code inside 1e-7 in fp64."""
+    errs = PU.compare_each(wl, ref, res)
+    grad_keys = ("g_x0", "g_s0", "g_y0", "g_rho", "g_alpha")
+    off = []
+    for b, e in zip(ref["idx"], errs):
+        print(wl.name, "instance", b, {k: float("%.2g" % v) for k, v in e.items()})
+        for k in ("x", "s", "y"):
+            assert e[k] <= PU.TOL["f32"]["iter"], (b, k, e[k])
+        if max(e[k] for k in grad_keys) > PU.TOL["f32"]["grad"]:
+            off.append(b)
+    assert len(off) <= max_off, f"instances outside the gradient tolerance: {off}"
+    if not off:
+        assert PU.compare(wl, ref, res, True)["g_sigma"] <= PU.TOL["f32"]["grad"]
+    assert res["stats"]["flags_or"] == 0
+
+
+def test_full_size_cfg5_all_instances():
+    """All 8 instances of cfg5 against the oracle (FULL checkpoints, the configuration bench.py's headline times)."""
     wl = W.make_config(5)
     ref = PU.oracle_reference(wl, list(range(wl.batch)))
     res = PU.gpu_run(wl, PU.full_cotangent(wl, ref), per_problem=True)
     PU.assert_batch_sane(wl, res, 1e-4)
-    errs = PU.compare_each(wl, ref, res)
-    grad_keys = ("g_x0", "g_s0", "g_y0", "g_rho", "g_alpha", "g_sigma")
-    off = []
-    for b, e in enumerate(errs):
-        print(wl.name, "instance", b, {k: float("%.2g" % v) for k, v in e.items()})
-        for k in ("x", "s", "y"):
-            assert e[k] <= PU.TOL["f32"]["iter"], (b, k, e[k])
-        if max(e[k] for k in grad_keys if k != "g_sigma") > PU.TOL["f32"]["grad"]:
-            off.append(b)
-    assert PU.compare(wl, ref, res, True)["g_sigma"] <= PU.TOL["f32"]["grad"]
-    assert len(off) <= 1, f"instances outside the gradient tolerance: {off}"
-    assert res["stats"]["flags_or"] == 0
+    _check_cfg5_instances(wl, ref, res, max_off=1)
+
+
+def test_full_size_cfg5_lean():
+    """LEAN checkpoints at full size: two sampled instances against the oracle, random cotangents on the other six."""
+    wl = W.make_config(5)
+    ref = PU.oracle_reference(wl, [3, 6])
+    res = PU.gpu_run(wl, PU.full_cotangent(wl, ref, 5), ckpt_mode=1, per_problem=True)
+    PU.assert_batch_sane(wl, res, 1e-4)
+    _check_cfg5_instances(wl, ref, res, max_off=1)
 
 
 def test_full_size_cfg5_fp64_instance():
@@ -398,14 +412,6 @@ def test_full_size_cfg5_fp64_instance():
     e, st = PU.check(wl)
     print(wl.name, e, st)
     PU.assert_within(e, "f64")
-    assert st["flags_or"] == 0
-
-
-def test_full_size_cfg5_lean():
-    wl = W.make_config(5)
-    e, st = PU.check(wl, problems=[3, 6], per_problem=True, ckpt_mode=1, fill_seed=5, sane_tol=1e-4)
-    print(wl.name, e, st)
-    PU.assert_within(e, wl.dtype)
     assert st["flags_or"] == 0
 
 
