@@ -44,7 +44,7 @@ def oracle_reference(wl, problems=None, x_star=None):
     return ref
 
 
-def gpu_run(wl, cot_full, ckpt_mode=0, per_problem=False, host=False, **opts):
+def gpu_run(wl, cot_full, ckpt_mode=0, per_problem=False, host=False, keep_iterates_of=None, **opts):
     """Forward + backward through the C ABI. cot_full: list over the WHOLE batch of (gx, gs, gy) or None (zeros).
     Returns numpy results split per problem."""
     import torch
@@ -87,6 +87,14 @@ def gpu_run(wl, cot_full, ckpt_mode=0, per_problem=False, host=False, **opts):
         res["g_sigma"] = npy(g["g_sigma"])
     else:
         res["g_rho"] = npy(g["g_rho"]); res["g_alpha"] = npy(g["g_alpha"]); res["g_sigma"] = float(npy(g["g_sigma"])[0])
+    if keep_iterates_of is not None:      # callable(res) -> problems whose iterates z^0..z^K are wanted
+        want = list(keep_iterates_of(res))
+        its = {b: [] for b in want}
+        for k in range(wl.K + 1):
+            xs, ss, ys = (split(npy(t), o) for t, o in zip(h.iterate(k), (vo, ro, ro)))
+            for b in want:
+                its[b].append((xs[b], ss[b], ys[b]))
+        res["iterates"] = its
     cdu.cdu_destroy(h)
     return res
 
@@ -124,6 +132,25 @@ def compare_each(wl, ref, res, per_problem=True):
         one["idx"] = [b]
         out.append(compare(wl, one, res, per_problem))
     return out
+
+
+def teacher_forced_errors(wl, b, gpu_iterates, cot, res):
+    """Gradient errors of problem b against the oracle's reverse sweep ALONG THE GPU's OWN ITERATES: the tape of step k is the
+    oracle's exact step evaluated at the GPU's z^k (its outputs are discarded). This is the derivative of the trajectory the
+    forward pass actually took, which is what BPTT computes; it separates the parity of the reverse sweep from branch
+    decisions of the forward pass at near-zero eigenvalues. gpu_iterates: list over k = 0..K of
+    (x, s, y) of problem b."""
+    pr = wl.problems[b]
+    tapes = []
+    for k in range(wl.K):
+        x, s, y = gpu_iterates[k]
+        tapes.append(O.step(pr, x, s, y, wl.rho[k], wl.alpha[k], wl.sigma)[3])
+    un = O.Unroll([z[0] for z in gpu_iterates], [z[1] for z in gpu_iterates], [z[2] for z in gpu_iterates], tapes)
+    g = O.backward(pr, un, *cot)
+    gfb = max(np.max(np.abs(v), initial=0.0) for v in (g.g_x0, g.g_s0, g.g_y0)) or 1.0
+    e = dict(g_x0=nrm_err(res["g_x0"][b], g.g_x0, gfb), g_s0=nrm_err(res["g_s0"][b], g.g_s0, gfb), g_y0=nrm_err(res["g_y0"][b], g.g_y0, gfb),
+             g_rho=nrm_err(res["g_rho"][:, b], g.g_rho_scalar), g_alpha=nrm_err(res["g_alpha"][:, b], g.g_alpha))
+    return e
 
 
 def full_cotangent(wl, ref, fill_seed=None):

@@ -365,22 +365,36 @@ def test_cfg3_full_size_worst_conditioned_problem():
     assert st["flags_or"] == 0
 
 
-def _check_cfg5_instances(wl, ref, res, max_off):
-    """Iterates: every compared instance inside 1e-4. Gradients: the fp32 iterates are accurate to ~3e-5 of ||w||, while every
-    cfg5 instance meets eigenvalues of w within 1e-5 ||w|| of zero somewhere along its K = 200 steps (oracle conditioning log,
-    DESIGN.md section 6): which side of zero such an eigenvalue falls on is decided by fp32 rounding, and a different side is a
-    different branch of the piecewise-smooth projection. At most `max_off` instances may leave the 1e-3 bound for that
-    reason; test_full_size_cfg5_fp64_instance shows the same code inside 1e-7 in fp64."""
+GRAD_KEYS = ("g_x0", "g_s0", "g_y0", "g_rho", "g_alpha")
+
+
+def _off_instances(wl, ref, res):
     errs = PU.compare_each(wl, ref, res)
-    grad_keys = ("g_x0", "g_s0", "g_y0", "g_rho", "g_alpha")
+    return [b for b, e in zip(ref["idx"], errs) if max(e[k] for k in GRAD_KEYS) > PU.TOL["f32"]["grad"]]
+
+
+def _check_cfg5_instances(wl, ref, res, max_off):
+    """Iterates: every compared instance inside 1e-4 of the oracle. Gradients: inside 1e-3 of the oracle, except that an instance
+    may leave that bound when its forward pass took another branch of the projection than the oracle's: every cfg5 instance
+    meets eigenvalues of w within 1e-5 ||w|| of zero somewhere along its K = 200 steps, the fp32 iterates are accurate to ~4e-5
+    ||w||, so the side of zero such an eigenvalue falls on is decided by rounding, and the derivative of the projection is
+    discontinuous there (f'(lambda) = 1 iff lambda > 0). For such an instance (at most `max_off`) the reverse sweep is compared
+    with the oracle's reverse sweep along the GPU's OWN iterates instead (PU.teacher_forced_errors) - the derivative of the
+    trajectory that was actually computed - and must be inside 1e-3 there. DESIGN.md section 6 has the measurements."""
+    errs = PU.compare_each(wl, ref, res)
     off = []
     for b, e in zip(ref["idx"], errs):
         print(wl.name, "instance", b, {k: float("%.2g" % v) for k, v in e.items()})
         for k in ("x", "s", "y"):
             assert e[k] <= PU.TOL["f32"]["iter"], (b, k, e[k])
-        if max(e[k] for k in grad_keys) > PU.TOL["f32"]["grad"]:
+        if max(e[k] for k in GRAD_KEYS) > PU.TOL["f32"]["grad"]:
             off.append(b)
     assert len(off) <= max_off, f"instances outside the gradient tolerance: {off}"
+    for b in off:
+        cot = ref["cot"][ref["idx"].index(b)]
+        e = PU.teacher_forced_errors(wl, b, res["iterates"][b], cot, res)
+        print(wl.name, "instance", b, "along the GPU's own iterates:", {k: float("%.2g" % v) for k, v in e.items()})
+        assert max(e.values()) <= PU.TOL["f32"]["grad"], (b, e)
     if not off:
         assert PU.compare(wl, ref, res, True)["g_sigma"] <= PU.TOL["f32"]["grad"]
     assert res["stats"]["flags_or"] == 0
@@ -390,18 +404,18 @@ def test_full_size_cfg5_all_instances():
     """All 8 instances of cfg5 against the oracle (FULL checkpoints, the configuration bench.py's headline times)."""
     wl = W.make_config(5)
     ref = PU.oracle_reference(wl, list(range(wl.batch)))
-    res = PU.gpu_run(wl, PU.full_cotangent(wl, ref), per_problem=True)
+    res = PU.gpu_run(wl, PU.full_cotangent(wl, ref), per_problem=True, keep_iterates_of=lambda r: _off_instances(wl, ref, r))
     PU.assert_batch_sane(wl, res, 1e-4)
-    _check_cfg5_instances(wl, ref, res, max_off=1)
+    _check_cfg5_instances(wl, ref, res, max_off=3)
 
 
 def test_full_size_cfg5_lean():
     """LEAN checkpoints at full size: two sampled instances against the oracle, random cotangents on the other six."""
     wl = W.make_config(5)
     ref = PU.oracle_reference(wl, [3, 6])
-    res = PU.gpu_run(wl, PU.full_cotangent(wl, ref, 5), ckpt_mode=1, per_problem=True)
+    res = PU.gpu_run(wl, PU.full_cotangent(wl, ref, 5), ckpt_mode=1, per_problem=True, keep_iterates_of=lambda r: _off_instances(wl, ref, r))
     PU.assert_batch_sane(wl, res, 1e-4)
-    _check_cfg5_instances(wl, ref, res, max_off=1)
+    _check_cfg5_instances(wl, ref, res, max_off=2)
 
 
 def test_full_size_cfg5_fp64_instance():
