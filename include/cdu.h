@@ -37,7 +37,11 @@ typedef enum { CDU_OK = 0, CDU_EINVAL = 1, CDU_ENOMEM = 2, CDU_ECUDA = 3, CDU_ES
 typedef enum { CDU_F32 = 0, CDU_F64 = 1 } cdu_dtype;
 typedef enum { CDU_ZERO = 0, CDU_NONNEG = 1, CDU_SOC = 2, CDU_PSD = 3 } cdu_cone_kind;
 typedef enum { CDU_RHO_PER_ITER = 0,    /* rho[K], alpha[K] shared by the batch; g_rho[K], g_alpha[K], g_sigma[1] are batch sums */
-               CDU_RHO_PER_PROBLEM = 1  /* rho[K][B], alpha[K][B]; g_rho[K][B], g_alpha[K][B], g_sigma[B] */
+               CDU_RHO_PER_PROBLEM = 1, /* rho[K][B], alpha[K][B]; g_rho[K][B], g_alpha[K][B], g_sigma[B] */
+               CDU_RHO_PER_ROW = 2      /* rho[K][sum m_b] (D = diag(rho) in M = P + sigma I + A'DA, L78; Eq. 6 L90 row by row),
+                                           alpha[K][B]; g_rho[K][sum m_b], g_alpha[K][B], g_sigma[B]. rho must be constant
+                                           inside every SOC / PSD block (the projection of Eq. 3d couples their rows, L343):
+                                           cdu_rectify_rho averages a per-row prediction over each block */
 } cdu_rho_mode;
 typedef enum { CDU_CKPT_FULL = 0, /* store z^k plus x-tilde, s-tilde and (U, lambda) of every PSD block            */
                CDU_CKPT_LEAN = 1  /* store z^k only ((n+2m) doubles per iteration); backward re-solves and re-factors */
@@ -136,6 +140,10 @@ cdu_status cdu_backward_eq12(cdu_handle h, void* loss, void* g_rho, void* g_sigm
  *   scal [batch][3]   = log(|rp_bar|_inf + 1e-12), log(|rd_bar|_inf + 1e-12), log(|delta_p|_inf + 1e-12) */
 cdu_status cdu_get_features(cdu_handle h, int32_t k, void* rp_bar, void* rd_bar, void* delta_p, void* delta_d, void* scal,
                             int32_t io_on_host, void* cuda_stream);
+
+/* Rectification of PAPER.md App. E (L343), in place on rho [K][sum m_b] (or on a g_rho of that layout: the operation is its
+ * own adjoint): every SOC / PSD block gets the mean of its rows; zero / nonneg rows are left as they are. */
+cdu_status cdu_rectify_rho(cdu_handle h, int32_t K, void* rho, int32_t io_on_host, void* cuda_stream);
 
 /* Vanilla COSMO run to tolerance (the baseline workload of PAPER.md Table 1): iterates in chunks of `check_every`
  * (<= K_max) steps through the kernels of cdu_forward with a fixed alpha and one rho per problem, starting at rho0. After

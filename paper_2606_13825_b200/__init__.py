@@ -22,13 +22,13 @@ LIB_PATH = os.path.join(_PKG, "libcdu.so")
 CDU_OK, CDU_EINVAL, CDU_ENOMEM, CDU_ECUDA, CDU_ESTATE, CDU_ENUMERIC = range(6)
 CDU_F32, CDU_F64 = 0, 1
 CDU_ZERO, CDU_NONNEG, CDU_SOC, CDU_PSD = 0, 1, 2, 3
-CDU_RHO_PER_ITER, CDU_RHO_PER_PROBLEM = 0, 1
+CDU_RHO_PER_ITER, CDU_RHO_PER_PROBLEM, CDU_RHO_PER_ROW = 0, 1, 2
 CDU_CKPT_FULL, CDU_CKPT_LEAN = 0, 1
 _STATUS = {0: "CDU_OK", 1: "CDU_EINVAL", 2: "CDU_ENOMEM", 3: "CDU_ECUDA", 4: "CDU_ESTATE", 5: "CDU_ENUMERIC"}
 
 EXPORTED_SYMBOLS = ("cdu_create", "cdu_forward", "cdu_backward", "cdu_get_stats", "cdu_get_iterate", "cdu_last_error",
                     "cdu_destroy", "cdu_version", "cdu_psd_project", "cdu_psd_vjp", "cdu_profile", "cdu_get_profile",
-                    "cdu_measure_peak", "cdu_backward_inject", "cdu_backward_eq12", "cdu_get_features", "cdu_solve")
+                    "cdu_measure_peak", "cdu_backward_inject", "cdu_backward_eq12", "cdu_get_features", "cdu_solve", "cdu_rectify_rho")
 
 
 class CduError(RuntimeError):
@@ -87,6 +87,8 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.cdu_backward_eq12.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, vp]
     lib.cdu_get_features.restype = i32
     lib.cdu_get_features.argtypes = [vp, i32, vp, vp, vp, vp, vp, i32, vp]
+    lib.cdu_rectify_rho.restype = i32
+    lib.cdu_rectify_rho.argtypes = [vp, i32, vp, i32, vp]
     lib.cdu_solve.restype = i32
     lib.cdu_solve.argtypes = [vp, i32, i32, f64, f64, f64, f64, i32, vp, vp, vp, vp, vp, vp, vp, vp, i32, vp]
     lib.cdu_get_stats.restype = i32
@@ -191,8 +193,8 @@ class Handle:
         """cdu_forward. Device mode: torch CUDA tensors in, returns (xK, sK, yK) CUDA tensors.
         Host mode: pinned torch CPU tensors / numpy arrays in and out (copies are inside the call)."""
         torch = _torch()
-        cnt = K * (self.B if rho_mode == CDU_RHO_PER_PROBLEM else 1)
-        for nm, t, n in (("rho", rho, cnt), ("alpha", alpha, cnt), ("x0", x0, self.N), ("s0", s0, self.M), ("y0", y0, self.M)):
+        cnt = K * (1 if rho_mode == CDU_RHO_PER_ITER else self.B)
+        for nm, t, n in (("rho", rho, K * self.M if rho_mode == CDU_RHO_PER_ROW else cnt), ("alpha", alpha, cnt), ("x0", x0, self.N), ("s0", s0, self.M), ("y0", y0, self.M)):
             self._want(nm, t, n, host)
         if out is None:
             if host:
@@ -207,14 +209,8 @@ class Handle:
     def backward(self, g_xK=None, g_sK=None, g_yK=None, out=None, host=False):
         """cdu_backward -> dict(g_rho, g_alpha, g_sigma, g_x0, g_s0, g_y0)."""
         torch = _torch()
-        cnt = self.K * (self.B if self.rho_mode == CDU_RHO_PER_PROBLEM else 1)
-        scnt = self.B if self.rho_mode == CDU_RHO_PER_PROBLEM else 1
         if out is None:
-            sizes = dict(g_rho=cnt, g_alpha=cnt, g_sigma=scnt, g_x0=self.N, g_s0=self.M, g_y0=self.M)
-            if host:
-                out = {k: torch.empty(n, dtype=self.torch_dtype).pin_memory() for k, n in sizes.items()}
-            else:
-                out = {k: torch.empty(n, dtype=self.torch_dtype, device="cuda") for k, n in sizes.items()}
+            out = self._grad_out(host)
         for nm, t, n in (("g_xK", g_xK, self.N), ("g_sK", g_sK, self.M), ("g_yK", g_yK, self.M)):
             self._want(nm, t, n, host)
         self._check(self.lib.cdu_backward(self.h, _ptr(g_xK), _ptr(g_sK), _ptr(g_yK), _ptr(out.get("g_rho")),
@@ -224,9 +220,9 @@ class Handle:
 
     def _grad_out(self, host):
         torch = _torch()
-        cnt = self.K * (self.B if self.rho_mode == CDU_RHO_PER_PROBLEM else 1)
-        scnt = self.B if self.rho_mode == CDU_RHO_PER_PROBLEM else 1
-        sizes = dict(g_rho=cnt, g_alpha=cnt, g_sigma=scnt, g_x0=self.N, g_s0=self.M, g_y0=self.M)
+        cnt = self.K * (1 if self.rho_mode == CDU_RHO_PER_ITER else self.B)
+        scnt = 1 if self.rho_mode == CDU_RHO_PER_ITER else self.B
+        sizes = dict(g_rho=self.K * self.M if self.rho_mode == CDU_RHO_PER_ROW else cnt, g_alpha=cnt, g_sigma=scnt, g_x0=self.N, g_s0=self.M, g_y0=self.M)
         if host:
             return {k: torch.empty(n, dtype=self.torch_dtype).pin_memory() for k, n in sizes.items()}
         return {k: torch.empty(n, dtype=self.torch_dtype, device="cuda") for k, n in sizes.items()}
@@ -257,6 +253,11 @@ class Handle:
                                               _ptr(o["scal"]), 0, _stream()))
         o["scal"] = o["scal"].view(self.B, 3)
         return o
+
+    def rectify_rho(self, K, rho):
+        """cdu_rectify_rho in place on a device tensor [K, M]."""
+        self._check(self.lib.cdu_rectify_rho(self.h, int(K), _ptr(rho), 0, _stream()))
+        return rho
 
     def solve(self, max_iter, check_every, eps, rho0=0.1, alpha=1.6, sigma=1e-6, adapt_rho=True, x0=None, s0=None, y0=None):
         """cdu_solve (device pointers) -> (x, s, y, iters [B] numpy int32, res [B, 2] numpy)."""

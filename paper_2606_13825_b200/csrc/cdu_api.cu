@@ -98,6 +98,12 @@ cdu_status cdu_solve(cdu_handle h, int32_t max_iter, int32_t check_every, double
                   reinterpret_cast<cudaStream_t>(cuda_stream));
 }
 
+cdu_status cdu_rectify_rho(cdu_handle h, int32_t K, void* rho, int32_t io_on_host, void* cuda_stream) {
+  if (!h) return CDU_EINVAL;
+  DeviceGuard g(h->device);
+  return h->rectify(K, rho, io_on_host, reinterpret_cast<cudaStream_t>(cuda_stream));
+}
+
 cdu_status cdu_get_stats(cdu_handle h, cdu_stats* out) {
   if (!h) return CDU_EINVAL;
   DeviceGuard g(h->device);

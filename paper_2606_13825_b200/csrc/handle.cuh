@@ -487,6 +487,8 @@ struct HandleT : cdu_handle_s {
   double* GZ[2] = {nullptr, nullptr};
   double *g_rho_pb = nullptr, *g_alpha_pb = nullptr, *g_sigma_pb = nullptr, *part_pre = nullptr;
   T *d_rho = nullptr, *d_alpha = nullptr;
+  T *d_rho_row = nullptr, *row_stage = nullptr;   // CDU_RHO_PER_ROW: rho [K_max][sum m_b], staging of g_rho for host output (lazy)
+  double* g_rho_row = nullptr;                    // CDU_RHO_PER_ROW: [K_max][sum m_b] row-wise g_rho (lazy)
   T* stage = nullptr;        // host-I/O staging, N + 2 Mtot (+ gradient outputs)
   T* stage_g = nullptr;      // 2 K_max B + B
   int *cg_f = nullptr, *cg_b = nullptr, *cg_f0 = nullptr, *cg_b0 = nullptr, *cg_max = nullptr, *flags = nullptr;
@@ -527,6 +529,7 @@ struct HandleT : cdu_handle_s {
     Hyper<T> H;
     H.rho = d_rho; H.alpha = d_alpha; H.sigma = sigma_last;
     H.kstride = mode_last == CDU_RHO_PER_ITER ? 1 : B; H.pstride = mode_last == CDU_RHO_PER_ITER ? 0 : 1;
+    if (mode_last == CDU_RHO_PER_ROW) { H.rho_row = d_rho_row; H.mstride = Mtot; H.rho = nullptr; }
     return H;
   }
   cdu_status forward(int K, const void* rho, int mode, double sigma, const void* alpha, const void* x0, const void* s0,
@@ -538,6 +541,8 @@ struct HandleT : cdu_handle_s {
   cdu_status solve(int max_iter, int check_every, double eps, double rho0, double alpha, double sigma, int adapt_rho, const void* x0,
                    const void* s0, const void* y0, void* x, void* s, void* y, int* iters_out, double* res_out, int host, cudaStream_t st) override;
   bool continue_from_last = false;
+  int n_rect = 0; const long long* rect_row0 = nullptr; const int* rect_rows = nullptr;
+  cdu_status rectify(int K, void* rho, int host, cudaStream_t st) override;
   cdu_status stats(cdu_stats* out) override;
   cdu_status iterate(int k, void* x, void* s, void* y, int host, cudaStream_t st) override;
   void profile_enable(int on) override { prof.on = on != 0; }
@@ -594,6 +599,15 @@ cdu_status HandleT<T, IT>::init(const cdu_problem* pr, const cdu_options* op, cu
     soc_off[b + 1] = (int)soc_start.size(); psdblk_off[b + 1] = (int)psd_p.size();
   }
   has_psd = !psd_p.empty();
+  {   // blocks whose rows must share one rho (cdu_rectify_rho)
+    std::vector<long long> r0v; std::vector<int> nr;
+    for (int b = 0; b < B; ++b)
+      for (int j = soc_off[b]; j < soc_off[b + 1]; ++j) { r0v.push_back(pr->row_off[b] + soc_start[j]); nr.push_back(soc_dim[j]); }
+    for (size_t j = 0; j < psd_p.size(); ++j) { r0v.push_back(psd_row0[j]); nr.push_back(psd_p[j] * (psd_p[j] + 1) / 2); }
+    n_rect = (int)nr.size();
+    rect_row0 = pool.upload(r0v, st); rect_rows = pool.upload(nr, st);
+    CU_OK(cudaStreamSynchronize(st));
+  }
 
   // ---- CSR re-packing: int32 rowptr, transposed copy, diag(P), column square sums ----------------------------
   const T* Av = reinterpret_cast<const T*>(pr->A_val);
@@ -933,19 +947,32 @@ cdu_status HandleT<T, IT>::forward(int K, const void* rho, int mode, double sigm
   if (K < 1 || K > K_max) { err = "cdu_forward: K out of [1, K_max]"; return CDU_EINVAL; }
   if (!rho || !alpha) { err = "cdu_forward: NULL rho/alpha"; return CDU_EINVAL; }
   if (!(sigma > 0.0)) { err = "cdu_forward: sigma must be > 0"; return CDU_EINVAL; }
-  if (mode != CDU_RHO_PER_ITER && mode != CDU_RHO_PER_PROBLEM) { err = "cdu_forward: bad rho_mode"; return CDU_EINVAL; }
-  const size_t cnt = (size_t)K * (mode == CDU_RHO_PER_ITER ? 1 : B);
+  if (mode != CDU_RHO_PER_ITER && mode != CDU_RHO_PER_PROBLEM && mode != CDU_RHO_PER_ROW) { err = "cdu_forward: bad rho_mode"; return CDU_EINVAL; }
+  const bool rows = mode == CDU_RHO_PER_ROW;
+  const size_t cnt = (size_t)K * (mode == CDU_RHO_PER_ITER ? 1 : B);          // alpha (and rho unless per row)
+  const size_t cnt_rho = rows ? (size_t)K * (size_t)Mtot : cnt;
+  if (rows && !d_rho_row) {
+    d_rho_row = pool.alloc<T>((size_t)K_max * Mtot); row_stage = pool.alloc<T>((size_t)K_max * Mtot);
+    g_rho_row = pool.alloc<double>((size_t)K_max * Mtot);
+    if (!d_rho_row || !row_stage || !g_rho_row) { err = "cudaMalloc (per-row rho)"; return CDU_ENOMEM; }
+  }
   if (host) {
     const T* r = reinterpret_cast<const T*>(rho); const T* a = reinterpret_cast<const T*>(alpha);
-    for (size_t i = 0; i < cnt; ++i)
-      if (!(r[i] > (T)0) || !(a[i] > (T)0) || !(a[i] < (T)2)) { err = "cdu_forward: rho must be > 0 and alpha in (0,2)"; return CDU_EINVAL; }
+    for (size_t i = 0; i < cnt_rho; ++i) if (!(r[i] > (T)0)) { err = "cdu_forward: rho must be > 0"; return CDU_EINVAL; }
+    for (size_t i = 0; i < cnt; ++i) if (!(a[i] > (T)0) || !(a[i] < (T)2)) { err = "cdu_forward: alpha must be in (0,2)"; return CDU_EINVAL; }
   }
   const cudaMemcpyKind kind = host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
-  CU_OK(cudaMemcpyAsync(d_rho, rho, cnt * sizeof(T), kind, st));
+  CU_OK(cudaMemcpyAsync(rows ? d_rho_row : d_rho, rho, cnt_rho * sizeof(T), kind, st));
   CU_OK(cudaMemcpyAsync(d_alpha, alpha, cnt * sizeof(T), kind, st));
   CU_OK(cudaMemsetAsync(flags, 0, B * sizeof(int), st));
   if (!host) {   // device-resident hyper-parameters: checked by a kernel, reported through the per-problem flags
-    k_check_hyper<T><<<std::min<int>((int)((cnt + 255) / 256), 64), 256, 0, st>>>(d_rho, d_alpha, (long long)cnt, mode == CDU_RHO_PER_ITER ? 0 : B, B, flags);
+    if (rows) {
+      k_check_hyper_rows<T><<<std::min<int>((int)((cnt_rho + 255) / 256), 256), 256, 0, st>>>(d_rho_row, (long long)cnt_rho, (long long)Mtot, D.row_off, B, flags);
+      k_check_hyper<T><<<std::min<int>((int)((cnt + 255) / 256), 64), 256, 0, st>>>(d_alpha, d_alpha, (long long)cnt, B, B, flags);
+      ++launches;
+    } else {
+      k_check_hyper<T><<<std::min<int>((int)((cnt + 255) / 256), 64), 256, 0, st>>>(d_rho, d_alpha, (long long)cnt, mode == CDU_RHO_PER_ITER ? 0 : B, B, flags);
+    }
     ++launches;
     CU_OK(cudaGetLastError());
   }
@@ -1078,6 +1105,32 @@ cdu_status HandleT<T, IT>::solve(int max_iter, int check_every, double eps, doub
 }
 
 template <typename T, typename IT>
+cdu_status HandleT<T, IT>::rectify(int K, void* rho, int host, cudaStream_t st) {
+  if (K < 1 || K > K_max || !rho) { err = "cdu_rectify_rho: bad arguments"; return CDU_EINVAL; }
+  if (n_rect == 0) return CDU_OK;
+  const size_t cnt = (size_t)K * Mtot;
+  T* d = reinterpret_cast<T*>(rho);
+  if (host) {
+    if (!row_stage) {
+      d_rho_row = pool.alloc<T>((size_t)K_max * Mtot); row_stage = pool.alloc<T>((size_t)K_max * Mtot);
+      g_rho_row = pool.alloc<double>((size_t)K_max * Mtot);
+      if (!d_rho_row || !row_stage || !g_rho_row) { err = "cudaMalloc (per-row rho)"; return CDU_ENOMEM; }
+    }
+    d = row_stage;
+    CU_OK(cudaMemcpyAsync(d, rho, cnt * sizeof(T), cudaMemcpyHostToDevice, st));
+  }
+  for (int j0 = 0; j0 < n_rect; j0 += 65535 * 32) {
+    const int nb = std::min(n_rect - j0, 65535 * 32);
+    k_rectify<T><<<dim3(nb, K), 32, 0, st>>>(d, (long long)Mtot, rect_row0 + j0, rect_rows + j0, nb);
+    ++launches;
+  }
+  CU_OK(cudaGetLastError());
+  last_stream = st;
+  if (host) { CU_OK(cudaMemcpyAsync(rho, d, cnt * sizeof(T), cudaMemcpyDeviceToHost, st)); CU_OK(cudaStreamSynchronize(st)); }
+  return CDU_OK;
+}
+
+template <typename T, typename IT>
 cdu_status HandleT<T, IT>::features(int k, void* rp_bar, void* rd_bar, void* delta_p, void* delta_d, void* scal, int host, cudaStream_t st) {
   if (k < 0 || k > K_last || K_last < 1) { err = "cdu_get_features: k out of range (or no forward pass)"; return CDU_EINVAL; }
   if (delta_p && k >= 1 && ckpt_mode != CDU_CKPT_FULL) { err = "cdu_get_features: delta_p needs FULL checkpoints (s-tilde is not stored in LEAN mode)"; return CDU_ESTATE; }
@@ -1138,6 +1191,7 @@ cdu_status HandleT<T, IT>::backward(const void* gx, const void* gs, const void* 
     Q.XT = XT + (full ? (size_t)k * N : 0); Q.ST = ST + (full ? (size_t)k * Mtot : 0);
     Q.Gin = GZ[(k + 1) & 1]; Q.Gout = GZ[k & 1];
     Q.g_rho_pb = g_rho_pb; Q.g_alpha_pb = g_alpha_pb; Q.g_sigma_pb = g_sigma_pb; Q.part_pre = part_pre;
+    Q.g_rho_row = mode_last == CDU_RHO_PER_ROW ? g_rho_row : nullptr;
     Q.recompute = full ? 0 : 1;
     Q.warm_adjoint = k < K - 1 ? 1 : 0;
     if (!has_psd && !diag_on) {
@@ -1172,12 +1226,23 @@ cdu_status HandleT<T, IT>::backward(const void* gx, const void* gs, const void* 
     }
     if ((s = add_extra(k, Q.Gout, ex, host, st)) != CDU_OK) return s;     // cotangents that enter at z^k
   }
-  const int pp = mode_last == CDU_RHO_PER_PROBLEM;
+  const bool rows = mode_last == CDU_RHO_PER_ROW;
+  const int pp = mode_last != CDU_RHO_PER_ITER;
   const size_t cnt = (size_t)K * (pp ? B : 1), scnt = pp ? B : 1;
+  if (rows && g_rho) {     // g_rho [K][sum m_b]: one entry per row, no reduction
+    const long long nr = (long long)K * Mtot;
+    T* o = host ? row_stage : reinterpret_cast<T*>(g_rho);
+    k_store_vec<T><<<(int)std::min<long long>((nr + 255) / 256, 4096), 256, 0, st>>>(o, g_rho_row, nr);
+    ++launches;
+    CU_OK(cudaGetLastError());
+    if (host) CU_OK(cudaMemcpyAsync(g_rho, o, nr * sizeof(T), cudaMemcpyDeviceToHost, st));
+    g_rho = nullptr;
+  }
   T* o_rho = host ? stage_g : reinterpret_cast<T*>(g_rho);
   T* o_alpha = host ? stage_g + cnt : reinterpret_cast<T*>(g_alpha);
   T* o_sigma = host ? stage_g + 2 * cnt : reinterpret_cast<T*>(g_sigma);
   if (host) { if (!g_rho) o_rho = nullptr; if (!g_alpha) o_alpha = nullptr; if (!g_sigma) o_sigma = nullptr; }
+  if (rows) o_rho = nullptr;
   k_reduce_grads<T><<<1, 256, 0, st>>>(g_rho_pb, g_alpha_pb, g_sigma_pb, K, B, pp, o_rho, o_alpha, o_sigma);
   ++launches;
   CU_OK(cudaGetLastError());

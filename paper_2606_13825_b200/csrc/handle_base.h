@@ -21,6 +21,7 @@ struct cdu_handle_s {
   virtual cdu_status solve(int max_iter, int check_every, double eps, double rho0, double alpha, double sigma, int adapt_rho,
                            const void* x0, const void* s0, const void* y0, void* x, void* s, void* y, int* iters_out, double* res_out,
                            int host, cudaStream_t st) = 0;
+  virtual cdu_status rectify(int K, void* rho, int host, cudaStream_t st) = 0;
   virtual cdu_status features(int k, void* rp_bar, void* rd_bar, void* delta_p, void* delta_d, void* scal, int host, cudaStream_t st) = 0;
   virtual cdu_status stats(cdu_stats* out) = 0;
   virtual cdu_status iterate(int k, void* x, void* s, void* y, int host, cudaStream_t st) = 0;

@@ -72,7 +72,11 @@ struct BatchDev {
 template <typename T>
 struct Hyper {  // per-iteration hyper-parameters as the caller laid them out (cdu_rho_mode)
   const T* rho; const T* alpha; int kstride, pstride; double sigma;
+  const T* rho_row = nullptr; long long mstride = 0;   // CDU_RHO_PER_ROW: rho_row[k][sum m_b] (constant inside SOC / PSD blocks)
   __device__ double rho_at(int k, int b) const { return (double)rho[(size_t)k * kstride + (size_t)b * pstride]; }
+  // rho of the cone block that starts at global row `grow` of problem b
+  __device__ double rho_blk(int k, int b, long long grow) const { return rho_row ? (double)rho_row[(size_t)k * mstride + grow] : rho_at(k, b); }
+  __device__ const T* rows_of(int k, long long r0) const { return rho_row ? rho_row + (size_t)k * mstride + r0 : nullptr; }
   __device__ double alpha_at(int k, int b) const { return (double)alpha[(size_t)k * kstride + (size_t)b * pstride]; }
 };
 
@@ -286,6 +290,8 @@ struct Prob {  // one problem's view of the batch, as seen by one CTA of its tea
   double *xi, *rd, *tm, *W, *GW, *lam;
   T *r, *p, *Ap, *d, *dinv, *tA;
   double rho, alpha, sigma;
+  const T* rrow = nullptr;            // per-row rho of this problem at this iteration (NULL: the scalar rho)
+  __device__ __forceinline__ double rh(int row) const { return rrow ? (double)rrow[row] : rho; }
   Team<MULTI>* team;
   double* scratch;                    // partial sums of multi-chunk rows (sell_rows), D.sell_slots doubles
   __device__ Prob(const BatchDev<T, IT>& D, int b_, Team<MULTI>* tm_, unsigned char* dsm) : b(b_), team(tm_) {
@@ -339,8 +345,8 @@ __device__ __forceinline__ void rows_P(const BatchDev<T, IT>& D, const Prob<T, I
 // q = M p for the CG: tA = rho A p ; Ap = A' tA + P p + sigma p ; returns the team-wide <p, Ap>.
 template <typename T, typename IT, int MULTI>
 __device__ __forceinline__ double apply_M(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c) {
-  const T rhoT = (T)c.rho, sigT = (T)c.sigma;
-  rows_A<T>(D, c, c.p, [&](int row, T a) { c.tA[row] = rhoT * a; });
+  const T sigT = (T)c.sigma;
+  rows_A<T>(D, c, c.p, [&](int row, T a) { c.tA[row] = (T)c.rh(row) * a; });
   c.team->sync();
   rows_AT<T>(D, c, c.tA, [&](int row, T a) { c.Ap[row] = a; });
   __syncthreads();   // Ap rows are owned by this CTA
@@ -408,7 +414,12 @@ __device__ int solve_M(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, co
   const int tid = threadIdx.x, nt = blockDim.x;
   double acc[1] = {0.0};
   for (int i = c.nlo + tid; i < c.nhi; i += nt) {
-    c.dinv[i] = (T)(1.0 / ((double)c.diagP[i] + c.sigma + c.rho * (double)c.colsq[i]));
+    double dA = c.rho * (double)c.colsq[i];
+    if (c.rrow) {        // diag(A' D(rho) A)_i = sum_r a_ri^2 rho_r
+      dA = 0.0;
+      for (int e = c.AT_rp[i]; e < c.AT_rp[i + 1]; ++e) { const double v = (double)D.AT_v[e]; dA += v * v * (double)c.rrow[(int)D.AT_ci[e]]; }
+    }
+    c.dinv[i] = (T)(1.0 / ((double)c.diagP[i] + c.sigma + dA));
     const double v = rhs[i];
     acc[0] += v * v;
     out[i] = xbase ? xbase[i] : 0.0;
@@ -429,7 +440,7 @@ __device__ int solve_M(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, co
       rr0 = nr2;
       __syncthreads();
     } else {  // r = rhs - M out, fp64
-      rows_A<double>(D, c, out, [&](int row, double a) { c.tm[row] = c.rho * a; });
+      rows_A<double>(D, c, out, [&](int row, double a) { c.tm[row] = c.rh(row) * a; });
       c.team->sync();
       rows_AT<double>(D, c, c.tm, [&](int row, double a) { c.rd[row] = a; });
       __syncthreads();
@@ -464,7 +475,7 @@ template <typename T, typename IT, int MULTI>
 __device__ int lin_solve_step(const BatchDev<T, IT>& D, const Prob<T, IT, MULTI>& c, const double* x, const double* s,
                               const double* y, double* xt, int* flag, int* it0, const double* xstart = nullptr) {
   const int tid = threadIdx.x, nt = blockDim.x;
-  for (int i = c.mlo + tid; i < c.mhi; i += nt) c.tm[i] = c.rho * ((double)c.bv[i] - s[i]) - y[i];
+  for (int i = c.mlo + tid; i < c.mhi; i += nt) c.tm[i] = c.rh(i) * ((double)c.bv[i] - s[i]) - y[i];
   c.team->sync();
   rows_AT<double>(D, c, c.tm, [&](int row, double a) { c.xi[row] = c.sigma * x[row] - (double)c.q[row] + a; });
   c.team->sync();   // tm is reused by solve_M's residual pass
@@ -496,19 +507,20 @@ __global__ void __launch_bounds__(1024) k_fwd(BatchDev<T, IT> D, Hyper<T> H, Ite
   const int tid = threadIdx.x, nt = blockDim.x;
   for (int b = team_id; b < D.B; b += nteams) {
     Prob<T, IT, MULTI> c(D, b, &team, dsm_);
-    c.rho = H.rho_at(k, b); c.alpha = H.alpha_at(k, b); c.sigma = H.sigma;
+    c.rho = H.rho_row ? 0.0 : H.rho_at(k, b); c.alpha = H.alpha_at(k, b); c.sigma = H.sigma;
     const long long v0 = D.var_off[b], r0 = D.row_off[b];
+    c.rrow = H.rows_of(k, r0);
     const double *x = I.Zk + v0, *s = I.Zk + D.N + r0, *y = I.Zk + D.N + D.Mtot + r0;
     double *x1 = I.Zk1 + v0, *s1 = I.Zk1 + D.N + r0, *y1 = I.Zk1 + D.N + D.Mtot + r0;
     double *xt = I.XT + v0, *st = I.ST + r0;
     int flag = 0, it0 = 0;
     const int iters = lin_solve_step(D, c, x, s, y, xt, &flag, &it0, I.XTprev ? I.XTprev + v0 : nullptr);
-    const double al = c.alpha, rho = c.rho;
+    const double al = c.alpha;
     const uint8_t* kind = D.rowkind + r0;
     rows_A<double>(D, c, xt, [&](int row, double a) {
       const double stv = (double)c.bv[row] - a;
       st[row] = stv;
-      const double yv = y[row];
+      const double yv = y[row], rho = c.rh(row);
       const double w = al * stv + (1.0 - al) * s[row] - yv / rho;
       c.W[row] = w;
       const int kd = kind[row];
@@ -527,6 +539,7 @@ __global__ void __launch_bounds__(1024) k_fwd(BatchDev<T, IT> D, Hyper<T> H, Ite
       for (int j = D.soc_off[b] + gw; j < D.soc_off[b + 1]; j += wtot) {
         const int st0 = D.soc_start[j], dim = D.soc_dim[j];
         const double* w = c.W + st0;
+        const double rho = c.rh(st0);
         double nu2 = 0.0;
         for (int i = 1 + lane; i < dim; i += 32) { const double wi = ldv<MULTI>(w + i); nu2 += wi * wi; }
         nu2 = warp_sum(nu2);
@@ -567,6 +580,7 @@ struct BwdPtrs {
   double* g_alpha_pb;
   double* g_sigma_pb;
   double* part_pre;    // [B][2] partials handed from the pre to the post phase
+  double* g_rho_row = nullptr;   // CDU_RHO_PER_ROW: [K][sum m_b] row-wise g_rho (Eq. 6 verbatim plus the RHS terms)
   int recompute;       // LEAN: re-solve for xt, st
   int warm_adjoint;    // not the first reverse step: D.lam holds the previous step's adjoint solution
 };
@@ -581,7 +595,7 @@ __device__ void bwd_pre(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const B
   const double* s1 = Q.Zk1 + D.N + r0;
   const double *gs = Q.Gin + D.N + r0, *gy = Q.Gin + D.N + D.Mtot + r0;
   double *xt = Q.XT + v0, *st = Q.ST + r0;
-  const double al = c.alpha, rho = c.rho;
+  const double al = c.alpha;
   if (Q.recompute) {
     *iters += lin_solve_step(D, c, x, s, y, xt, flag, it0);
     rows_A<double>(D, c, xt, [&](int row, double a) { st[row] = (double)c.bv[row] - a; });
@@ -590,7 +604,7 @@ __device__ void bwd_pre(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const B
   const uint8_t* kind = D.rowkind + r0;
   double acc[2] = {0.0, 0.0};   // [0]: <gy, s+ - w>, [1]: <gw, y>
   for (int i = c.mlo + tid; i < c.mhi; i += nt) {
-    const double yv = y[i];
+    const double yv = y[i], rho = c.rh(i);
     const double w = al * st[i] + (1.0 - al) * s[i] - yv / rho;
     c.W[i] = w;
     const int kd = kind[i];
@@ -610,6 +624,7 @@ __device__ void bwd_pre(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const B
     for (int j = D.soc_off[b] + gwp; j < D.soc_off[b + 1]; j += wtot) {
       const int st0 = D.soc_start[j], dim = D.soc_dim[j];
       const double* w = c.W + st0;
+      const double rho = c.rh(st0);
       double nu2 = 0.0, dot = 0.0;   // dot = u . G_u
       for (int i = 1 + lane; i < dim; i += 32) {
         const double wi = ldv<MULTI>(w + i);
@@ -652,7 +667,11 @@ __device__ void bwd_post(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const 
   const double* gx1 = Q.Gin + v0;
   double *gx = Q.Gout + v0, *gs = Q.Gout + D.N + r0, *gy = Q.Gout + D.N + D.Mtot + r0;
   const double *xt = Q.XT + v0, *st = Q.ST + r0;
-  const double al = c.alpha, rho = c.rho, sg = c.sigma;
+  const double al = c.alpha, sg = c.sigma;
+  const double* gy1 = Q.Gin + D.N + D.Mtot + r0;         // per-row rho: the terms of g_rho that the scalar modes take from dots
+  const double* s1 = Q.Zk1 + D.N + r0;
+  const double* yk = Q.Zk + D.N + D.Mtot + r0;
+  double* grow = Q.g_rho_row ? Q.g_rho_row + (size_t)k * D.Mtot + r0 : nullptr;
   double d_gy_sw = part[0], d_gw_y = part[1];
   for (int j = D.psdblk_off[b]; j < D.psdblk_off[b + 1]; ++j) { d_gy_sw += D.psd_part[2 * j]; d_gw_y += D.psd_part[2 * j + 1]; }
   // B6: rhs = alpha g_x+ - A'(alpha g_w)   (g_st = alpha g_w)
@@ -668,9 +687,10 @@ __device__ void bwd_post(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const 
   double acc[3] = {0.0, 0.0, 0.0};   // rho, alpha, sigma
   rows_A<double>(D, c, c.lam, [&](int row, double u) {
     const double gw = ldv<MULTI>(c.GW + row);   // SOC rows may have been written by a peer CTA
-    const double ds = st[row] - s[row];
+    const double ds = st[row] - s[row], rho = c.rh(row);
     acc[0] += u * ds;
     acc[1] += gw * ds;                                  // B5: <g_vhat, st - s>
+    if (grow) grow[row] = u * ds + gy1[row] * (s1[row] - ldv<MULTI>(c.W + row)) + gw * yk[row] / (rho * rho);   // B1 + B4 + (B7+B9), row by row
     gs[row] = (1.0 - al) * gw - rho * u;                // B5 + B9
     gy[row] = -gw / rho - u;                            // B4 + B9
   });
@@ -683,7 +703,7 @@ __device__ void bwd_post(const BatchDev<T, IT>& D, Prob<T, IT, MULTI>& c, const 
   c.team->sum(acc);
   if (tid == 0 && c.team->rank == 0) {
     const size_t o = (size_t)k * D.B + b;
-    Q.g_rho_pb[o] = acc[0] + d_gy_sw + d_gw_y / (rho * rho);   // B1 + B4 + (B7+B9)
+    Q.g_rho_pb[o] = grow ? 0.0 : acc[0] + d_gy_sw + d_gw_y / (c.rho * c.rho);   // B1 + B4 + (B7+B9)
     Q.g_alpha_pb[o] = acc[1];
     Q.g_sigma_pb[o] = acc[2];
   }
@@ -695,7 +715,8 @@ __global__ void __launch_bounds__(1024) k_bwd(BatchDev<T, IT> D, Hyper<T> H, Bwd
   CDU_TEAM_PROLOGUE();
   for (int b = team_id; b < D.B; b += nteams) {
     Prob<T, IT, MULTI> c(D, b, &team, dsm_);
-    c.rho = H.rho_at(k, b); c.alpha = H.alpha_at(k, b); c.sigma = H.sigma;
+    c.rho = H.rho_row ? 0.0 : H.rho_at(k, b); c.alpha = H.alpha_at(k, b); c.sigma = H.sigma;
+    c.rrow = H.rows_of(k, D.row_off[b]);
     int flag = 0, iters = 0, it0 = 0;
     double part[2];
     if (phase != 2) {
@@ -728,6 +749,33 @@ __global__ void k_check_hyper(const T* rho, const T* alpha, long long cnt, int p
     }
   }
 }
+// per-row rho (CDU_RHO_PER_ROW): rho[k][row] > 0, flag on the problem that owns the row
+template <typename T>
+__global__ void k_check_hyper_rows(const T* rho, long long cnt, long long Mtot, const int* row_off, int B, int* flags) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < cnt; i += (long long)gridDim.x * blockDim.x) {
+    if (!(rho[i] > (T)0)) {
+      const int row = (int)(i % Mtot);
+      int lo = 0, hi = B;
+      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (row_off[mid] <= row) lo = mid; else hi = mid; }
+      atomicOr(flags + lo, FLAG_BAD_HYPER);
+    }
+  }
+}
+
+// Rectification of PAPER.md App. E (L343): a per-row rho is averaged over every SOC / PSD block and the mean is broadcast
+// back over the block (the operation is its own adjoint, so the same kernel rectifies g_rho). One warp per (block, k).
+template <typename T>
+__global__ void k_rectify(T* rho, long long Mtot, const long long* blk_row0, const int* blk_rows, int nblk) {
+  const int j = blockIdx.x, lane = threadIdx.x;
+  if (j >= nblk) return;
+  T* r = rho + (size_t)blockIdx.y * Mtot + blk_row0[j];
+  const int n = blk_rows[j];
+  double a = 0.0;
+  for (int i = lane; i < n; i += 32) a += (double)r[i];
+  a = warp_sum(a) / (double)n;
+  for (int i = lane; i < n; i += 32) r[i] = (T)a;
+}
+
 template <typename T>
 __global__ void k_load_vec(double* dst, const T* src, long long n) {   // dst = src (NULL -> 0)
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)

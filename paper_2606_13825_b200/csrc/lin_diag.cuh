@@ -28,26 +28,30 @@ struct DiagCtx {   // one problem as seen by one thread
   int b, n, m;
   long long v0, r0;
   double rho, alpha, sigma;
+  const T* rrow;                     // per-row rho of this problem at this iteration, or NULL
   __device__ DiagCtx(const BatchDev<T, IT>& D_, const Hyper<T>& H, int k, int b_) : D(D_), b(b_) {
     v0 = D.var_off[b]; r0 = D.row_off[b];
     n = D.var_off[b + 1] - (int)v0; m = D.row_off[b + 1] - (int)r0;
-    rho = H.rho_at(k, b); alpha = H.alpha_at(k, b); sigma = H.sigma;
+    rho = H.rho_row ? 0.0 : H.rho_at(k, b); alpha = H.alpha_at(k, b); sigma = H.sigma;
+    rrow = H.rows_of(k, r0);
   }
+  __device__ __forceinline__ double rh(int row) const { return rrow ? (double)rrow[row] : rho; }
   // t_j = sum_e v_e f(row_e) over column j of A, and diag(M)_j (exact: the squares are summed here, in fp64)
   template <typename F> __device__ __forceinline__ double col_gather(int j, double& dM, F f) const {
     double a = 0.0, sq = 0.0;
     for (int e = D.AT_rp[v0 + j]; e < D.AT_rp[v0 + j + 1]; ++e) {
       const double v = (double)D.AT_v[e];
-      a += v * f((int)D.AT_ci[e]);
-      sq += v * v;
+      const int r = (int)D.AT_ci[e];
+      a += v * f(r);
+      sq += v * v * rh(r);
     }
-    dM = (double)D.diagP[v0 + j] + sigma + rho * sq;
+    dM = (double)D.diagP[v0 + j] + sigma + sq;
     return a;
   }
   // S1 + S2: xt_j = (sigma x_j - q_j + [A'(rho (b - s) - y)]_j) / diag(M)_j
   __device__ __forceinline__ double xt_of(int j, const double* x, const double* s, const double* y) const {
     double dM;
-    const double a = col_gather(j, dM, [&](int r) { return rho * ((double)D.b[r0 + r] - s[r]) - y[r]; });
+    const double a = col_gather(j, dM, [&](int r) { return rh(r) * ((double)D.b[r0 + r] - s[r]) - y[r]; });
     return (sigma * x[j] - (double)D.q[v0 + j] + a) / dM;
   }
   // S10 + S11: lam_j = alpha (g_x+_j - [A' g_w]_j) / diag(M)_j
@@ -110,7 +114,7 @@ __global__ void __launch_bounds__(DIAG_THREADS) k_dfwd(BatchDev<T, IT> D, DiagTa
   const double *x = I.Zk + c.v0, *s = I.Zk + D.N + c.r0, *y = I.Zk + D.N + D.Mtot + c.r0;
   double *x1 = I.Zk1 + c.v0, *s1 = I.Zk1 + D.N + c.r0, *y1 = I.Zk1 + D.N + D.Mtot + c.r0;
   double *xt = I.XT + c.v0, *st = I.ST + c.r0;
-  const double al = c.alpha, rho = c.rho;
+  const double al = c.alpha;
   bool bad = false;
   for (int j = ch.y + tid; j < min(ch.z, c.n); j += DIAG_THREADS) {
     const double v = c.xt_of(j, x, s, y);
@@ -122,6 +126,7 @@ __global__ void __launch_bounds__(DIAG_THREADS) k_dfwd(BatchDev<T, IT> D, DiagTa
   for (int r = ch.y + tid; r < min(ch.z, c.m); r += DIAG_THREADS) {
     const double stv = diag_row_st(c, G, aval, r, x, s, y);
     st[r] = stv;
+    const double rho = c.rh(r);
     const double w = al * stv + (1.0 - al) * s[r] - y[r] / rho;
     D.W[c.r0 + r] = w;
     const int kd = kind[r];
@@ -146,7 +151,7 @@ __global__ void __launch_bounds__(DIAG_THREADS) k_dbwd_pre(BatchDev<T, IT> D, Di
   const double* s1 = Q.Zk1 + D.N + c.r0;
   const double *gs = Q.Gin + D.N + c.r0, *gy = Q.Gin + D.N + D.Mtot + c.r0;
   double *xt = Q.XT + c.v0, *st = Q.ST + c.r0;
-  const double al = c.alpha, rho = c.rho;
+  const double al = c.alpha;
   if (Q.recompute)
     for (int j = ch.y + tid; j < min(ch.z, c.n); j += DIAG_THREADS) xt[j] = c.xt_of(j, x, s, y);
   const uint8_t* kind = D.rowkind + c.r0;
@@ -154,7 +159,7 @@ __global__ void __launch_bounds__(DIAG_THREADS) k_dbwd_pre(BatchDev<T, IT> D, Di
   for (int r = ch.y + tid; r < min(ch.z, c.m); r += DIAG_THREADS) {
     double stv;
     if (Q.recompute) { stv = diag_row_st(c, G, aval, r, x, s, y); st[r] = stv; } else stv = st[r];
-    const double yv = y[r];
+    const double yv = y[r], rho = c.rh(r);
     const double w = al * stv + (1.0 - al) * s[r] - yv / rho;
     D.W[c.r0 + r] = w;
     const int kd = kind[r];
@@ -186,7 +191,11 @@ __global__ void __launch_bounds__(DIAG_THREADS) k_dbwd_post(BatchDev<T, IT> D, D
   double *gx = Q.Gout + c.v0, *gs = Q.Gout + D.N + c.r0, *gy = Q.Gout + D.N + D.Mtot + c.r0;
   const double *xt = Q.XT + c.v0, *st = Q.ST + c.r0;
   const double* gw = D.GW + c.r0;
-  const double al = c.alpha, rho = c.rho, sg = c.sigma;
+  const double al = c.alpha, sg = c.sigma;
+  const double* gy1 = Q.Gin + D.N + D.Mtot + c.r0;
+  const double* s1 = Q.Zk1 + D.N + c.r0;
+  const double* yk = Q.Zk + D.N + D.Mtot + c.r0;
+  double* grow = Q.g_rho_row ? Q.g_rho_row + (size_t)k * D.Mtot + c.r0 : nullptr;
   double acc[3] = {0.0, 0.0, 0.0};   // rho, alpha, sigma
   for (int j = ch.y + tid; j < min(ch.z, c.n); j += DIAG_THREADS) {
     const double l = c.lam_of(j, gx1, gw), g1 = gx1[j], dx = xt[j] - x[j];
@@ -197,9 +206,10 @@ __global__ void __launch_bounds__(DIAG_THREADS) k_dbwd_post(BatchDev<T, IT> D, D
   for (int r = ch.y + tid; r < min(ch.z, c.m); r += DIAG_THREADS) {
     const int jc = G.acol[c.r0 + r];
     const double u = jc >= 0 ? (double)aval[c.r0 + r] * c.lam_of(jc, gx1, gw) : 0.0;   // u = A lam
-    const double g = gw[r], ds = st[r] - s[r];
+    const double g = gw[r], ds = st[r] - s[r], rho = c.rh(r);
     acc[0] += u * ds;                                   // B7+B9: <u, st - s>
     acc[1] += g * ds;                                   // B5: <g_vhat, st - s>
+    if (grow) grow[r] = u * ds + gy1[r] * (s1[r] - D.W[c.r0 + r]) + g * yk[r] / (rho * rho);   // per-row rho: B1 + B4 + (B7+B9) row by row
     gs[r] = (1.0 - al) * g - rho * u;                   // B5 + B9
     gy[r] = -g / rho - u;                               // B4 + B9
   }
@@ -208,7 +218,7 @@ __global__ void __launch_bounds__(DIAG_THREADS) k_dbwd_post(BatchDev<T, IT> D, D
     double d_gy_sw = Q.part_pre[2 * c.b], d_gw_y = Q.part_pre[2 * c.b + 1];
     for (int j = D.psdblk_off[c.b]; j < D.psdblk_off[c.b + 1]; ++j) { d_gy_sw += D.psd_part[2 * j]; d_gw_y += D.psd_part[2 * j + 1]; }
     const size_t o = (size_t)k * D.B + c.b;
-    Q.g_rho_pb[o] = acc[0] + d_gy_sw + d_gw_y / (rho * rho);   // B1 + B4 + (B7+B9)
+    Q.g_rho_pb[o] = grow ? 0.0 : acc[0] + d_gy_sw + d_gw_y / (c.rho * c.rho);   // B1 + B4 + (B7+B9)
     Q.g_alpha_pb[o] = acc[1];
     Q.g_sigma_pb[o] = acc[2];
     D.cg_iters[c.b] += 1; D.cg_iters0[c.b] += 1;

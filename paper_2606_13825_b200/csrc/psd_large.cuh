@@ -49,7 +49,7 @@ __global__ void __launch_bounds__(256) k_large_smat(PsdTab tab, LargeTab lt, con
   const int lb = blockIdx.y, blk = lt.gblk[lb], nch = gridDim.x, ch = blockIdx.x;
   const int p = tab.p[blk];
   const long long row0 = tab.row0[blk];
-  const double sc = use_rho_scale ? H.rho_at(k, tab.prob[blk]) : 0.0;
+  const double sc = use_rho_scale ? H.rho_blk(k, tab.prob[blk], row0) : 0.0;
   T* g = G + lt.moff[lb];
   const double* a = v + row0;
   const double* a2 = v2 ? v2 + row0 : nullptr;
@@ -251,7 +251,7 @@ __global__ void __launch_bounds__(1024) k_large_finish_fwd(PsdTab tab, LargeTab 
   const int lb = blockIdx.y, blk = lt.gblk[lb];
   const int p = tab.p[blk];
   const long long row0 = tab.row0[blk];
-  const double rho = H.rho_at(k, tab.prob[blk]);
+  const double rho = H.rho_blk(k, tab.prob[blk], row0);
   const T* tm = Tm + lt.moff[lb];
   const double* w = A.W + row0;
   double *s1 = A.S1 + row0, *y1 = A.Y1 + row0;
@@ -293,7 +293,7 @@ __global__ void __launch_bounds__(256) k_large_finish_bwd(PsdTab tab, LargeTab l
   const int lb = blockIdx.y, blk = lt.gblk[lb], nch = gridDim.x, ch = blockIdx.x;
   const int p = tab.p[blk];
   const long long row0 = tab.row0[blk];
-  const double rho = H.rho_at(k, tab.prob[blk]);
+  const double rho = H.rho_blk(k, tab.prob[blk], row0);
   const T* o = Out + lt.moff[lb];
   const double *w = A.W + row0, *yk = A.Yk + row0, *s1 = A.S1 + row0, *gy = A.Gy + row0;
   double* gw = A.GW + row0;

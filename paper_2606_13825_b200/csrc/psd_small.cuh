@@ -380,7 +380,7 @@ __global__ void __launch_bounds__(psd_small_max_threads(MAXI)) k_psd_fwd_small(P
   double* shred = reinterpret_cast<double*>(smem_raw);                 // 64 doubles
   const JacobiWs<T> ws = jacobi_ws_carve<T>(smem_raw + 512, pe);
   T* lp = reinterpret_cast<T*>(smem_raw + 512 + jacobi_ws_bytes<T>(pe));   // pe: max(lambda, 0) by player
-  const double rho = H.rho_at(k, prob);
+  const double rho = H.rho_blk(k, prob, row0);
   const double* w = A.W + row0;
   const int ldv = ws.ldv;
   const int h = pe >> 1, ldh = h | 1, psz = h * ldh;
@@ -488,7 +488,7 @@ __global__ void __launch_bounds__(psd_small_max_threads(MAXI)) k_psd_bwd_small(P
   const int ldv = ws.ldv;
   T* G = ws.P0;             // the two p x p work matrices alias the Jacobi planes (dead after a recompute)
   T* Tm = G + pe * pe;
-  const double rho = H.rho_at(k, prob);
+  const double rho = H.rho_blk(k, prob, row0);
   const double* w = A.W + row0;
   int flag = 0;
   if (A.recompute) {
