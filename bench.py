@@ -503,13 +503,40 @@ def run_dk(args, cdu, torch):
                           paper_context="Fig. 4: DK ~ autograd ~ Tikhonov, Newton-Schulz ~10x slower; RTX 4090, fp64, curves only", points=pts)))
 
 
+def run_solve(args, cdu, torch):
+    """the vanilla baseline workload of PAPER.md Table 1 (L158-172): COSMO run to the OSQP-scaled tolerance 1e-3
+    with residual-balancing rho (L349) and 1e3 rho on the equality rows (L306), on 100 synthetic instances per class at the paper's
+    sizes (max-cut n = 50, Lovasz n = 60; ER graphs as in configs 2 and 4), fp64 like the paper. Paper (RTX 4090, fp64, its own
+    instances): max-cut 471 median iterations / 1.40 s, Lovasz theta 10 925 / 32.1 s - context, not a target."""
+    out = []
+    for name, mk, cfg in (("maxcut-n50", lambda g: W.maxcut_problem(g), dict(n=50, p=0.3, w="uniform")),
+                          ("lovasz-n60", lambda g: W.lovasz_problem(g), dict(n=60, p=0.1, w="unit"))):
+        probs = []
+        for b in range(args.batch or 100):
+            rng = np.random.default_rng(W.generators.BASE_SEED + 9000 + b)
+            probs.append(W.generators._round_problem(mk(W.erdos_renyi(rng, cfg["n"], cfg["p"], cfg["w"])), "f64"))
+        h = cdu.cdu_create(W.pack_batch(probs, "f64"), K_max=25)
+        h.solve(50, 25, 1e-3, rho0=0.1, adapt_rho=True, eq_scale=1e3)          # warm-up
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        x, s, y, iters, res = h.solve(20000, 25, 1e-3, rho0=0.1, alpha=1.6, adapt_rho=True, eq_scale=1e3)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        conv = iters[iters > 0]
+        out.append(dict(workload=name, instances=len(probs), converged=int((iters > 0).sum()), median_iters=float(np.median(conv)) if conv.size else None,
+                        max_iters=int(np.abs(iters).max()), seconds_for_the_batch=dt, check_every=25, eps=1e-3, flags=h.stats()["flags_or"]))
+        h.close()
+    print(json.dumps(dict(metric="vanilla_cosmo_to_tolerance", unit="iterations / s", dtype="f64", data="synthetic", higher_is_better=False,
+                          config=dict(workload="Table 1 baseline workload (PAPER.md L158-172)"), points=out)))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="all", choices=["all", "fig2", "dk"] + sorted(WORKLOADS))
+    ap.add_argument("--workload", default="all", choices=["all", "fig2", "dk", "solve"] + sorted(WORKLOADS))
     ap.add_argument("--n", type=int, default=0, help="fig2: one problem size instead of the sweep 1k .. 50k")
     ap.add_argument("--dtype", default=None, help="fig2: f64 (default, the paper's precision) or f32")
     ap.add_argument("--ckpt", default="full", choices=["full", "lean"])
@@ -525,7 +552,7 @@ def main():
     ap.add_argument("--no-batch", type=int, default=0, help="1: lane groups per row instead of warp row batches (debug)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    cfgs = [5, 3, 2] if args.workload in ("all", "fig2", "dk") else [WORKLOADS[args.workload]]
+    cfgs = [5, 3, 2] if args.workload in ("all", "fig2", "dk", "solve") else [WORKLOADS[args.workload]]
 
     def opts_of(cfg):
         o = dict(cg_refine=args.cg_refine, cg_refine_tol=args.cg_refine_tol)
@@ -549,9 +576,9 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     peaks = load_peaks(cdu)
-    if args.workload in ("fig2", "dk"):
+    if args.workload in ("fig2", "dk", "solve"):
         if rank == 0:
-            run_fig2(args, cdu, torch, peaks) if args.workload == "fig2" else run_dk(args, cdu, torch)
+            {"fig2": lambda: run_fig2(args, cdu, torch, peaks), "dk": lambda: run_dk(args, cdu, torch), "solve": lambda: run_solve(args, cdu, torch)}[args.workload]()
         return
     results = [run_config(c, args, cdu, torch, dist, peaks, world, rank, local, args.ckpt, opts_of(c)) for c in cfgs]
     if rank == 0:

@@ -146,15 +146,16 @@ cdu_status cdu_get_features(cdu_handle h, int32_t k, void* rp_bar, void* rd_bar,
 cdu_status cdu_rectify_rho(cdu_handle h, int32_t K, void* rho, int32_t io_on_host, void* cuda_stream);
 
 /* Vanilla COSMO run to tolerance (the baseline workload of PAPER.md Table 1): iterates in chunks of `check_every`
- * (<= K_max) steps through the kernels of cdu_forward with a fixed alpha and one rho per problem, starting at rho0. After
- * every chunk the OSQP-scaled residuals of App. E (L323) are read back - the only host synchronisation - and a problem is
- * converged when |rp_bar|_inf <= eps and |rd_bar|_inf <= eps. adapt_rho != 0: residual balancing (L349), rho <- rho
- * sqrt(|rp_bar|_inf / |rd_bar|_inf) clipped to [1e-6, 1e6] when the two differ by more than 5x (one scalar per problem:
- * per-row rho with the x1e3 equality scaling is not implemented). x0, s0, y0 (NULL = zeros) and x, s, y (may be NULL) as in
- * cdu_forward; iters_out [batch] (HOST): iterations at the first check that found the problem converged, or -(iterations
- * done) if it did not converge within max_iter; res_out [batch][2] (HOST): the last scaled residuals. */
+ * (<= K_max) steps through the kernels of cdu_forward with a fixed alpha and one base penalty rho_b per problem, starting at
+ * rho0; the equality (ZERO cone) rows run on eq_scale rho_b (COSMO / OSQP use 1e3, L306; eq_scale <= 0 or 1: every row on
+ * rho_b). After every chunk the OSQP-scaled residuals of App. E (L323) are read back - the only host synchronisation - and a
+ * problem is converged when |rp_bar|_inf <= eps and |rd_bar|_inf <= eps. adapt_rho != 0: residual balancing (L349), rho_b <-
+ * rho_b sqrt(|rp_bar|_inf / |rd_bar|_inf) clipped to [1e-6, 1e6] when the two differ by more than 5x. x0, s0, y0 (NULL = zeros)
+ * and x, s, y (may be NULL) as in cdu_forward; iters_out [batch] (HOST): iterations at the first check that found the problem
+ * converged, or -(iterations done) if it did not converge within max_iter; res_out [batch][2] (HOST): the last scaled
+ * residuals. */
 cdu_status cdu_solve(cdu_handle h, int32_t max_iter, int32_t check_every, double eps, double rho0, double alpha, double sigma,
-                     int32_t adapt_rho, const void* x0, const void* s0, const void* y0, void* x, void* s, void* y,
+                     int32_t adapt_rho, double eq_scale, const void* x0, const void* s0, const void* y0, void* x, void* s, void* y,
                      int32_t* iters_out, double* res_out, int32_t io_on_host, void* cuda_stream);
 
 typedef struct {

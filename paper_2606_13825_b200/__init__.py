@@ -90,7 +90,7 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.cdu_rectify_rho.restype = i32
     lib.cdu_rectify_rho.argtypes = [vp, i32, vp, i32, vp]
     lib.cdu_solve.restype = i32
-    lib.cdu_solve.argtypes = [vp, i32, i32, f64, f64, f64, f64, i32, vp, vp, vp, vp, vp, vp, vp, vp, i32, vp]
+    lib.cdu_solve.argtypes = [vp, i32, i32, f64, f64, f64, f64, i32, f64, vp, vp, vp, vp, vp, vp, vp, vp, i32, vp]
     lib.cdu_get_stats.restype = i32
     lib.cdu_get_stats.argtypes = [vp, C.POINTER(_Stats)]
     lib.cdu_get_iterate.restype = i32
@@ -259,13 +259,13 @@ class Handle:
         self._check(self.lib.cdu_rectify_rho(self.h, int(K), _ptr(rho), 0, _stream()))
         return rho
 
-    def solve(self, max_iter, check_every, eps, rho0=0.1, alpha=1.6, sigma=1e-6, adapt_rho=True, x0=None, s0=None, y0=None):
+    def solve(self, max_iter, check_every, eps, rho0=0.1, alpha=1.6, sigma=1e-6, adapt_rho=True, eq_scale=1.0, x0=None, s0=None, y0=None):
         """cdu_solve (device pointers) -> (x, s, y, iters [B] numpy int32, res [B, 2] numpy)."""
         torch = _torch()
         out = tuple(torch.empty(n, dtype=self.torch_dtype, device="cuda") for n in (self.N, self.M, self.M))
         iters = np.zeros(self.B, np.int32); res = np.zeros((self.B, 2), np.float64)
         self._check(self.lib.cdu_solve(self.h, int(max_iter), int(check_every), float(eps), float(rho0), float(alpha), float(sigma),
-                                       1 if adapt_rho else 0, _ptr(x0), _ptr(s0), _ptr(y0), _ptr(out[0]), _ptr(out[1]), _ptr(out[2]),
+                                       1 if adapt_rho else 0, float(eq_scale), _ptr(x0), _ptr(s0), _ptr(y0), _ptr(out[0]), _ptr(out[1]), _ptr(out[2]),
                                        iters.ctypes.data, res.ctypes.data, 0, _stream()))
         self.K, self.rho_mode = int(check_every), CDU_RHO_PER_PROBLEM
         return out[0], out[1], out[2], iters, res

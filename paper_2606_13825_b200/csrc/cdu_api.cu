@@ -90,11 +90,11 @@ cdu_status cdu_get_features(cdu_handle h, int32_t k, void* rp_bar, void* rd_bar,
 }
 
 cdu_status cdu_solve(cdu_handle h, int32_t max_iter, int32_t check_every, double eps, double rho0, double alpha, double sigma,
-                     int32_t adapt_rho, const void* x0, const void* s0, const void* y0, void* x, void* s, void* y, int32_t* iters_out,
+                     int32_t adapt_rho, double eq_scale, const void* x0, const void* s0, const void* y0, void* x, void* s, void* y, int32_t* iters_out,
                      double* res_out, int32_t io_on_host, void* cuda_stream) {
   if (!h) return CDU_EINVAL;
   DeviceGuard g(h->device);
-  return h->solve(max_iter, check_every, eps, rho0, alpha, sigma, adapt_rho, x0, s0, y0, x, s, y, iters_out, res_out, io_on_host,
+  return h->solve(max_iter, check_every, eps, rho0, alpha, sigma, adapt_rho, eq_scale, x0, s0, y0, x, s, y, iters_out, res_out, io_on_host,
                   reinterpret_cast<cudaStream_t>(cuda_stream));
 }
 

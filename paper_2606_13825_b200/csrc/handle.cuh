@@ -538,9 +538,11 @@ struct HandleT : cdu_handle_s {
                       void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st, const Extra* ex) override;
   cdu_status features(int k, void* rp_bar, void* rd_bar, void* delta_p, void* delta_d, void* scal, int host, cudaStream_t st) override;
   cdu_status add_extra(int k, double* Gz, const Extra* ex, int host, cudaStream_t st);
-  cdu_status solve(int max_iter, int check_every, double eps, double rho0, double alpha, double sigma, int adapt_rho, const void* x0,
-                   const void* s0, const void* y0, void* x, void* s, void* y, int* iters_out, double* res_out, int host, cudaStream_t st) override;
+  cdu_status solve(int max_iter, int check_every, double eps, double rho0, double alpha, double sigma, int adapt_rho, double eq_scale,
+                   const void* x0, const void* s0, const void* y0, void* x, void* s, void* y, int* iters_out, double* res_out, int host,
+                   cudaStream_t st) override;
   bool continue_from_last = false;
+  std::vector<uint8_t> h_rowkind; std::vector<long long> h_row_off;
   int n_rect = 0; const long long* rect_row0 = nullptr; const int* rect_rows = nullptr;
   cdu_status rectify(int K, void* rho, int host, cudaStream_t st) override;
   cdu_status stats(cdu_stats* out) override;
@@ -599,6 +601,7 @@ cdu_status HandleT<T, IT>::init(const cdu_problem* pr, const cdu_options* op, cu
     soc_off[b + 1] = (int)soc_start.size(); psdblk_off[b + 1] = (int)psd_p.size();
   }
   has_psd = !psd_p.empty();
+  h_rowkind = rowkind; h_row_off.assign(pr->row_off, pr->row_off + B + 1);     // cdu_solve: x eq_scale on the equality rows
   {   // blocks whose rows must share one rho (cdu_rectify_rho)
     std::vector<long long> r0v; std::vector<int> nr;
     for (int b = 0; b < B; ++b)
@@ -1056,13 +1059,14 @@ cdu_status HandleT<T, IT>::add_extra(int k, double* Gz, const Extra* ex, int hos
 // back (the only host sync) and, per problem, rho <- rho sqrt(|rp_bar|_inf / |rd_bar|_inf) when the two differ by more than 5x.
 template <typename T, typename IT>
 cdu_status HandleT<T, IT>::solve(int max_iter, int check_every, double eps, double rho0, double alpha, double sigma, int adapt_rho,
-                                 const void* x0, const void* s0, const void* y0, void* x, void* s, void* y, int* iters_out,
+                                 double eq_scale, const void* x0, const void* s0, const void* y0, void* x, void* s, void* y, int* iters_out,
                                  double* res_out, int host, cudaStream_t st) {
   if (check_every < 1 || check_every > K_max || max_iter < 1 || !(eps > 0.0) || !(rho0 > 0.0) || !(alpha > 0.0 && alpha < 2.0)) {
     err = "cdu_solve: bad arguments (1 <= check_every <= K_max, max_iter >= 1, eps > 0, rho0 > 0, alpha in (0,2))"; return CDU_EINVAL;
   }
   const int Kc = check_every;
-  std::vector<T> hr((size_t)Kc * B), ha((size_t)Kc * B, (T)alpha), sc((size_t)B * 3);
+  const bool rows = eq_scale > 0.0 && eq_scale != 1.0;      // per-row rho: rho_b on the cone rows, eq_scale rho_b on the equality rows (L306, L349)
+  std::vector<T> hr((size_t)Kc * (rows ? (size_t)Mtot : (size_t)B)), ha((size_t)Kc * B, (T)alpha), sc((size_t)B * 3);
   std::vector<double> rho(B, rho0);
   std::vector<int> done(B, -1);
   T *d_r = nullptr, *d_a = nullptr;
@@ -1074,9 +1078,16 @@ cdu_status HandleT<T, IT>::solve(int max_iter, int check_every, double eps, doub
   int it = 0;
   continue_from_last = true;
   while (it < max_iter) {
-    for (int k = 0; k < Kc; ++k) for (int b = 0; b < B; ++b) hr[(size_t)k * B + b] = (T)rho[b];
+    if (rows) {
+      for (int b = 0; b < B; ++b)
+        for (long long i = h_row_off[b]; i < h_row_off[b + 1]; ++i) hr[(size_t)i] = (T)(rho[b] * (h_rowkind[(size_t)i] == CDU_ZERO ? eq_scale : 1.0));
+      for (int k = 1; k < Kc; ++k) std::copy(hr.begin(), hr.begin() + Mtot, hr.begin() + (size_t)k * Mtot);
+    } else {
+      for (int k = 0; k < Kc; ++k) for (int b = 0; b < B; ++b) hr[(size_t)k * B + b] = (T)rho[b];
+    }
     CU_OK(cudaMemcpyAsync(d_r, hr.data(), hr.size() * sizeof(T), cudaMemcpyHostToDevice, st));
-    r = forward(Kc, d_r, CDU_RHO_PER_PROBLEM, sigma, d_a, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, st);
+    CU_OK(cudaStreamSynchronize(st));     // hr is rewritten for the next chunk
+    r = forward(Kc, d_r, rows ? CDU_RHO_PER_ROW : CDU_RHO_PER_PROBLEM, sigma, d_a, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, st);
     if (r != CDU_OK) break;
     it += Kc;
     r = features(Kc, nullptr, nullptr, nullptr, nullptr, sc.data(), 1, st);     // host read-back of [B][3] (synchronises)

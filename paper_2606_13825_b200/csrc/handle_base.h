@@ -19,7 +19,7 @@ struct cdu_handle_s {
   virtual cdu_status backward(const void* gx, const void* gs, const void* gy, void* g_rho, void* g_sigma, void* g_alpha,
                               void* g_x0, void* g_s0, void* g_y0, int host, cudaStream_t st, const Extra* ex = nullptr) = 0;
   virtual cdu_status solve(int max_iter, int check_every, double eps, double rho0, double alpha, double sigma, int adapt_rho,
-                           const void* x0, const void* s0, const void* y0, void* x, void* s, void* y, int* iters_out, double* res_out,
+                           double eq_scale, const void* x0, const void* s0, const void* y0, void* x, void* s, void* y, int* iters_out, double* res_out,
                            int host, cudaStream_t st) = 0;
   virtual cdu_status rectify(int K, void* rho, int host, cudaStream_t st) = 0;
   virtual cdu_status features(int k, void* rp_bar, void* rd_bar, void* delta_p, void* delta_d, void* scal, int host, cudaStream_t st) = 0;

@@ -45,3 +45,21 @@ def test_solver_reaches_the_closed_form_values(dtype):
         val = -(pr.q @ xs[off_n[b]:off_n[b + 1]])
         assert abs(val - want[b]) <= (2e-4 if dtype == "f64" else 2e-3) * want[b], (b, val, want[b], iters[b])
     h.close()
+
+
+def test_equality_rows_on_a_scaled_penalty():
+    """eq_scale = 1e3 (COSMO / OSQP practice): the equality rows run on 1e3 rho_b through the per-row mode; the
+    solver reaches the same closed-form values, and Lovasz theta(C5), whose edge constraints are equalities, in fewer iterations."""
+    probs = [maxcut_problem(complete_graph(5)), lovasz_problem(cycle_graph(5))]
+    want = [6.25, np.sqrt(5.0)]
+    its = {}
+    for es in (1.0, 1e3):
+        h = _handle(probs, "f64", 25)
+        x, s, y, iters, res = h.solve(20000, 25, 1e-6, rho0=0.1, alpha=1.6, adapt_rho=True, eq_scale=es)
+        assert np.all(iters > 0), (es, iters, res)
+        off_n = np.cumsum([0] + [p.n for p in probs]); xs = x.cpu().numpy()
+        for b, pr in enumerate(probs):
+            assert abs(-(pr.q @ xs[off_n[b]:off_n[b + 1]]) - want[b]) <= 1e-4 * want[b], (es, b)
+        its[es] = iters.copy()
+        h.close()
+    print("iterations to 1e-6, eq_scale 1 vs 1e3:", its)
