@@ -184,8 +184,8 @@ class Handle:
         want = "float32" if self.dtype == "f32" else "float64"
         if dt != want:
             raise ValueError(f"{name}: dtype {dt}, the handle computes in {want}")
-        if n != numel:
-            raise ValueError(f"{name}: {n} elements, expected {numel}")
+        if n < numel:
+            raise ValueError(f"{name}: {n} elements, at least {numel} are read")
         if not isinstance(t, np.ndarray) and t.is_cuda == bool(host):
             raise ValueError(f"{name}: {'host' if host else 'device'} tensor expected (host={host})")
 

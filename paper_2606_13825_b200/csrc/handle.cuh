@@ -396,7 +396,7 @@ struct PsdEngine {
       }
       if (s != CDU_OK) return s;
       pb(PC_LARGE_MISC, st);
-      k_large_finish_fwd<T><<<dim3(64, n_large), 256, 0, st>>>(tab, lt, H, k, Tm, Vt, lamL, A);
+      k_large_finish_fwd<T><<<dim3(LARGE_NCH, n_large), 256, 0, st>>>(tab, lt, H, k, Tm, Vt, lamL, A);
       pe(st);
       ++launches;
       CU_OK(cudaGetLastError());

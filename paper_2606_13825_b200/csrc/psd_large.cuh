@@ -244,9 +244,42 @@ __global__ void __launch_bounds__(256) k_large_post(const int* pvec, const int* 
   }
 }
 
+// svec of the symmetric part of a p x p row-major matrix M, tile by tile: 32 x 32 tiles of the lower triangle (tile row bi >=
+// tile column bj). The tile and its mirror image are read coalesced into shared memory; element (R, Cc <= R) is
+// 1/2 (M[R][Cc] + M[Cc][R]) (x sqrt 2 off the diagonal) and goes to f(svec index, value) with the index contiguous along the
+// lanes (idx = R (R + 1) / 2 + Cc), so whatever f reads or writes at that index is coalesced too. CTA ch of nch.
+template <typename T, typename F>
+__device__ __forceinline__ void svec_of_sym_tiles(int p, const T* M, int ch, int nch, F f) {
+  __shared__ T ta[32][33];
+  __shared__ T tb[32][33];
+  const int ntr = (p + 31) >> 5, ntiles = ntr * (ntr + 1) / 2;
+  const int lane = threadIdx.x & 31, wy = threadIdx.x >> 5, nwy = blockDim.x >> 5;
+  for (int tl = ch; tl < ntiles; tl += nch) {
+    int bi = (int)((sqrt(8.0 * tl + 1.0) - 1.0) * 0.5);
+    while (bi * (bi + 1) / 2 > tl) --bi;
+    while ((bi + 1) * (bi + 2) / 2 <= tl) ++bi;
+    const int bj = tl - bi * (bi + 1) / 2;
+    for (int rr = wy; rr < 32; rr += nwy) {
+      const int R = bi * 32 + rr, Cc = bj * 32 + lane;         // tile (bi, bj): row R, column Cc
+      ta[rr][lane] = (R < p && Cc < p) ? M[(long long)R * p + Cc] : (T)0;
+      const int Rm = bj * 32 + rr, Cm = bi * 32 + lane;        // tile (bj, bi): row Rm, column Cm
+      tb[rr][lane] = (Rm < p && Cm < p) ? M[(long long)Rm * p + Cm] : (T)0;
+    }
+    __syncthreads();
+    for (int rr = wy; rr < 32; rr += nwy) {
+      const int R = bi * 32 + rr, Cc = bj * 32 + lane;
+      if (R < p && Cc <= R) {
+        const double v = (R == Cc) ? (double)ta[rr][lane] : 0.5 * ((double)ta[rr][lane] + (double)tb[lane][rr]) * 1.41421356237309504880;
+        f(svec_idx(Cc, R), v);
+      }
+    }
+    __syncthreads();
+  }
+}
+
 // s+ = svec(Tm), y+ = rho (s+ - w); also copies Vt, lam into the checkpoint store.
 template <typename T>
-__global__ void __launch_bounds__(1024) k_large_finish_fwd(PsdTab tab, LargeTab lt, Hyper<T> H, int k, const T* Tm,
+__global__ void __launch_bounds__(256) k_large_finish_fwd(PsdTab tab, LargeTab lt, Hyper<T> H, int k, const T* Tm,
                                                            const T* Vt, const T* lam, PsdFwdArgs A) {
   const int lb = blockIdx.y, blk = lt.gblk[lb];
   const int p = tab.p[blk];
@@ -258,16 +291,12 @@ __global__ void __launch_bounds__(1024) k_large_finish_fwd(PsdTab tab, LargeTab 
   T* U = reinterpret_cast<T*>(A.Ustore) + tab.uoff[blk];
   T* L = reinterpret_cast<T*>(A.Lstore) + tab.loff[blk];
   const long long stride = (long long)gridDim.x * blockDim.x, t0 = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  for (long long t = t0; t < (long long)p * p; t += stride) {
-    const int r = (int)(t / p), c = (int)(t - (long long)r * p);
-    if (U != Vt + lt.moff[lb]) U[t] = Vt[lt.moff[lb] + t];
-    if (r <= c) {
-      const double o = (r == c) ? (double)tm[t] : 0.5 * ((double)tm[t] + (double)tm[(long long)c * p + r]) * 1.41421356237309504880;
-      const int idx = svec_idx(r, c);
-      s1[idx] = o;
-      y1[idx] = rho * (o - w[idx]);
-    }
-  }
+  if (U != Vt + lt.moff[lb])
+    for (long long t = t0; t < (long long)p * p; t += stride) U[t] = Vt[lt.moff[lb] + t];
+  svec_of_sym_tiles<T>(p, tm, (int)blockIdx.x, (int)gridDim.x, [&](int idx, double o) {
+    s1[idx] = o;
+    y1[idx] = rho * (o - w[idx]);
+  });
   for (long long t = t0; t < p; t += stride) L[t] = lam[lt.voff[lb] + t];
 }
 
@@ -298,20 +327,13 @@ __global__ void __launch_bounds__(256) k_large_finish_bwd(PsdTab tab, LargeTab l
   const double *w = A.W + row0, *yk = A.Yk + row0, *s1 = A.S1 + row0, *gy = A.Gy + row0;
   double* gw = A.GW + row0;
   double acc[2] = {0.0, 0.0};
-  const long long tot = (long long)p * p;
-  const long long t0 = tot * ch / nch, t1 = tot * (ch + 1) / nch;
-  for (long long t = t0 + threadIdx.x; t < t1; t += blockDim.x) {
-    const int r = (int)(t / p), c = (int)(t - (long long)r * p);
-    if (r <= c) {
-      const double ov = (r == c) ? (double)o[t] : 0.5 * ((double)o[t] + (double)o[(long long)c * p + r]) * 1.41421356237309504880;
-      const int idx = svec_idx(r, c);
-      const double gyv = gy[idx];
-      const double g = -rho * gyv + ov;
-      gw[idx] = g;
-      acc[0] += gyv * (s1[idx] - w[idx]);
-      acc[1] += g * yk[idx];
-    }
-  }
+  svec_of_sym_tiles<T>(p, o, ch, nch, [&](int idx, double ov) {
+    const double gyv = gy[idx];
+    const double g = -rho * gyv + ov;
+    gw[idx] = g;
+    acc[0] += gyv * (s1[idx] - w[idx]);
+    acc[1] += g * yk[idx];
+  });
   block_sum<2>(acc, sh);
   if (threadIdx.x == 0) {
     scr[((size_t)lb * LARGE_NCH + ch) * 2] = acc[0]; scr[((size_t)lb * LARGE_NCH + ch) * 2 + 1] = acc[1];

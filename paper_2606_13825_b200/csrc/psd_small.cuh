@@ -308,9 +308,71 @@ __device__ int jacobi_planes(int pe, const JacobiWs<T>& w, double* shred, int ma
 // threads along j. When B is read transposed (sbk == 1: the rows of B' are k-contiguous with an even stride) the
 // threads of a warp would hit the same few banks at every k; they then walk k skewed by their tile column, which
 // makes the B loads and the (no longer broadcast) A loads conflict free.
+// fp32: the same product on the tensor cores (warp-level mma.sync m16n8k8, 3xTF32 split as in psd_bjacobi.cuh). One warp per
+// 16 x 16 tile of C; out-of-range rows / columns / k read element 0 with weight 0. The tensor core adds into its accumulator
+// with truncation, so the leading term is accumulated over 32 k at a time and the chunks are added round-to-nearest
+// (gemm_tc.cuh has the measurement that made this necessary). ~2x the FMA version at pe = 100 (cfg4).
+__device__ __forceinline__ void sg_split(float a, uint32_t& hi, uint32_t& lo) {
+  hi = (__float_as_uint(a) + 0x1000u) & 0xffffe000u;
+  lo = (__float_as_uint(a - __uint_as_float(hi)) + 0x1000u) & 0xffffe000u;
+}
+__device__ __forceinline__ void sg_mma(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3]) : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ void smem_gemm_tc(int pe, const float* A, int sai, int sak, const float* B, int sbk, int sbj, float* C,
+                                             int ldc) {
+  const int warp = threadIdx.x >> 5, nw = blockDim.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  const int nt = (pe + 15) >> 4;
+  for (int tile = warp; tile < nt * nt; tile += nw) {
+    const int i0 = (tile / nt) * 16, j0 = (tile % nt) * 16;
+    float sum[2][4] = {}, accS[2][4] = {};
+    for (int kc = 0; kc < pe; kc += 32) {
+      float accM[2][4] = {};
+#pragma unroll
+      for (int kk = 0; kk < 32; kk += 8) {
+        const int k0 = kc + kk;
+        if (k0 >= pe) break;
+        uint32_t ah[4], al[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {      // a0 (g, t), a1 (g + 8, t), a2 (g, t + 4), a3 (g + 8, t + 4)
+          const int i = i0 + g + 8 * (e & 1), k = k0 + t + 4 * (e >> 1);
+          const float v = (i < pe && k < pe) ? A[i * sai + k * sak] : 0.f;
+          sg_split(v, ah[e], al[e]);
+        }
+#pragma unroll
+        for (int n = 0; n < 2; ++n) {
+          uint32_t bh[2], bl[2];
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {    // b0 (k = t, n = g), b1 (k = t + 4, n = g)
+            const int k = k0 + t + 4 * e, j = j0 + 8 * n + g;
+            const float v = (k < pe && j < pe) ? B[k * sbk + j * sbj] : 0.f;
+            sg_split(v, bh[e], bl[e]);
+          }
+          sg_mma(accS[n], al, bh[0], bh[1]);
+          sg_mma(accS[n], ah, bl[0], bl[1]);
+          sg_mma(accM[n], ah, bh[0], bh[1]);
+        }
+      }
+#pragma unroll
+      for (int n = 0; n < 2; ++n)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) sum[n][e] += accM[n][e];
+    }
+#pragma unroll
+    for (int n = 0; n < 2; ++n)
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {        // c0 (g, 2t), c1 (g, 2t + 1), c2 (g + 8, 2t), c3 (g + 8, 2t + 1)
+        const int i = i0 + g + 8 * (e >> 1), j = j0 + 8 * n + 2 * t + (e & 1);
+        if (i < pe && j < pe) C[i * ldc + j] = sum[n][e] + accS[n][e];
+      }
+  }
+}
+
 template <typename T>
 __device__ __forceinline__ void smem_gemm(int pe, const T* A, int sai, int sak, const T* B, int sbk, int sbj, T* C,
                                           int ldc) {
+  if constexpr (sizeof(T) == 4) { smem_gemm_tc(pe, A, sai, sak, B, sbk, sbj, C, ldc); return; }
   const int h = pe >> 1;
   const bool skewed = (sbk == 1 && sbj != 1 && sak == 1);
   for (int t = threadIdx.x; t < h * h; t += blockDim.x) {
