@@ -754,8 +754,10 @@ k_bjacobi_tc2(int lb0, int C, const int* pvec, const long long* moff, const int*
           uint32_t* Qh = reinterpret_cast<uint32_t*>(part); uint32_t* Ql = Qh + RP * LQ;    // the Gram partials are spent
           for (int e = threadIdx.x; e < RP * RP; e += 512) { const int o = (e >> 5) * LQ + (e & 31); split_fast(Q[o] - ((e >> 5) == (e & 31) ? 1.f : 0.f), Qh[o], Ql[o]); }
           __syncthreads();
+          BW_T(9);
           apply_mma(Qh, Ql, X, ldx, ks, p);
           __syncthreads();
+          BW_T(10);
           store_pair(g, p, bi, bj2, X, ldx);
           if (threadIdx.x == 0) atomicMax(reinterpret_cast<unsigned*>(rf) + sweep, __float_as_uint(sqrtf(mx2)));
           BW_CNT(7, 1); BW_CNT(8, __popc(active));
