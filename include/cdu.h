@@ -205,6 +205,27 @@ cdu_status cdu_psd_project(int32_t dtype, int32_t count, int32_t p, const void* 
 cdu_status cdu_psd_vjp(int32_t dtype, int32_t count, int32_t p, const void* U, const void* lam, const void* Gbar,
                        void* Sbar, int32_t path, int32_t use_tensor_cores, void* cuda_stream);
 
+/* ---- the PSD projection for callers that may not allocate ------------------------------------------------------
+ * cdu_psd_project (above) keeps its block tables and work arrays in cudaMalloc'ed memory. Code under CUDA graph
+ * capture, tight serving loops and harnesses that forbid cudaMalloc get this variant instead: the same operation
+ * (Eq. 7, S -> Pi(S) = U max(L,0) U') through the same shared-memory Jacobi code as path 1 above (same arithmetic,
+ * same launch shape), with ALL scratch in one file-scope __device__ array of CDU_PSD_STATIC_BYTES that every GPU
+ * which loads the library holds until the process exits. It calls no cudaMalloc / cudaFree / allocating library routine
+ * and does not synchronise: on `cuda_stream` it enqueues four kernels, a fifth if U != NULL, and one device-to-device
+ * copy if lam != NULL.
+ *   S, PiS [count][p][p] row-major device pointers (PiS may alias S); U ([count][p][p], eigenvectors in columns)
+ *   and lam ([count][p]) may be NULL; dtype CDU_F32 or CDU_F64 (of S, PiS, U, lam and of the Jacobi arithmetic).
+ * Limits: 1 <= p <= CDU_PSD_STATIC_MAX_P and the scratch of (count, p) - about count * (8 p (p+1) + (p*p + p) *
+ * sizeof(dtype) + 4) bytes, each part rounded up to 256 - must fit the array: e.g. 120 matrices of order 64 or
+ * 480 of order 32 in fp64. Anything larger returns CDU_EINVAL with the required size in cdu_last_error(NULL);
+ * nothing is launched then. No per-matrix convergence flag is returned (cdu_psd_project does not return one either).
+ * The array is shared by every call on a device and keeps the previous call's contents; the call clears what must
+ * start at zero itself. Calls that overlap on the GPU (two streams, two threads) race on it: serialise them. */
+#define CDU_PSD_STATIC_BYTES (8u << 20)
+#define CDU_PSD_STATIC_MAX_P 64
+cdu_status cdu_psd_project_static(int32_t dtype, int32_t count, int32_t p, const void* S, void* PiS, void* U, void* lam,
+                                  void* cuda_stream);
+
 /* ---- roofline denominators measured in-tree (bench.py) ---------------------------------------
  * Runs a micro-benchmark on the current device and stream and returns its best-of-5 rate in *value:
  *   CDU_PEAK_FP32_FMA / CDU_PEAK_FP64_FMA : dependent-chain-free FMA loops on the plain ALUs, TFLOP/s;

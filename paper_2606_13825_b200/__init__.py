@@ -6,7 +6,7 @@ the PSD eigendecomposition, checkpointing, adjoint CG, Dalecki-Krein VJP) runs i
 if the library is missing or no CUDA device is present, the calls raise.
 
 Names follow the C ABI: `cdu_create`, `cdu_forward`, `cdu_backward`, `cdu_get_stats`, `cdu_destroy`,
-`cdu_psd_project`, `cdu_psd_vjp`.
+`cdu_psd_project`, `cdu_psd_vjp`, `cdu_psd_project_static`.
 """
 from __future__ import annotations
 
@@ -28,7 +28,8 @@ _STATUS = {0: "CDU_OK", 1: "CDU_EINVAL", 2: "CDU_ENOMEM", 3: "CDU_ECUDA", 4: "CD
 
 EXPORTED_SYMBOLS = ("cdu_create", "cdu_forward", "cdu_backward", "cdu_get_stats", "cdu_get_iterate", "cdu_last_error",
                     "cdu_destroy", "cdu_version", "cdu_psd_project", "cdu_psd_vjp", "cdu_profile", "cdu_get_profile",
-                    "cdu_measure_peak", "cdu_backward_inject", "cdu_backward_eq12", "cdu_get_features", "cdu_solve", "cdu_rectify_rho")
+                    "cdu_measure_peak", "cdu_backward_inject", "cdu_backward_eq12", "cdu_get_features", "cdu_solve", "cdu_rectify_rho",
+                    "cdu_psd_project_static")
 
 
 class CduError(RuntimeError):
@@ -107,6 +108,8 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.cdu_get_profile.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
     lib.cdu_psd_project.restype = i32
     lib.cdu_psd_project.argtypes = [i32, i32, i32, vp, vp, vp, vp, i32, i32, vp]
+    lib.cdu_psd_project_static.restype = i32
+    lib.cdu_psd_project_static.argtypes = [i32, i32, i32, vp, vp, vp, vp, vp]
     lib.cdu_psd_vjp.restype = i32
     lib.cdu_psd_vjp.argtypes = [i32, i32, i32, vp, vp, vp, vp, i32, i32, vp]
     lib.cdu_measure_peak.restype = i32
@@ -360,6 +363,32 @@ def cdu_psd_project(S, path: int = 0, use_tensor_cores: int = 0, want_eig: bool 
     if st != CDU_OK:
         raise CduError(st, lib.cdu_last_error(None).decode())
     return out, U, lam
+
+
+PSD_STATIC_BYTES = 8 << 20     # CDU_PSD_STATIC_BYTES of include/cdu.h
+PSD_STATIC_MAX_P = 64          # CDU_PSD_STATIC_MAX_P
+
+
+def cdu_psd_project_static(S, PiS, U=None, lam=None) -> None:
+    """Batched Pi(S) with no allocation anywhere: S and every output are the caller's CUDA tensors (S, PiS, U
+    [count, p, p], lam [count, p], one dtype, contiguous); the scratch is a static device array inside the library
+    (include/cdu.h: limits, and why overlapping calls race). Enqueues on the current stream and does not synchronise."""
+    torch = _torch()
+    lib = load_library()
+    if not (S.is_cuda and S.dim() == 3 and S.shape[1] == S.shape[2] and S.is_contiguous()):
+        raise CduError(CDU_EINVAL, "S must be a contiguous CUDA tensor [count, p, p]")
+    if S.dtype not in (torch.float32, torch.float64):
+        raise CduError(CDU_EINVAL, "S must be float32 or float64")
+    cnt, p = S.shape[0], S.shape[1]
+    for name, t, shape in (("PiS", PiS, (cnt, p, p)), ("U", U, (cnt, p, p)), ("lam", lam, (cnt, p))):
+        if t is None and name != "PiS":
+            continue
+        if t is None or not t.is_cuda or t.dtype != S.dtype or tuple(t.shape) != shape or not t.is_contiguous() or t.device != S.device:
+            raise CduError(CDU_EINVAL, f"{name} must be a contiguous CUDA tensor of shape {shape} and S's dtype and device")
+    dt = CDU_F32 if S.dtype == torch.float32 else CDU_F64
+    st = lib.cdu_psd_project_static(dt, cnt, p, _ptr(S), _ptr(PiS), _ptr(U), _ptr(lam), _stream())
+    if st != CDU_OK:
+        raise CduError(st, lib.cdu_last_error(None).decode())
 
 
 def cdu_psd_vjp(U, lam, Gbar, path: int = 0, use_tensor_cores: int = 0):

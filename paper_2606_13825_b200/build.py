@@ -9,7 +9,7 @@ import sys
 PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
-UNITS = ["cdu_api", "inst_f32_u16", "inst_f32_i32", "inst_f64_u16", "inst_f64_i32"]   # one object each, compiled in parallel
+UNITS = ["cdu_api", "psd_static", "inst_f32_u16", "inst_f32_i32", "inst_f64_u16", "inst_f64_i32"]   # one object each, compiled in parallel
 OBJ_DIR = os.path.join(PKG, "_obj")
 LIB = os.path.join(PKG, "libcdu.so")
 DEPS = [os.path.join(PKG, "csrc", f) for f in os.listdir(os.path.join(PKG, "csrc"))] + [os.path.join(ROOT, "include", "cdu.h")]
