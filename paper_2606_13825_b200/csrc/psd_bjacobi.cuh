@@ -500,45 +500,46 @@ __device__ __forceinline__ void split_fast(float a, uint32_t& hi, uint32_t& lo) 
 }
 
 // One cyclic sweep of two-sided Jacobi on W (rounds outside `active` skipped), Q = product of the rotations
-// (row i of Q: the combination of old rows that makes new row i). One barrier per round. Warps 0-7: thread (a, b) owns
-// the 2x2 block (row pair a, column pair b) of W; warps 8-11: thread (a, c) owns columns 4c..4c+3 of the row pair a of
-// Q. Lane l of every working warp derives the rotation of pair l mod 16 from the current W; the rotation of the own
-// row pair comes by shuffle.
+// (row i of Q: the combination of old rows that makes new row i). Warps 0-7 work, one named barrier per round among
+// them; thread (a, b) owns the 2x2 block (row pair a, column pair b) of W and columns 2b, 2b+1 of the row pair a of Q.
+// It derives BOTH of its rotations (pair a for the rows, pair b for the columns) from the current W itself: 32-fold
+// redundant arithmetic, but no shuffle and every load of a round issues at its top, and the round is a dependent chain
+// (load, rotation, update, store, barrier: 440 cycles against 530 with one rotation per thread and shuffles, measured).
+// The pair indices of the next active round are fetched while the rotations are computed. Ends with a CTA barrier.
 __device__ __forceinline__ void inner_sweep(float* W0, float* W1, float* Q, float thr2, unsigned active, const unsigned char* ptab) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   for (int e = tid; e < RP * RP; e += 512) { const int i = e >> 5, j = e & 31; Q[i * LQ + j] = (i == j) ? 1.f : 0.f; }
   __syncthreads();
-  if (warp >= 12) {                       // nothing to do but keep the barrier count
-    for (int r = 0; r < RP - 1; ++r) if ((active >> r) & 1u) __syncthreads();
-    return;
-  }
-  const bool wthread = warp < 8;
-  const int b = lane & 15;
-  const int a = wthread ? 2 * warp + (lane >> 4) : 4 * (warp - 8) + (lane >> 3);
-  const int c4 = 4 * (lane & 7);
-  float* Wc = W0; float* Wn = W1;
-  for (int r = 0; r < RP - 1; ++r) {
-    if (!((active >> r) & 1u)) continue;
-    int ib, jb;
-    inner_pair(r, b, ptab, ib, jb);
-    float csB, snB;
-    rot_cs(Wc[ib * LW + ib], Wc[jb * LW + jb], Wc[ib * LW + jb], thr2, csB, snB);
-    const float csA = __shfl_sync(0xffffffffu, csB, a), snA = __shfl_sync(0xffffffffu, snB, a);
-    const int ia = __shfl_sync(0xffffffffu, ib, a), ja = __shfl_sync(0xffffffffu, jb, a);
-    if (wthread) {
+  if (warp < 8) {
+    const int b = lane & 15, a = 2 * warp + (lane >> 4);
+    float* Wc = W0; float* Wn = W1;
+    int r = __ffs(active) - 1;           // active != 0 (caller)
+    int ib, jb, ia, ja;
+    inner_pair(r, b, ptab, ib, jb); inner_pair(r, a, ptab, ia, ja);
+    while (r >= 0) {
+      const unsigned rest = active & ~((2u << r) - 1u);
+      const int rn = rest ? __ffs(rest) - 1 : -1;
+      const float bii = Wc[ib * LW + ib], bjj = Wc[jb * LW + jb], bij = Wc[ib * LW + jb];
+      const float aii = Wc[ia * LW + ia], ajj = Wc[ja * LW + ja], aij = Wc[ia * LW + ja];
       const float p0 = Wc[ia * LW + ib], q0 = Wc[ia * LW + jb], r0 = Wc[ja * LW + ib], s0 = Wc[ja * LW + jb];
+      float2* xi = reinterpret_cast<float2*>(Q + ia * LQ + 2 * b); float2* xj = reinterpret_cast<float2*>(Q + ja * LQ + 2 * b);
+      const float2 x = *xi, y = *xj;
+      int ibn = 0, jbn = 0, ian = 0, jan = 0;
+      if (rn >= 0) { inner_pair(rn, b, ptab, ibn, jbn); inner_pair(rn, a, ptab, ian, jan); }
+      float csB, snB, csA, snA;
+      rot_cs(bii, bjj, bij, thr2, csB, snB);
+      rot_cs(aii, ajj, aij, thr2, csA, snA);
       const float p1 = csA * p0 - snA * r0, r1 = snA * p0 + csA * r0, q1 = csA * q0 - snA * s0, s1 = snA * q0 + csA * s0;
       Wn[ia * LW + ib] = csB * p1 - snB * q1; Wn[ia * LW + jb] = snB * p1 + csB * q1;
       Wn[ja * LW + ib] = csB * r1 - snB * s1; Wn[ja * LW + jb] = snB * r1 + csB * s1;
-    } else {
-      float4* xi = reinterpret_cast<float4*>(Q + ia * LQ + c4); float4* xj = reinterpret_cast<float4*>(Q + ja * LQ + c4);
-      const float4 x = *xi, y = *xj;
-      *xi = make_float4(csA * x.x - snA * y.x, csA * x.y - snA * y.y, csA * x.z - snA * y.z, csA * x.w - snA * y.w);
-      *xj = make_float4(snA * x.x + csA * y.x, snA * x.y + csA * y.y, snA * x.z + csA * y.z, snA * x.w + csA * y.w);
+      *xi = make_float2(csA * x.x - snA * y.x, csA * x.y - snA * y.y);
+      *xj = make_float2(snA * x.x + csA * y.x, snA * x.y + csA * y.y);
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      float* t2 = Wc; Wc = Wn; Wn = t2;
+      r = rn; ib = ibn; jb = jbn; ia = ian; ja = jan;
     }
-    __syncthreads();
-    float* t2 = Wc; Wc = Wn; Wn = t2;
   }
+  __syncthreads();
 }
 
 __device__ __forceinline__ void mma_tf32(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
