@@ -11,7 +11,7 @@
 //   * a row needs xt (or lam) of its column, which another thread (possibly another CTA) owns: it is recomputed from
 //     the column's entries of A' (cdu_create admits the path only if no column holds more than DIAG_MAXCOL entries);
 //   * per-problem dot products (g_rho, g_alpha, g_sigma and the two partials handed from the pre to the post phase):
-//     block sums into part[chunk][], the last CTA of a problem to arrive (ticket) adds them in chunk order, so the
+//     block sums into part[chunk][], the last CTA of a problem to arrive (ticket) adds them in a fixed order, so the
 //     results are bit-reproducible.
 #pragma once
 #include "lin.cuh"
@@ -19,7 +19,7 @@
 namespace cdu {
 
 constexpr int DIAG_MAXCOL = 8;        // admitted entries per column of A
-constexpr int DIAG_CHUNK = 2048;      // local indices per CTA
+constexpr int DIAG_CHUNK = 512;       // local indices per CTA (two per thread: the gathers are dependent loads, parallelism hides them)
 constexpr int DIAG_THREADS = 256;
 
 template <typename T, typename IT>
@@ -63,7 +63,7 @@ struct DiagCtx {   // one problem as seen by one thread
 };
 
 // Sum of NV doubles over the chunks of a problem: every CTA leaves its block sums in part[chunk]; the last one to arrive
-// adds the problem's chunks in order and returns true (to all its threads) with the totals in v.
+// adds the problem's chunks in a fixed order and returns true (to all its threads) with the totals in v.
 template <int NV>
 __device__ __forceinline__ bool diag_problem_sum(double (&v)[NV], double* sh, double* part, unsigned* ticket, int chunk0, int nch,
                                                  int chunk) {
@@ -79,12 +79,15 @@ __device__ __forceinline__ bool diag_problem_sum(double (&v)[NV], double* sh, do
   }
   __syncthreads();
   if (!is_last) return false;
+  // thread t adds the chunks t, t + blockDim.x, ... and the block sums those: a fixed order, whatever CTA arrives last
 #pragma unroll
-  for (int i = 0; i < NV; ++i) {
-    double t = 0.0;
-    for (int c = 0; c < nch; ++c) t += __ldcg(part + (size_t)(chunk0 + c) * 4 + i);
-    v[i] = t;
+  for (int i = 0; i < NV; ++i) v[i] = 0.0;
+  for (int c = threadIdx.x; c < nch; c += blockDim.x) {
+#pragma unroll
+    for (int i = 0; i < NV; ++i) v[i] += __ldcg(part + (size_t)(chunk0 + c) * 4 + i);
   }
+  __syncthreads();
+  block_sum<NV>(v, sh);
   return true;
 }
 

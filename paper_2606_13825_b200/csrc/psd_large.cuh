@@ -33,7 +33,7 @@ struct LargeTab {
 //              (capped by ||S||_F): between ADMM iterates the difference is small, so mu ~ 1.5 ||S||_2 instead of
 //              ~ sqrt(p) ||S||_2, and the rounding error of the Jacobi sweeps (eps (mu + ||S||_2)) shrinks with it.
 // shift >= 1 also refreshes wprev.
-constexpr int LARGE_NCH = 32;   // CTAs per block in the chunked glue kernels
+constexpr int LARGE_NCH = 144;  // CTAs per block in the chunked glue kernels (one 32 x 32 tile each up to order 512: these kernels are latency bound, so many small CTAs)
 
 // Chunked over gridDim.x CTAs per block (blockIdx.y = block). The reductions (||svec||^2, ||svec - wprev||^2) go
 // through per-chunk partials in `scr` ([nblk][LARGE_NCH][2] doubles + one ticket per block in `tick`); the last CTA
