@@ -609,9 +609,16 @@ __device__ __forceinline__ void gram_mma(const float* X, int ldx, int ks, float*
 }
 
 
-// X' = X + E X, E = Q - I (hi / lo parts pre-split in shared memory), for this warp's column slice, in place. The tensor core adds into its accumulators with truncation; on Q X that
+// X' = X + E X, E = Q - I (hi / lo parts pre-split in shared memory, fragment order), for this warp's column slice, in place. The tensor core adds into its accumulators with truncation; on Q X that
 // is a bias of ~1e-7 per block round on every row, which BPTT through 200 iterations amplified to wrong gradients (measured:
 // cfg5 gradient error 0.48). On E X it is 1e-7 of the correction only, and the correction is small once the sweeps converge.
+// Element (i, k) of E -> its place in the fragment-ordered copies [m tile][k step][lane][4] that apply_mma reads: a thread's
+// four A registers of one mma are one 16-byte piece, a warp's load is 512 contiguous bytes (16 conflict-free LDS.128 per
+// thread instead of 32 LDS.64 that cost 900 cycles more per visit, measured).
+__device__ __forceinline__ int frag_pos(int i, int k) {
+  const int mt = i >> 4, r = i & 15, g = r & 7, hf = r >> 3, ks = k >> 3, kk = k & 7, t = kk >> 1, wh = kk & 1;
+  return ((mt * 4 + ks) * 32 + 4 * g + t) * 4 + hf + 2 * wh;
+}
 __device__ __forceinline__ void apply_mma(const uint32_t* Qh, const uint32_t* Ql, float* X, int ldx, int ns, int p) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   uint32_t qh[2][4][4], ql[2][4][4];      // [m tile][k step][fragment register]; k slot t <-> row 2t, slot t+4 <-> row 2t+1
@@ -619,11 +626,10 @@ __device__ __forceinline__ void apply_mma(const uint32_t* Qh, const uint32_t* Ql
   for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
     for (int ks = 0; ks < 4; ++ks) {
-      const int o0 = (16 * mt + g) * LQ + 8 * ks + 2 * t, o1 = o0 + 8 * LQ;
-      const uint2 uh = *reinterpret_cast<const uint2*>(Qh + o0), vh = *reinterpret_cast<const uint2*>(Qh + o1);
-      const uint2 ul = *reinterpret_cast<const uint2*>(Ql + o0), vl = *reinterpret_cast<const uint2*>(Ql + o1);
-      qh[mt][ks][0] = uh.x; qh[mt][ks][1] = vh.x; qh[mt][ks][2] = uh.y; qh[mt][ks][3] = vh.y;
-      ql[mt][ks][0] = ul.x; ql[mt][ks][1] = vl.x; ql[mt][ks][2] = ul.y; ql[mt][ks][3] = vl.y;
+      const uint4 h = *reinterpret_cast<const uint4*>(Qh + ((mt * 4 + ks) * 32 + lane) * 4);
+      const uint4 l = *reinterpret_cast<const uint4*>(Ql + ((mt * 4 + ks) * 32 + lane) * 4);
+      qh[mt][ks][0] = h.x; qh[mt][ks][1] = h.y; qh[mt][ks][2] = h.z; qh[mt][ks][3] = h.w;
+      ql[mt][ks][0] = l.x; ql[mt][ks][1] = l.y; ql[mt][ks][2] = l.z; ql[mt][ks][3] = l.w;
     }
   for (int n0 = warp * ns; n0 < (warp + 1) * ns; n0 += 8) {
     if (n0 >= p) break;
@@ -753,7 +759,7 @@ k_bjacobi_tc2(int lb0, int C, const int* pvec, const long long* moff, const int*
           inner_sweep(W, W1, Q, thr2, active, ptab);
           BW_T(3);
           uint32_t* Qh = reinterpret_cast<uint32_t*>(part); uint32_t* Ql = Qh + RP * LQ;    // the Gram partials are spent
-          for (int e = threadIdx.x; e < RP * RP; e += 512) { const int o = (e >> 5) * LQ + (e & 31); split_fast(Q[o] - ((e >> 5) == (e & 31) ? 1.f : 0.f), Qh[o], Ql[o]); }
+          for (int e = threadIdx.x; e < RP * RP; e += 512) { const int i = e >> 5, k = e & 31, o = frag_pos(i, k); split_fast(Q[i * LQ + k] - (i == k ? 1.f : 0.f), Qh[o], Ql[o]); }
           __syncthreads();
           BW_T(9);
           apply_mma(Qh, Ql, X, ldx, ks, p);
