@@ -365,7 +365,7 @@ struct PsdEngine {
     else s = gemm(Vt, 0, T2, 0, G, nullptr, 0, st);
     if (s != CDU_OK) return s;
     pb(PC_LARGE_MISC, st);
-    k_large_rayleigh<T><<<dim3(16, n_large), 256, 0, st>>>(lt.pvec, lt.moff, lt.voff, G, Vt, lamL, cur_need);
+    k_large_rayleigh<T><<<dim3(64, n_large), 256, 0, st>>>(lt.pvec, lt.moff, lt.voff, G, Vt, lamL, cur_need);
     ++launches;
     k_large_post<T><<<n_large, 256, 0, st>>>(lt.pvec, lt.voff, lamL, scaleL, lmaxL, mu, cur_need, need);
     pe(st);
