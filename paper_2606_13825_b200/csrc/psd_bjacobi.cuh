@@ -787,6 +787,9 @@ k_bjacobi_tc2(int lb0, int C, const int* pvec, const long long* moff, const int*
         BW_T(1);
         unsigned active;
         const float mx2 = gram_reduce(part, W, red, rtab, lim2, active);
+        // block-cyclic ordering: the pairs inside a block are rotated at the block's visit of round 0 (every block has one), the
+        // other 30 visits of a sweep rotate the 256 cross pairs only; what those leave inside a block is of second order
+        if (r > 0) active &= 0xffffu;
         BW_T(2);
         if (active) {
           inner_sweep(W, W1, Q, thr2, active, ptab);
