@@ -441,7 +441,7 @@ __device__ __forceinline__ void inner_pair(int r, int q, const unsigned char* pt
 // W = sum of the 16 partials (fixed order). Returns max_{i<j} w_ij^2 / (w_ii w_jj) and the mask of inner rounds that
 // hold a pair with that ratio above lim2.
 __device__ __forceinline__ float gram_reduce(const float* part, float* W, unsigned* red, const unsigned char* rtab, float lim2,
-                                             unsigned& active) {
+                                             unsigned& active, bool cross_only = false) {
   const int tid = threadIdx.x;
   if (tid < 384) {     // (i, j pair): rows 0-15 all 16 column pairs, rows 16-31 column pairs 8-15 (the rest by symmetry)
     int i, jp;
@@ -451,6 +451,9 @@ __device__ __forceinline__ float gram_reduce(const float* part, float* W, unsign
 #pragma unroll
     for (int w = 0; w < NWARP; ++w) { const float2 v = *reinterpret_cast<const float2*>(src + (size_t)w * RP * LP); a.x += v.x; a.y += v.y; }
     const int j = 2 * jp;
+    if (cross_only && ((i < 16) == (j < 16))) {      // inside a diagonal block only the diagonal entry was formed (gram_mma_cross)
+      a.x = (j == i) ? a.x : 0.f; a.y = (j + 1 == i) ? a.y : 0.f;
+    }
     W[i * LW + j] = a.x; W[i * LW + j + 1] = a.y;
     if (i < 16 && j >= 16) { W[j * LW + i] = a.x; W[(j + 1) * LW + i] = a.y; }
   }
@@ -612,6 +615,51 @@ __device__ __forceinline__ void gram_mma(const float* X, int ldx, int ks, float*
 // X' = X + E X, E = Q - I (hi / lo parts pre-split in shared memory, fragment order), for this warp's column slice, in place. The tensor core adds into its accumulators with truncation; on Q X that
 // is a bias of ~1e-7 per block round on every row, which BPTT through 200 iterations amplified to wrong gradients (measured:
 // cfg5 gradient error 0.48). On E X it is 1e-7 of the correction only, and the correction is small once the sweeps converge.
+// The cross block only (rows 0-15 against rows 16-31: tiles (0,2), (0,3)) and the 32 diagonal entries, for the visits that
+// rotate cross pairs only (block-cyclic ordering, see the kernel): a third of the mma of gram_mma. The diagonal entries are
+// plain fp32 sums of squares of the fragments the thread holds anyway (lanes t = 0..3 of a row group add by shuffle); the
+// entries inside the two diagonal blocks are NOT written (gram_reduce takes them as zero: they are of second order after the
+// block's round-0 visit, and an error there only perturbs the angles of later inner rounds, not the orthogonality of Q).
+__device__ __forceinline__ void gram_mma_cross(const float* X, int ldx, int ks, float* part) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  float accM[2][4], accS[2][4], sq[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+  for (int i = 0; i < 2; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { accM[i][j] = 0.f; accS[i][j] = 0.f; }
+  const float* xb = X + (size_t)g * ldx + warp * ks + t;
+  for (int kk = 0; kk < ks; kk += 8) {
+    uint32_t h[4][2], l[4][2];
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+      const float x0 = xb[(size_t)(8 * a) * ldx + kk], x1 = xb[(size_t)(8 * a) * ldx + kk + 4];
+      sq[a] = fmaf(x0, x0, fmaf(x1, x1, sq[a]));
+      split_fast(x0, h[a][0], l[a][0]);
+      split_fast(x1, h[a][1], l[a][1]);
+    }
+#pragma unroll
+    for (int n = 0; n < 2; ++n) {      // m tile 0 (rows g, g + 8), n tiles 2, 3 (rows 16 + g, 24 + g)
+      mma_tf32(accS[n], l[0][0], l[1][0], l[0][1], l[1][1], h[2 + n][0], h[2 + n][1]);
+      mma_tf32(accS[n], h[0][0], h[1][0], h[0][1], h[1][1], l[2 + n][0], l[2 + n][1]);
+      mma_tf32(accM[n], h[0][0], h[1][0], h[0][1], h[1][1], h[2 + n][0], h[2 + n][1]);
+    }
+  }
+  float* pw = part + (size_t)warp * RP * LP;
+#pragma unroll
+  for (int n = 0; n < 2; ++n) {
+    const int c0 = 8 * (2 + n) + 2 * t;
+    *reinterpret_cast<float2*>(pw + g * LP + c0) = make_float2(accM[n][0] + accS[n][0], accM[n][1] + accS[n][1]);
+    *reinterpret_cast<float2*>(pw + (g + 8) * LP + c0) = make_float2(accM[n][2] + accS[n][2], accM[n][3] + accS[n][3]);
+  }
+#pragma unroll
+  for (int a = 0; a < 4; ++a) {
+    float v = sq[a];
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    v += __shfl_xor_sync(0xffffffffu, v, 2);
+    if (t == 0) pw[(g + 8 * a) * LP + g + 8 * a] = v;
+  }
+}
+
 // Element (i, k) of E -> its place in the fragment-ordered copies [m tile][k step][lane][4] that apply_mma reads: a thread's
 // four A registers of one mma are one 16-byte piece, a warp's load is 512 contiguous bytes (16 conflict-free LDS.128 per
 // thread instead of 32 LDS.64 that cost 900 cycles more per visit, measured).
@@ -774,6 +822,7 @@ k_bjacobi_tc2(int lb0, int C, const int* pvec, const long long* moff, const int*
   const float quad_exit = (float)sqrt(tol / (16.0 * sqrt((double)p)));
   int sweep = 0;
   bool capped = true;
+  bool small_rot = false;      // the previous sweep met no cosine above 0.1: what cross rotations leave inside a block is negligible
   for (; sweep < max_sweeps; ++sweep) {
     for (int r = 0; r < NBe - 1; ++r) {
       for (int q = rank; q < NP; q += C) {
@@ -782,11 +831,12 @@ k_bjacobi_tc2(int lb0, int C, const int* pvec, const long long* moff, const int*
         if (sliced) load_slice_t<8>(g, p, bi, bj2, X, ldx);
         else { load_pair(g, p, bi, bj2, X, ldx); __syncthreads(); }
         BW_T(0);
-        gram_mma(X, ldx, ks, part);
+        const bool cross_only = r > 0 && small_rot;
+        if (cross_only) gram_mma_cross(X, ldx, ks, part); else gram_mma(X, ldx, ks, part);
         __syncthreads();
         BW_T(1);
         unsigned active;
-        const float mx2 = gram_reduce(part, W, red, rtab, lim2, active);
+        const float mx2 = gram_reduce(part, W, red, rtab, lim2, active, cross_only);
         // block-cyclic ordering: the pairs inside a block are rotated at the block's visit of round 0 (every block has one), the
         // other 30 visits of a sweep rotate the 256 cross pairs only; what those leave inside a block is of second order
         if (r > 0) active &= 0xffffu;
@@ -814,6 +864,7 @@ k_bjacobi_tc2(int lb0, int C, const int* pvec, const long long* moff, const int*
       BW_T(5);
     }
     const unsigned worst = (unsigned)__ldcg(rf + sweep);     // largest |w_ij| / sqrt(w_ii w_jj) any pair showed in this sweep
+    small_rot = __uint_as_float(worst) <= 0.1f;
     if (!worst) { capped = false; break; }
     if (__uint_as_float(worst) <= quad_exit) { ++sweep; capped = false; break; }
   }
