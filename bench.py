@@ -376,17 +376,25 @@ def run_config(cfg, args, cdu, torch, dist, peaks, world, rank, local, ckpt, opt
             # eigendecomposition = the first pass plus the (mostly skipped) polish pass: time per decomposition, not per launch
             ndec = nprof * wl.K * (1 if full else 2)
             dur = prof[kc]["ms"] * 1e-3 / ndec
-            fl = float(np.mean([8.0 * (1.0 - 16.0 / p) * p ** 3 for p in ps])) * st["eig_sweeps_sum"] / wl.K
             f32 = wl.dtype == "f32"
+            spm = st["eig_sweeps_sum"] / max(1, wl.K * len(ps))                 # sweeps per matrix
+            fl_full = float(np.mean([8.0 * (1.0 - 16.0 / p) * p ** 3 for p in ps]))   # one sweep, full 32 x 32 Gram + apply per block pair
+            # fp32 kernel, block-cyclic ordering: after the first sweep only the round-0 visit of a block pair forms the full Gram
+            # matrix (2 * 32 * 32 * p), the other NB - 2 visits the 16 x 16 cross block and the 32 row norms (576 p); apply 2048 p
+            fl_red = float(np.mean([(p / 32.0) * 4096.0 * p + (p / 32.0) * (p / 16.0 - 2.0) * 2624.0 * p for p in ps])) if f32 else fl_full
+            fl_textbook = fl_full * st["eig_sweeps_sum"] / wl.K
+            fl = (fl_full + max(0.0, spm - 1.0) * fl_red) * len(ps) if spm >= 1.0 else fl_textbook
             pk = peaks["tf32_mma_sync_tflops"] if f32 else peaks["fp64_tflops"]
             ach = fl / dur / 1e12
             r = dict(kernel=kc, bound="tensor" if f32 else "alu", achieved=ach, peak=pk, unit="TFLOP/s", frac=(3.0 if f32 else 1.0) * ach / pk,
                      traffic=traffic_of(kc), executed=(3.0 if f32 else 1.0) * ach,
                      peak_source="measured in this process (cdu_measure_peak: warp-level mma.sync m16n8k8 tf32, the path these products run on)" if f32
                      else "measured in this process (cdu_measure_peak)",
-                     sweeps_per_matrix=st["eig_sweeps_sum"] / max(1, wl.K * len(ps)),
-                     note="achieved = algorithmic flops of the Gram + apply products counted as if every block pair rotated; executed = 3 x "
-                          "(3xTF32); frac = executed / peak. The kernel is bound by the dependent chain of its Jacobi rounds (load, Gram, "
+                     sweeps_per_matrix=spm, achieved_full_gram_count=fl_textbook / dur / 1e12,
+                     note="achieved = flops of the Gram + apply products the block-cyclic method needs, counted as if every block pair "
+                          "rotated (first sweep: full 32x32 Gram per visit; later sweeps: full Gram at the round-0 visit, cross block + row "
+                          "norms otherwise); achieved_full_gram_count = the same time against a full Gram at every visit (the count of "
+                          "earlier rounds); executed = 3 x achieved (3xTF32); frac = executed / peak. The kernel is bound by the dependent chain of its Jacobi rounds (load, Gram, "
                           "32x32 sweep, apply, barrier per block round), not by the tensor pipe (DESIGN.md section 7); avg_launch_ms = "
                           "time per batch of eigendecompositions (first pass + polish pass)")
         else:
