@@ -862,6 +862,9 @@ k_bjacobi_tc2(int lb0, int C, const int* pvec, const long long* moff, const int*
       BW_T0();
       matrix_barrier(ctr, gen, C);
       BW_T(5);
+      // first sweep: round 0 has shown every block once (a thirty-first of the pairs); if no cosine there exceeded 0.03 the
+      // rotations of this sweep are small already (a good warm start) and the other rounds form the cross block only
+      if (sweep == 0 && r == 0) small_rot = __uint_as_float((unsigned)__ldcg(rf)) <= 0.03f;
     }
     const unsigned worst = (unsigned)__ldcg(rf + sweep);     // largest |w_ij| / sqrt(w_ii w_jj) any pair showed in this sweep
     small_rot = __uint_as_float(worst) <= 0.1f;
